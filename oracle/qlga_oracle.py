@@ -1,0 +1,166 @@
+"""ctypes front-end of the CPU oracle (oracle/qlga_oracle.c).
+
+TEST INFRASTRUCTURE, NOT THE PRODUCT: only tests/, __graft_entry__.smoke() and
+bench.py's cpu_baseline / --impl reference legs may import this module.  It never
+imports the CUDA package and the CUDA package never imports it.
+
+`Oracle(precision="double" | "longdouble")` wraps one build of the C file;
+arrays are numpy complex128 (or clongdouble) in the layout q[5][2][Ny][Nx].
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+import subprocess
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "qlga_oracle.c")
+_LIBS = {"double": ("libqlga_oracle.so", []),
+         "longdouble": ("libqlga_oracle_ld.so", ['-DREAL=long double'])}
+
+OBS_FIELDS = ("n_p2", "n_p1", "n_0", "n_m1", "n_m2", "norm_psi", "norm_q",
+              "F_x", "F_y", "F_z", "A00_re", "A00_im", "A00_abs2",
+              "e_kin", "e_c0", "e_c1", "e_c2", "e_total", "e_dt_re", "e_dt_im")
+
+
+def build(force: bool = False) -> None:
+    """Compile the oracle's C file (both precisions) with gcc; no FMA contraction."""
+    for lib, defs in _LIBS.values():
+        out = os.path.join(_HERE, lib)
+        if (not force and os.path.exists(out)
+                and os.path.getmtime(out) >= os.path.getmtime(_SRC)):
+            continue
+        cmd = ["gcc", "-O2", "-std=c11", "-ffp-contract=off", "-fcx-limited-range", "-fPIC", "-shared",
+               *defs, _SRC, "-o", out, "-lm"]
+        subprocess.run(cmd, check=True)
+
+
+class Oracle:
+    def __init__(self, precision: str = "double"):
+        build()
+        self.precision = precision
+        self.lib = ctypes.CDLL(os.path.join(_HERE, _LIBS[precision][0]))
+        if precision == "double":
+            self.ctype, self.rtype, self.creal = np.complex128, np.float64, ctypes.c_double
+        else:
+            self.ctype, self.rtype, self.creal = np.clongdouble, np.longdouble, ctypes.c_longdouble
+        self.lib.orc_sizeof_real.restype = ctypes.c_size_t
+        assert self.lib.orc_sizeof_real() == np.dtype(self.rtype).itemsize
+        L, I, P, R = ctypes.c_long, ctypes.c_int, ctypes.c_void_p, self.creal
+        sig = {
+            "orc_split_psi": [P, P, L, L],
+            "orc_psi_of_q": [P, P, L, L],
+            "orc_collide": [P, L, L],
+            "orc_stream": [P, L, L, I, I, I],
+            "orc_kinetic_factor": [P, L, L, I, I],
+            "orc_spin_matrices": [P, P, P],
+            "orc_site_hamiltonian": [P, R, R, R, P],
+            "orc_interaction": [P, L, L, R, R, R, R],
+            "orc_step": [P, L, L, I, R, R, R, I, L],
+            "orc_observables": [P, P, L, L, I, R, R, R, P],
+            "orc_vorticity": [P, L, L, P],
+        }
+        for name, args in sig.items():
+            fn = getattr(self.lib, name)
+            fn.argtypes = args
+            fn.restype = None
+
+    # -- helpers ---------------------------------------------------------
+    def _c(self, a, shape=None):
+        a = np.ascontiguousarray(a, dtype=self.ctype)
+        if shape is not None:
+            assert a.shape == tuple(shape), (a.shape, shape)
+        return a
+
+    @staticmethod
+    def _p(a):
+        return a.ctypes.data_as(ctypes.c_void_p)
+
+    @staticmethod
+    def _dims(q):
+        assert q.ndim == 4 and q.shape[0] == 5 and q.shape[1] == 2, q.shape
+        return q.shape[3], q.shape[2]
+
+    # -- operators (each returns a new array) ------------------------------
+    def split_psi(self, psi):
+        psi = self._c(psi)
+        _, ny, nx = psi.shape
+        q = np.empty((5, 2, ny, nx), dtype=self.ctype)
+        self.lib.orc_split_psi(self._p(psi), self._p(q), nx, ny)
+        return q
+
+    def psi_of_q(self, q):
+        q = self._c(q)
+        nx, ny = self._dims(q)
+        psi = np.empty((5, ny, nx), dtype=self.ctype)
+        self.lib.orc_psi_of_q(self._p(q), self._p(psi), nx, ny)
+        return psi
+
+    def collide(self, q):
+        q = self._c(q).copy()
+        nx, ny = self._dims(q)
+        self.lib.orc_collide(self._p(q), nx, ny)
+        return q
+
+    def stream(self, q, d, sigma, transpose=False):
+        q = self._c(q).copy()
+        nx, ny = self._dims(q)
+        self.lib.orc_stream(self._p(q), nx, ny, int(d), int(sigma), int(bool(transpose)))
+        return q
+
+    def kinetic_factor(self, q, d, sigma):
+        q = self._c(q).copy()
+        nx, ny = self._dims(q)
+        self.lib.orc_kinetic_factor(self._p(q), nx, ny, int(d), int(sigma))
+        return q
+
+    def spin_matrices(self):
+        f = [np.empty((5, 5), dtype=self.ctype) for _ in range(3)]
+        self.lib.orc_spin_matrices(*(self._p(a) for a in f))
+        return f
+
+    def site_hamiltonian(self, psi5, couplings):
+        psi5 = self._c(psi5, (5,))
+        H = np.empty((5, 5), dtype=self.ctype)
+        c0, c1, c2 = couplings
+        self.lib.orc_site_hamiltonian(self._p(psi5), self.creal(c0), self.creal(c1),
+                                      self.creal(c2), self._p(H))
+        return H
+
+    def interaction(self, q, couplings, s):
+        q = self._c(q).copy()
+        nx, ny = self._dims(q)
+        c0, c1, c2 = couplings
+        self.lib.orc_interaction(self._p(q), nx, ny, self.creal(c0), self.creal(c1),
+                                 self.creal(c2), self.creal(s))
+        return q
+
+    def step(self, q, ndim, couplings, order, nsteps=1):
+        """order: 0 = plain (eq. 108), 1 = interleaved (eq. 112)."""
+        q = self._c(q).copy()
+        nx, ny = self._dims(q)
+        assert ndim in (1, 2) and (ndim == 2 or ny == 1)
+        c0, c1, c2 = couplings
+        self.lib.orc_step(self._p(q), nx, ny, int(ndim), self.creal(c0), self.creal(c1),
+                          self.creal(c2), int(order), int(nsteps))
+        return q
+
+    def observables(self, q, ndim, couplings, qprev=None):
+        q = self._c(q)
+        nx, ny = self._dims(q)
+        out = np.empty(20, dtype=np.float64)
+        c0, c1, c2 = couplings
+        if qprev is not None:
+            qprev = self._c(qprev, q.shape)
+        self.lib.orc_observables(self._p(q), None if qprev is None else self._p(qprev),
+                                 nx, ny, int(ndim), self.creal(c0), self.creal(c1),
+                                 self.creal(c2), self._p(out))
+        return dict(zip(OBS_FIELDS, out.tolist()))
+
+    def vorticity(self, q):
+        q = self._c(q)
+        nx, ny = self._dims(q)
+        om = np.empty((5, ny, nx), dtype=self.rtype)
+        self.lib.orc_vorticity(self._p(q), nx, ny, self._p(om))
+        return om
