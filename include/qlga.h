@@ -1,0 +1,156 @@
+/*
+ * qlga.h -- C ABI of the B200-native spin-2 BEC quantum lattice gas (QLGA) step.
+ *
+ * Method: arXiv:1907.12834.  Five coupled Gross-Pitaevskii fields
+ * psi_m (m_f = +2..-2, eq. 34/37), each carried by a pair of
+ * spinor amplitudes per lattice site:  psi_m = q_m1 + q_m2.
+ * One time step is the operator product of eq. (108) (plain) or eq. (112)
+ * (interleaved), built from the kinetic factors
+ * I'_i = S_i C S_i^T C of eq. (107) and the local interaction unitary U.
+ * Where the paper is silent the readings R1..R11 of DESIGN.md apply.
+ *
+ * All entry points are plain C, take plain pointers and sizes, return a status
+ * and never throw or abort.  Pointers are marked HOST or DEVICE below.  Device
+ * buffers and the CUDA stream are owned by the caller (e.g. torch tensors and a
+ * torch stream); the library only allocates small reduction / staging scratch
+ * of its own and frees it in qlga_destroy.  All work is enqueued on the caller's
+ * stream; calls that return data to the host synchronise that stream.
+ *
+ * Data layout (both for the caller's transfers and inside the device buffers):
+ *   q   : [5][2][Ny][Nx] complex   index ((j*2 + sigma)*Ny + y)*Nx + x
+ *   psi : [5][Ny][Nx]    complex
+ *   omega : [5][Ny][Nx]  real
+ *   j = 0..4 <-> m_f = +2,+1,0,-1,-2;  sigma = 0,1 <-> spinor component 1,2;
+ *   x fastest; Ny = 1 in 1D; complex = interleaved (re, im) of the context's real
+ *   type (double for QLGA_F64, float for QLGA_F32); lattice periodic in x and y.
+ */
+#ifndef QLGA_H
+#define QLGA_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct qlga_ctx qlga_ctx;   /* opaque, owned by the library */
+
+typedef enum {
+    QLGA_OK = 0,
+    QLGA_EINVAL = 1,   /* bad argument; no side effect                        */
+    QLGA_ENOMEM = 2,   /* host or device allocation of library scratch failed */
+    QLGA_ECUDA = 3,    /* CUDA error; text in qlga_last_error                 */
+    QLGA_ESTATE = 4,   /* call not valid in the current state (no state set)  */
+    QLGA_EUNSUP = 5    /* not supported for this context (e.g. vorticity in 1D) */
+} qlga_status;
+
+typedef enum { QLGA_F64 = 0, QLGA_F32 = 1 } qlga_prec;
+
+/* Operator ordering of one time step (rightmost operator acts first):
+ *   QLGA_PLAIN        eq. (108):  I'_x1 I'_x1 I'_x2 I'_x2 [I'_y1 I'_y1 I'_y2 I'_y2] U
+ *   QLGA_INTERLEAVED  eq. (112):  every I' preceded by U^{1/(4 ndim)}, "n = 8" in 2D
+ *                                 (PAPER.md:1064).  The y factors act before the x factors (R7). */
+typedef enum { QLGA_PLAIN = 0, QLGA_INTERLEAVED = 1 } qlga_order;
+
+/* Tunables of qlga_set_option. */
+typedef enum {
+    QLGA_OPT_PATH = 0,        /* 0 = fused pass kernels (default), 1 = one kernel per operator   */
+    QLGA_OPT_STEPS_PER_LAUNCH = 1, /* 1D only: time steps fused per launch (halo 4 per step); 0 = auto */
+    QLGA_OPT_EXP_TOL_LOG2 = 2,/* truncation target of the interaction exponential, log2 (default -56 / -27) */
+    QLGA_OPT_THREADS_X = 3,   /* CTA size of the x pass: 128 or 256; 0 = auto                    */
+    QLGA_OPT_TILE_Y = 4       /* y pass: columns per CTA (1,2,4,8); 0 = auto                     */
+} qlga_option;
+
+/* Lattice sums returned by qlga_observables (always double).
+ *   n_m[j]   = sum_r |psi_m|^2                                   eq. (3)
+ *   norm_psi = sum_m n_m ;  norm_q = sum_{r,m,sigma} |q|^2  (the unitary invariant)
+ *   F[3]     = sum_r <psi|f_nu|psi>, nu = x,y,z                  eq. (5), (59)-(60)
+ *   A00      = sum_r A00(r), A00(r) = (2 psi_2 psi_-2 - 2 psi_1 psi_-1 + psi_0^2)/sqrt(5)   eq. (4), (35)
+ *   A00_abs2 = sum_r |A00(r)|^2
+ *   e_kin    = sum_r sum_m sum_d |psi_m(r+e_d) - psi_m(r)|^2     (eq. 12 with hbar = 1, m = 1/2)
+ *   e_c0, e_c1, e_c2 = (c0/2) sum rho^2, (c1/2) sum |F|^2, (c2/2) sum |A00|^2   eq. (32)
+ *   e_total  = e_kin + e_c0 + e_c1 + e_c2
+ *   e_dt     = i(<psi(t)|psi(t)> - <psi(t)|psi(t-tau)>)/<psi(t)|psi(t)>        eq. (85), PAPER.md:666;
+ *              NaN unless the previous step's state is still held (see qlga_init).
+ *   step     = number of time steps taken since the last qlga_set_state_*.        */
+typedef struct {
+    double n_m[5];
+    double norm_psi, norm_q;
+    double F[3];
+    double A00_re, A00_im, A00_abs2;
+    double e_kin, e_c0, e_c1, e_c2, e_total;
+    double e_dt_re, e_dt_im;
+    int64_t step;
+} qlga_obs;
+
+/* Create a context (BASELINE.json north_star "qlga_init").
+ *   out        HOST  receives the context.
+ *   ndim       1 or 2.        dims  HOST  {Nx, Ny}; Ny must be 1 when ndim == 1; Nx, Ny >= 1.
+ *   c0,c1,c2   the paper's g0, g1, g2 of eq. (32)-(34).
+ *   dev_buf_a, dev_buf_b   DEVICE, caller-owned, 16-byte aligned, each >= qlga_state_bytes().
+ *   dev_buf_c  DEVICE or NULL.  Optional third buffer: in 2D a step is two passes
+ *              (a -> b -> c), so the state of the previous step survives only with a
+ *              third buffer; without it e_dt is NaN in 2D.  Unused in 1D.
+ *   buf_bytes  size of each buffer.
+ *   cuda_stream  the caller's cudaStream_t (NULL = legacy default stream).
+ * Errors: QLGA_EINVAL (arguments), QLGA_ECUDA (no sm_100 device / CUDA failure), QLGA_ENOMEM. */
+qlga_status qlga_init(qlga_ctx** out, int ndim, const int64_t dims[2],
+                      double c0, double c1, double c2, qlga_order order, qlga_prec prec,
+                      void* dev_buf_a, void* dev_buf_b, void* dev_buf_c, size_t buf_bytes,
+                      void* cuda_stream);
+
+/* Bytes one state buffer needs: 10 * Nx * Ny * 2 * sizeof(real).  0 on bad arguments. */
+size_t qlga_state_bytes(int ndim, const int64_t dims[2], qlga_prec prec);
+
+/* Set a tunable (see qlga_option).  QLGA_EINVAL for unknown keys / bad values. */
+qlga_status qlga_set_option(qlga_ctx*, qlga_option key, int64_t value);
+
+/* Load the bosonic field: q_m1 = q_m2 = psi_m / 2 (reading R6).  psi: HOST or DEVICE
+ * ([5][Ny][Nx] complex of the context's real type) per src_on_device.  Resets step to 0. */
+qlga_status qlga_set_state_psi(qlga_ctx*, const void* psi, int src_on_device);
+/* Load / read back the full spinor state q ([5][2][Ny][Nx] complex); also the checkpoint format. */
+qlga_status qlga_set_state_q(qlga_ctx*, const void* q, int src_on_device);
+qlga_status qlga_get_state_q(qlga_ctx*, void* q, int dst_on_device);
+/* Read back psi_m = q_m1 + q_m2. */
+qlga_status qlga_get_state_psi(qlga_ctx*, void* psi, int dst_on_device);
+
+/* Advance n >= 0 time steps of eq. (108)/(112).  Asynchronous on the stream. */
+qlga_status qlga_step(qlga_ctx*, int64_t n);
+
+/* Lattice sums of the current state; host_out HOST.  Synchronises the stream. */
+qlga_status qlga_observables(qlga_ctx*, qlga_obs* host_out);
+
+/* Lattice vorticity, 2D only (eq. 99-104, reading R8), per m:
+ *   v_x(r) = (1/2) arg(psi(r+e_x) psi*(r-e_x)),  v_y(r) = (1/2) arg(psi(r+e_y) psi*(r-e_y)),
+ *   omega(r) = (1/2)[v_y(r+e_x) - v_y(r-e_x) - v_x(r+e_y) + v_x(r-e_y)],   arg(0) := 0.
+ * omega: HOST or DEVICE [5][Ny][Nx] real of the context's real type.  QLGA_EUNSUP in 1D. */
+qlga_status qlga_vorticity(qlga_ctx*, void* omega, int dst_on_device);
+
+/* Kernel timing hooks (used by bench.py for the roofline of the dominant kernel).
+ * While enabled, qlga_step records a CUDA event on the caller's stream before every
+ * pass kernel and one after the last; qlga_profile_read synchronises the stream,
+ * returns the summed durations and launch counts per kernel kind since the last
+ * read (0: x pass, 1: y pass, 2: per-operator kernels) and resets them.  At most
+ * 4096 launches are recorded between two reads; later ones are not timed. */
+typedef struct { double ms[3]; int64_t launches[3]; } qlga_profile;
+qlga_status qlga_profile_enable(qlga_ctx*, int on);
+qlga_status qlga_profile_read(qlga_ctx*, qlga_profile* host_out);
+
+/* Number of kernels this context has launched so far (for bench.py's gpu_launches). */
+int64_t qlga_launch_count(const qlga_ctx*);
+
+/* Text of the last error of this context (or of the failed qlga_init when ctx == NULL).
+ * Owned by the library; valid until the next call on the same context. */
+const char* qlga_last_error(const qlga_ctx*);
+
+/* Free the context and the library's scratch.  Never frees caller buffers. */
+qlga_status qlga_destroy(qlga_ctx*);
+
+/* Library version string, e.g. "qlga-b200 0.1 (sm_100a)". */
+const char* qlga_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* QLGA_H */

@@ -1,0 +1,447 @@
+// qlga_api.cu -- the C ABI of libqlga.so (include/qlga.h): context, sequencing of
+// the fused passes into time steps, state transfers, observables, vorticity.
+#include <math.h>
+#include <stdio.h>
+#include <stdlib.h>
+#include <string.h>
+#include <new>
+#include "qlga_internal.h"
+
+using namespace qlga;
+
+static char g_init_err[512] = "";
+
+static qlga_status fail(qlga_ctx* c, qlga_status st, const char* fmt, const char* a = "") {
+    char* dst = c ? c->err : g_init_err;
+    snprintf(dst, 512, fmt, a);
+    return st;
+}
+static qlga_status cuda_fail(qlga_ctx* c, const char* what, cudaError_t e) {
+    char* dst = c ? c->err : g_init_err;
+    snprintf(dst, 512, "%s: %s", what, cudaGetErrorString(e));
+    return QLGA_ECUDA;
+}
+#define CU(ctx, call)                                                       \
+    do {                                                                    \
+        cudaError_t e_ = (call);                                            \
+        if (e_ != cudaSuccess) return cuda_fail(ctx, #call, e_);            \
+    } while (0)
+
+static size_t real_size(qlga_prec p) { return p == QLGA_F64 ? sizeof(double) : sizeof(float); }
+
+// thresholds of the interaction polynomial: a degree-p Taylor polynomial of
+// exp(-i s K) has remainder <= theta^(p+1)/(p+1)!; thr[p-1] is the largest theta
+// for which that is below tol = 2^tol_log2.
+static void build_exp_table(ExpTable& tab, int tol_log2) {
+    const double tol = ldexp(1.0, tol_log2);
+    tab.rcp[0] = 0.0;
+    for (int k = 1; k < QLGA_PMAX + 2; ++k) tab.rcp[k] = 1.0 / (double)k;
+    double fact = 1.0;                       // (p+1)!
+    for (int p = 1; p <= QLGA_PMAX; ++p) {
+        fact = 1.0;
+        for (int k = 2; k <= p + 1; ++k) fact *= (double)k;
+        const double th = pow(tol * fact, 1.0 / (double)(p + 1));
+        tab.thr[p - 1] = (float)(th * 0.999);
+    }
+    const double top = tab.thr[QLGA_PMAX - 1];
+    tab.theta_split = (float)(top < 0.5 ? top : 0.5);
+}
+
+extern "C" const char* qlga_version(void) { return "qlga-b200 0.1 (sm_100a)"; }
+
+extern "C" size_t qlga_state_bytes(int ndim, const int64_t dims[2], qlga_prec prec) {
+    if (!dims || (ndim != 1 && ndim != 2)) return 0;
+    if (dims[0] < 1 || dims[1] < 1 || (ndim == 1 && dims[1] != 1)) return 0;
+    if (prec != QLGA_F64 && prec != QLGA_F32) return 0;
+    return (size_t)10 * (size_t)dims[0] * (size_t)dims[1] * 2 * real_size(prec);
+}
+
+extern "C" qlga_status qlga_init(qlga_ctx** out, int ndim, const int64_t dims[2],
+                                 double c0, double c1, double c2, qlga_order order, qlga_prec prec,
+                                 void* dev_buf_a, void* dev_buf_b, void* dev_buf_c, size_t buf_bytes,
+                                 void* cuda_stream) {
+    if (!out) return fail(nullptr, QLGA_EINVAL, "qlga_init: out is NULL");
+    *out = nullptr;
+    const size_t need = qlga_state_bytes(ndim, dims, prec);
+    if (need == 0) return fail(nullptr, QLGA_EINVAL, "qlga_init: bad ndim/dims/prec");
+    if (order != QLGA_PLAIN && order != QLGA_INTERLEAVED)
+        return fail(nullptr, QLGA_EINVAL, "qlga_init: bad order");
+    if (!isfinite(c0) || !isfinite(c1) || !isfinite(c2))
+        return fail(nullptr, QLGA_EINVAL, "qlga_init: non-finite coupling");
+    if (!dev_buf_a || !dev_buf_b || dev_buf_a == dev_buf_b || buf_bytes < need)
+        return fail(nullptr, QLGA_EINVAL, "qlga_init: need two distinct device buffers of qlga_state_bytes()");
+    if (((uintptr_t)dev_buf_a | (uintptr_t)dev_buf_b | (uintptr_t)dev_buf_c) & 15)
+        return fail(nullptr, QLGA_EINVAL, "qlga_init: device buffers must be 16-byte aligned");
+    if (dev_buf_c && (dev_buf_c == dev_buf_a || dev_buf_c == dev_buf_b))
+        return fail(nullptr, QLGA_EINVAL, "qlga_init: dev_buf_c aliases another buffer");
+    if (dims[0] * dims[1] > (int64_t)1 << 40)
+        return fail(nullptr, QLGA_EINVAL, "qlga_init: lattice too large");
+
+    int dev = 0;
+    cudaDeviceProp prop;
+    CU(nullptr, cudaGetDevice(&dev));
+    CU(nullptr, cudaGetDeviceProperties(&prop, dev));
+    if (prop.major < 10) return fail(nullptr, QLGA_ECUDA, "qlga_init: the library is built for sm_100a only");
+
+    qlga_ctx* c = new (std::nothrow) qlga_ctx;
+    if (!c) return fail(nullptr, QLGA_ENOMEM, "qlga_init: out of host memory");
+    memset(c, 0, sizeof(*c));
+    c->ndim = ndim; c->nx = dims[0]; c->ny = dims[1];
+    c->c[0] = c0; c->c[1] = c1; c->c[2] = c2;
+    c->order = order; c->prec = prec;
+    c->buf[0] = dev_buf_a; c->buf[1] = dev_buf_b; c->buf[2] = dev_buf_c;
+    c->buf_bytes = buf_bytes;
+    c->stream = (cudaStream_t)cuda_stream;
+    c->cur = 0; c->prev = -1; c->have_state = 0; c->step = 0; c->launches = 0;
+    c->path = 0; c->steps_per_launch = 0; c->threads_x = 0; c->tile_y = 0;
+    c->tol_log2 = (prec == QLGA_F64) ? -56 : -27;
+    build_exp_table(c->tab, c->tol_log2);
+    c->obs_blocks = prop.multiProcessorCount * 8;
+    cudaError_t e = cudaMalloc(&c->d_partials, sizeof(double) * (size_t)c->obs_blocks * OBS_NACC);
+    if (e == cudaSuccess) e = cudaMalloc(&c->d_sums, sizeof(double) * OBS_NACC);
+    if (e != cudaSuccess) {
+        cudaFree(c->d_partials);
+        delete c;
+        return cuda_fail(nullptr, "qlga_init: cudaMalloc(scratch)", e);
+    }
+    c->d_stage = nullptr; c->stage_bytes = 0;
+    c->err[0] = 0;
+    *out = c;
+    return QLGA_OK;
+}
+
+extern "C" qlga_status qlga_destroy(qlga_ctx* c) {
+    if (!c) return QLGA_EINVAL;
+    cudaStreamSynchronize(c->stream);
+    cudaFree(c->d_partials); cudaFree(c->d_sums); cudaFree(c->d_stage);
+    if (c->prof_ev) {
+        for (int k = 0; k < PROF_CAP; ++k) cudaEventDestroy(c->prof_ev[k]);
+        free(c->prof_ev); free(c->prof_kind);
+    }
+    delete c;
+    return QLGA_OK;
+}
+
+extern "C" const char* qlga_last_error(const qlga_ctx* c) { return c ? c->err : g_init_err; }
+extern "C" int64_t qlga_launch_count(const qlga_ctx* c) { return c ? c->launches : -1; }
+
+extern "C" qlga_status qlga_set_option(qlga_ctx* c, qlga_option key, int64_t v) {
+    if (!c) return QLGA_EINVAL;
+    switch (key) {
+        case QLGA_OPT_PATH:
+            if (v != 0 && v != 1) return fail(c, QLGA_EINVAL, "QLGA_OPT_PATH: 0 or 1");
+            c->path = (int)v; return QLGA_OK;
+        case QLGA_OPT_STEPS_PER_LAUNCH:
+            if (v < 0 || v > 64) return fail(c, QLGA_EINVAL, "QLGA_OPT_STEPS_PER_LAUNCH: 0..64");
+            c->steps_per_launch = (int)v; return QLGA_OK;
+        case QLGA_OPT_EXP_TOL_LOG2:
+            if (v > -8 || v < -100) return fail(c, QLGA_EINVAL, "QLGA_OPT_EXP_TOL_LOG2: -100..-8");
+            c->tol_log2 = (int)v; build_exp_table(c->tab, c->tol_log2); return QLGA_OK;
+        case QLGA_OPT_THREADS_X:
+            if (v != 0 && v != 128 && v != 256) return fail(c, QLGA_EINVAL, "QLGA_OPT_THREADS_X: 0, 128, 256");
+            c->threads_x = (int)v; return QLGA_OK;
+        case QLGA_OPT_TILE_Y:
+            if (v != 0 && v != 1 && v != 2 && v != 4 && v != 8) return fail(c, QLGA_EINVAL, "QLGA_OPT_TILE_Y: 0,1,2,4,8");
+            c->tile_y = (int)v; return QLGA_OK;
+    }
+    return fail(c, QLGA_EINVAL, "qlga_set_option: unknown key");
+}
+
+// ---------------------------------------------------------------------------
+// kernel timing hooks
+// ---------------------------------------------------------------------------
+static inline void prof_mark(qlga_ctx* c, int kind) {
+    if (!c->prof_on || c->prof_n >= PROF_CAP) return;
+    if (kind < 0 && (c->prof_n == 0 || c->prof_kind[c->prof_n - 1] < 0)) return;   // nothing to close
+    if (cudaEventRecord(c->prof_ev[c->prof_n], c->stream) != cudaSuccess) { cudaGetLastError(); return; }
+    c->prof_kind[c->prof_n++] = (signed char)kind;
+}
+
+extern "C" qlga_status qlga_profile_enable(qlga_ctx* c, int on) {
+    if (!c) return QLGA_EINVAL;
+    if (on && !c->prof_ev) {
+        c->prof_ev = (cudaEvent_t*)calloc(PROF_CAP, sizeof(cudaEvent_t));
+        c->prof_kind = (signed char*)calloc(PROF_CAP, 1);
+        if (!c->prof_ev || !c->prof_kind) return fail(c, QLGA_ENOMEM, "qlga_profile_enable: out of host memory");
+        for (int k = 0; k < PROF_CAP; ++k) CU(c, cudaEventCreate(&c->prof_ev[k]));
+    }
+    c->prof_on = on ? 1 : 0;
+    c->prof_n = 0;
+    return QLGA_OK;
+}
+
+extern "C" qlga_status qlga_profile_read(qlga_ctx* c, qlga_profile* out) {
+    if (!c || !out) return c ? fail(c, QLGA_EINVAL, "qlga_profile_read: NULL") : QLGA_EINVAL;
+    memset(out, 0, sizeof(*out));
+    CU(c, cudaStreamSynchronize(c->stream));
+    for (int k = 0; k + 1 < c->prof_n; ++k) {
+        const int kind = c->prof_kind[k];
+        if (kind < 0) continue;
+        float ms = 0.f;
+        CU(c, cudaEventElapsedTime(&ms, c->prof_ev[k], c->prof_ev[k + 1]));
+        out->ms[kind] += ms;
+        out->launches[kind] += 1;
+    }
+    c->prof_n = 0;
+    return QLGA_OK;
+}
+
+// ---------------------------------------------------------------------------
+// state transfers
+// ---------------------------------------------------------------------------
+static size_t state_bytes(const qlga_ctx* c) { return (size_t)10 * c->nx * c->ny * 2 * real_size(c->prec); }
+
+static qlga_status ensure_stage(qlga_ctx* c) {
+    if (c->d_stage) return QLGA_OK;
+    const size_t full = state_bytes(c) / 2;                // one psi array
+    size_t want = (size_t)64 << 20;
+    if (want > full) want = full;
+    want = (want + 255) & ~(size_t)255;
+    cudaError_t e = cudaMalloc(&c->d_stage, want);
+    if (e != cudaSuccess) { cudaGetLastError(); return fail(c, QLGA_ENOMEM, "cudaMalloc(staging) failed"); }
+    c->stage_bytes = want;
+    return QLGA_OK;
+}
+
+extern "C" qlga_status qlga_set_state_q(qlga_ctx* c, const void* q, int src_on_device) {
+    if (!c || !q) return c ? fail(c, QLGA_EINVAL, "qlga_set_state_q: NULL") : QLGA_EINVAL;
+    CU(c, cudaMemcpyAsync(c->buf[0], q, state_bytes(c),
+                          src_on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, c->stream));
+    if (!src_on_device) CU(c, cudaStreamSynchronize(c->stream));   // host buffer may be reused on return
+    c->cur = 0; c->prev = -1; c->have_state = 1; c->step = 0;
+    return QLGA_OK;
+}
+
+extern "C" qlga_status qlga_get_state_q(qlga_ctx* c, void* q, int dst_on_device) {
+    if (!c || !q) return c ? fail(c, QLGA_EINVAL, "qlga_get_state_q: NULL") : QLGA_EINVAL;
+    if (!c->have_state) return fail(c, QLGA_ESTATE, "qlga_get_state_q: no state set");
+    CU(c, cudaMemcpyAsync(q, c->buf[c->cur], state_bytes(c),
+                          dst_on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost, c->stream));
+    CU(c, cudaStreamSynchronize(c->stream));
+    return QLGA_OK;
+}
+
+extern "C" qlga_status qlga_set_state_psi(qlga_ctx* c, const void* psi, int src_on_device) {
+    if (!c || !psi) return c ? fail(c, QLGA_EINVAL, "qlga_set_state_psi: NULL") : QLGA_EINVAL;
+    const int64_t n = c->nx * c->ny;
+    Launch L{c->stream, &c->launches};
+    if (src_on_device) {
+        CU(c, launch_split_psi(L, c->prec, psi, c->buf[0], n, 0, n));
+    } else {
+        qlga_status st = ensure_stage(c);
+        if (st != QLGA_OK) return st;
+        const size_t cb = 2 * real_size(c->prec);                      // bytes per complex
+        const int64_t chunk = (int64_t)(c->stage_bytes / (5 * cb));
+        for (int64_t off = 0; off < n; off += chunk) {
+            const int64_t cnt = (n - off < chunk) ? n - off : chunk;
+            for (int j = 0; j < 5; ++j)
+                CU(c, cudaMemcpyAsync((char*)c->d_stage + (size_t)j * cnt * cb,
+                                      (const char*)psi + ((size_t)j * n + off) * cb, (size_t)cnt * cb,
+                                      cudaMemcpyHostToDevice, c->stream));
+            CU(c, launch_split_psi(L, c->prec, c->d_stage, c->buf[0], n, off, cnt));
+        }
+        CU(c, cudaStreamSynchronize(c->stream));
+    }
+    c->cur = 0; c->prev = -1; c->have_state = 1; c->step = 0;
+    return QLGA_OK;
+}
+
+extern "C" qlga_status qlga_get_state_psi(qlga_ctx* c, void* psi, int dst_on_device) {
+    if (!c || !psi) return c ? fail(c, QLGA_EINVAL, "qlga_get_state_psi: NULL") : QLGA_EINVAL;
+    if (!c->have_state) return fail(c, QLGA_ESTATE, "qlga_get_state_psi: no state set");
+    const int64_t n = c->nx * c->ny;
+    Launch L{c->stream, &c->launches};
+    if (dst_on_device) {
+        CU(c, launch_sum_psi(L, c->prec, c->buf[c->cur], psi, n, 0, n));
+    } else {
+        qlga_status st = ensure_stage(c);
+        if (st != QLGA_OK) return st;
+        const size_t cb = 2 * real_size(c->prec);
+        const int64_t chunk = (int64_t)(c->stage_bytes / (5 * cb));
+        for (int64_t off = 0; off < n; off += chunk) {
+            const int64_t cnt = (n - off < chunk) ? n - off : chunk;
+            CU(c, launch_sum_psi(L, c->prec, c->buf[c->cur], c->d_stage, n, off, cnt));
+            for (int j = 0; j < 5; ++j)
+                CU(c, cudaMemcpyAsync((char*)psi + ((size_t)j * n + off) * cb,
+                                      (const char*)c->d_stage + (size_t)j * cnt * cb, (size_t)cnt * cb,
+                                      cudaMemcpyDeviceToHost, c->stream));
+        }
+    }
+    CU(c, cudaStreamSynchronize(c->stream));
+    return QLGA_OK;
+}
+
+// ---------------------------------------------------------------------------
+// time stepping
+// ---------------------------------------------------------------------------
+// Constants of the interaction before factor f (0..3) of a pass.  The fused pass
+// defers the factor 1/2 of every kinetic factor, so before factor f the registers
+// hold 2^f q and the quadratic H_int[psi] is 4^f too large: fold 4^-f in.
+static void fill_pass_consts(const qlga_ctx* c, PassParams& P, double s) {
+    for (int f = 0; f < 4; ++f) {
+        const double sc = s * ldexp(1.0, -2 * f);
+        P.g[f][0] = sc * c->c[0];
+        P.g[f][1] = sc * c->c[1];
+        P.g[f][2] = sc * c->c[2] / 5.0;
+    }
+    P.out_scale = 0.0625;
+    P.tab = c->tab;
+}
+
+static int pick_other(const qlga_ctx* c, int a, int b) {   // a buffer index different from a and b
+    for (int k = 0; k < 3; ++k)
+        if (k != a && k != b && c->buf[k]) return k;
+    return -1;
+}
+
+static qlga_status step_fused(qlga_ctx* c, int64_t nsteps) {
+    Launch L{c->stream, &c->launches};
+    const bool inter = c->order == QLGA_INTERLEAVED;
+    const double s = inter ? 1.0 / (4.0 * c->ndim) : 1.0;
+    PassParams P;
+    P.nx = c->nx; P.ny = c->ny;
+    fill_pass_consts(c, P, s);
+    if (c->ndim == 1) {
+        const int threads = c->threads_x ? c->threads_x : 128;
+        int kmax = c->steps_per_launch;
+        if (kmax == 0) {
+            // auto: temporal blocking only pays when the lattice is too small to fill the GPU
+            kmax = (c->nx <= 262144) ? 4 : 1;
+        }
+        if (kmax > max_ksteps(threads) / 2) kmax = max_ksteps(threads) / 2;
+        if (kmax < 1) kmax = 1;
+        int64_t left = nsteps;
+        while (left > 0) {
+            // keep the very last step a single-step launch so that the previous state
+            // survives in the other buffer for eq. (85)
+            int k = (int)((left - 1 < kmax) ? left - 1 : kmax);
+            if (k < 1) k = 1;
+            const int dst = pick_other(c, c->cur, -1);
+            P.src = c->buf[c->cur]; P.dst = c->buf[dst];
+            P.ksteps = k; P.umode = inter ? 2 : 1;
+            prof_mark(c, 0);
+            CU(c, launch_pass(L, c->prec, 0, P, threads, 1));
+            c->prev = (k == 1) ? c->cur : -1;
+            c->cur = dst;
+            left -= k; c->step += k;
+        }
+        return QLGA_OK;
+    }
+    for (int64_t t = 0; t < nsteps; ++t) {
+        const int mid = pick_other(c, c->cur, -1);                     // any buffer but cur
+        int dst = pick_other(c, c->cur, mid);                          // third buffer if present
+        const bool keep_prev = dst >= 0;
+        if (dst < 0) dst = c->cur;
+        P.ksteps = 1;
+        P.src = c->buf[c->cur]; P.dst = c->buf[mid];
+        P.umode = inter ? 2 : 1;                                       // U is the rightmost operator
+        prof_mark(c, 1);
+        CU(c, launch_pass(L, c->prec, 1, P, 0, c->tile_y));
+        P.src = c->buf[mid]; P.dst = c->buf[dst];
+        P.umode = inter ? 2 : 0;
+        prof_mark(c, 0);
+        CU(c, launch_pass(L, c->prec, 0, P, c->threads_x, 1));
+        c->prev = keep_prev ? c->cur : -1;
+        c->cur = dst;
+        ++c->step;
+    }
+    return QLGA_OK;
+}
+
+static qlga_status step_per_operator(qlga_ctx* c, int64_t nsteps) {
+    Launch L{c->stream, &c->launches};
+    const bool inter = c->order == QLGA_INTERLEAVED;
+    const double s = inter ? 1.0 / (4.0 * c->ndim) : 1.0;
+    const double g[3] = {s * c->c[0], s * c->c[1], s * c->c[2] / 5.0};
+    for (int64_t t = 0; t < nsteps; ++t) {
+        prof_mark(c, 2);
+        if (!inter) CU(c, launch_interaction(L, c->prec, c->buf[c->cur], c->nx, c->ny, g, c->tab));
+        for (int d = c->ndim - 1; d >= 0; --d)
+            for (int k = 0; k < 4; ++k) {
+                const int sigma = (k < 2) ? 1 : 0;                     // components 2, 2, 1, 1
+                if (inter) CU(c, launch_interaction(L, c->prec, c->buf[c->cur], c->nx, c->ny, g, c->tab));
+                const int dst = pick_other(c, c->cur, -1);
+                CU(c, launch_kinetic(L, c->prec, c->buf[c->cur], c->buf[dst], c->nx, c->ny, d, sigma));
+                c->cur = dst;
+            }
+        c->prev = -1;
+        ++c->step;
+    }
+    return QLGA_OK;
+}
+
+extern "C" qlga_status qlga_step(qlga_ctx* c, int64_t n) {
+    if (!c) return QLGA_EINVAL;
+    if (n < 0) return fail(c, QLGA_EINVAL, "qlga_step: n < 0");
+    if (!c->have_state) return fail(c, QLGA_ESTATE, "qlga_step: no state set");
+    if (n == 0) return QLGA_OK;
+    const qlga_status st = c->path == 0 ? step_fused(c, n) : step_per_operator(c, n);
+    prof_mark(c, -1);
+    return st;
+}
+
+// ---------------------------------------------------------------------------
+// diagnostics
+// ---------------------------------------------------------------------------
+extern "C" qlga_status qlga_observables(qlga_ctx* c, qlga_obs* out) {
+    if (!c || !out) return c ? fail(c, QLGA_EINVAL, "qlga_observables: NULL") : QLGA_EINVAL;
+    if (!c->have_state) return fail(c, QLGA_ESTATE, "qlga_observables: no state set");
+    Launch L{c->stream, &c->launches};
+    const void* prev = (c->prev >= 0) ? c->buf[c->prev] : nullptr;
+    int64_t n = c->nx * c->ny;
+    int blocks = c->obs_blocks;
+    if ((int64_t)blocks * 256 > n) blocks = (int)((n + 255) / 256);
+    CU(c, launch_observables(L, c->prec, c->buf[c->cur], prev, c->nx, c->ny, c->ndim,
+                             c->d_partials, blocks, c->d_sums));
+    double h[OBS_NACC];
+    CU(c, cudaMemcpyAsync(h, c->d_sums, sizeof(h), cudaMemcpyDeviceToHost, c->stream));
+    CU(c, cudaStreamSynchronize(c->stream));
+    double npsi = 0.0;
+    for (int j = 0; j < 5; ++j) { out->n_m[j] = h[j]; npsi += h[j]; }
+    out->norm_psi = npsi; out->norm_q = h[5];
+    out->F[0] = h[6]; out->F[1] = h[7]; out->F[2] = h[8];
+    out->A00_re = h[9]; out->A00_im = h[10]; out->A00_abs2 = h[11];
+    out->e_kin = h[12];
+    out->e_c0 = 0.5 * c->c[0] * h[13];
+    out->e_c1 = 0.5 * c->c[1] * h[14];
+    out->e_c2 = 0.5 * c->c[2] * h[11];
+    out->e_total = out->e_kin + out->e_c0 + out->e_c1 + out->e_c2;
+    if (prev) {   // i (N - O)/N with O = <psi|psi_prev>:  re = Im(O)/N, im = (N - Re(O))/N
+        out->e_dt_re = h[16] / npsi;
+        out->e_dt_im = (npsi - h[15]) / npsi;
+    } else {
+        out->e_dt_re = NAN; out->e_dt_im = NAN;
+    }
+    out->step = c->step;
+    return QLGA_OK;
+}
+
+extern "C" qlga_status qlga_vorticity(qlga_ctx* c, void* omega, int dst_on_device) {
+    if (!c || !omega) return c ? fail(c, QLGA_EINVAL, "qlga_vorticity: NULL") : QLGA_EINVAL;
+    if (c->ndim != 2) return fail(c, QLGA_EUNSUP, "qlga_vorticity: 2D lattices only");
+    if (!c->have_state) return fail(c, QLGA_ESTATE, "qlga_vorticity: no state set");
+    Launch L{c->stream, &c->launches};
+    const size_t bytes = (size_t)5 * c->nx * c->ny * real_size(c->prec);
+    if (dst_on_device) {
+        CU(c, launch_vorticity(L, c->prec, c->buf[c->cur], omega, c->nx, c->ny));
+        return QLGA_OK;
+    }
+    // host destination: a buffer that holds neither the current nor the previous
+    // state serves as scratch (omega is a quarter of a state); else allocate
+    int scratch = -1;
+    for (int k = 0; k < 3; ++k)
+        if (c->buf[k] && k != c->cur && k != c->prev) scratch = k;
+    void* tmp = scratch >= 0 ? c->buf[scratch] : nullptr;
+    bool own = false;
+    if (!tmp) {
+        cudaError_t e = cudaMalloc(&tmp, bytes);
+        if (e != cudaSuccess) { cudaGetLastError(); return fail(c, QLGA_ENOMEM, "qlga_vorticity: cudaMalloc failed"); }
+        own = true;
+    }
+    cudaError_t e = launch_vorticity(L, c->prec, c->buf[c->cur], tmp, c->nx, c->ny);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(omega, tmp, bytes, cudaMemcpyDeviceToHost, c->stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
+    if (own) cudaFree(tmp);
+    if (e != cudaSuccess) return cuda_fail(c, "qlga_vorticity", e);
+    return QLGA_OK;
+}

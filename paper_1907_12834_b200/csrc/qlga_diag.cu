@@ -1,0 +1,247 @@
+// qlga_diag.cu -- lattice reductions (observables), lattice vorticity and the
+// psi <-> q conversions of the QLGA library (sm_100a).
+//
+// Observables: grid-stride loop, 19 fp64 accumulators per thread (fp64 even for an
+// fp32 state), warp-shuffle tree, one shared-memory tree per block, per-block
+// partials to global memory and a second single-block pass -- deterministic, no
+// atomics.  Definitions: include/qlga.h (eq. 3-5, 59-60, 85, 32 of PAPER.md).
+#include "qlga_internal.h"
+
+namespace qlga {
+
+// accumulator slots
+enum { A_N0 = 0, A_NQ = 5, A_FX = 6, A_FY = 7, A_FZ = 8, A_A00R = 9, A_A00I = 10, A_A2 = 11,
+       A_EKIN = 12, A_RHO2 = 13, A_F2 = 14, A_OVR = 15, A_OVI = 16, A_SPARE0 = 17, A_SPARE1 = 18 };
+
+template <typename T>
+__device__ __forceinline__ void load_psi(const typename vec2<T>::type* q, int64_t n, int64_t r,
+                                         double pr[5], double pi[5], double* normq) {
+    double nq = 0.0;
+#pragma unroll
+    for (int j = 0; j < 5; ++j) {
+        const typename vec2<T>::type a = q[(int64_t)(2 * j) * n + r], b = q[(int64_t)(2 * j + 1) * n + r];
+        const double ar = a.x, ai = a.y, br = b.x, bi = b.y;
+        pr[j] = ar + br; pi[j] = ai + bi;
+        nq += ar * ar + ai * ai + br * br + bi * bi;
+    }
+    if (normq) *normq = nq;
+}
+
+template <typename T>
+__global__ void __launch_bounds__(256) observables_kernel(const typename vec2<T>::type* q,
+                                                          const typename vec2<T>::type* qprev,
+                                                          int64_t nx, int64_t ny, int ndim,
+                                                          double* partials) {
+    const int64_t n = nx * ny;
+    double acc[OBS_NACC];
+#pragma unroll
+    for (int k = 0; k < OBS_NACC; ++k) acc[k] = 0.0;
+    const double rt6 = 2.4494897427831780981972840747059;
+    const double irt5 = 0.44721359549995793928183473374626;
+
+    for (int64_t r = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; r < n;
+         r += (int64_t)gridDim.x * blockDim.x) {
+        double pr[5], pi[5], nq;
+        load_psi<T>(q, n, r, pr, pi, &nq);
+        acc[A_NQ] += nq;
+        double nm[5];
+#pragma unroll
+        for (int j = 0; j < 5; ++j) { nm[j] = pr[j] * pr[j] + pi[j] * pi[j]; acc[A_N0 + j] += nm[j]; }
+        const double rho = nm[0] + nm[1] + nm[2] + nm[3] + nm[4];
+        const double Fz = 2.0 * (nm[0] - nm[4]) + (nm[1] - nm[3]);
+        // F_+ = 2(conj(psi_2) psi_1 + conj(psi_-1) psi_-2) + sqrt6 (conj(psi_1) psi_0 + conj(psi_0) psi_-1)
+        const double far_ = pr[0] * pr[1] + pi[0] * pi[1] + pr[3] * pr[4] + pi[3] * pi[4];
+        const double fai = pr[0] * pi[1] - pi[0] * pr[1] + pr[3] * pi[4] - pi[3] * pr[4];
+        const double fbr = pr[1] * pr[2] + pi[1] * pi[2] + pr[2] * pr[3] + pi[2] * pi[3];
+        const double fbi = pr[1] * pi[2] - pi[1] * pr[2] + pr[2] * pi[3] - pi[2] * pr[3];
+        const double Fx = 2.0 * far_ + rt6 * fbr, Fy = 2.0 * fai + rt6 * fbi;
+        acc[A_FX] += Fx; acc[A_FY] += Fy; acc[A_FZ] += Fz;
+        // A00 = (2 psi_2 psi_-2 - 2 psi_1 psi_-1 + psi_0^2)/sqrt5
+        const double tr = 2.0 * (pr[0] * pr[4] - pi[0] * pi[4]) - 2.0 * (pr[1] * pr[3] - pi[1] * pi[3])
+                        + (pr[2] * pr[2] - pi[2] * pi[2]);
+        const double ti = 2.0 * (pr[0] * pi[4] + pi[0] * pr[4]) - 2.0 * (pr[1] * pi[3] + pi[1] * pr[3])
+                        + 2.0 * pr[2] * pi[2];
+        const double ar = tr * irt5, ai = ti * irt5;
+        acc[A_A00R] += ar; acc[A_A00I] += ai; acc[A_A2] += ar * ar + ai * ai;
+        acc[A_RHO2] += rho * rho;
+        acc[A_F2] += Fx * Fx + Fy * Fy + Fz * Fz;
+        // kinetic: forward differences along x (and y)
+        const int64_t x = r % nx, y = r / nx;
+        for (int d = 0; d < ndim; ++d) {
+            int64_t rn;
+            if (d == 0) rn = y * nx + (x == nx - 1 ? 0 : x + 1);
+            else rn = (y == ny - 1 ? 0 : y + 1) * nx + x;
+            double qr[5], qi[5];
+            load_psi<T>(q, n, rn, qr, qi, nullptr);
+#pragma unroll
+            for (int j = 0; j < 5; ++j) {
+                const double dr = qr[j] - pr[j], di = qi[j] - pi[j];
+                acc[A_EKIN] += dr * dr + di * di;
+            }
+        }
+        if (qprev) {       // <psi(t)|psi(t - tau)>
+            double qr[5], qi[5];
+            load_psi<T>(qprev, n, r, qr, qi, nullptr);
+#pragma unroll
+            for (int j = 0; j < 5; ++j) {
+                acc[A_OVR] += pr[j] * qr[j] + pi[j] * qi[j];
+                acc[A_OVI] += pr[j] * qi[j] - pi[j] * qr[j];
+            }
+        }
+    }
+
+    __shared__ double sm[8][OBS_NACC];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+#pragma unroll
+    for (int k = 0; k < OBS_NACC; ++k) {
+        double v = acc[k];
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+        if (lane == 0) sm[warp][k] = v;
+    }
+    __syncthreads();
+    if (threadIdx.x < OBS_NACC) {
+        double v = 0.0;
+        for (int w = 0; w < 8; ++w) v += sm[w][threadIdx.x];
+        partials[(int64_t)blockIdx.x * OBS_NACC + threadIdx.x] = v;
+    }
+}
+
+__global__ void __launch_bounds__(256) reduce_partials_kernel(const double* partials, int nblocks,
+                                                              double* sums) {
+    __shared__ double sm[8];
+    for (int k = 0; k < OBS_NACC; ++k) {
+        double v = 0.0;
+        for (int b = threadIdx.x; b < nblocks; b += blockDim.x) v += partials[(int64_t)b * OBS_NACC + k];
+        for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+        if ((threadIdx.x & 31) == 0) sm[threadIdx.x >> 5] = v;
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            double s = 0.0;
+            for (int w = 0; w < 8; ++w) s += sm[w];
+            sums[k] = s;
+        }
+        __syncthreads();
+    }
+}
+
+cudaError_t launch_observables(const Launch& L, qlga_prec prec, const void* q, const void* qprev,
+                               int64_t nx, int64_t ny, int ndim, double* partials, int nblocks,
+                               double* sums) {
+    if (prec == QLGA_F64)
+        observables_kernel<double><<<nblocks, 256, 0, L.stream>>>((const double2*)q, (const double2*)qprev,
+                                                                   nx, ny, ndim, partials);
+    else
+        observables_kernel<float><<<nblocks, 256, 0, L.stream>>>((const float2*)q, (const float2*)qprev,
+                                                                  nx, ny, ndim, partials);
+    ++*L.counter;
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return e;
+    reduce_partials_kernel<<<1, 256, 0, L.stream>>>(partials, nblocks, sums);
+    ++*L.counter;
+    return cudaGetLastError();
+}
+
+// ---------------------------------------------------------------------------
+// Lattice vorticity (eq. 102-104, reading R8).  Substituting v_x, v_y into the
+// curl, omega(x,y) depends only on psi at the four diagonal neighbours:
+//   omega = (1/4)[ arg(p(x+1,y+1) p*(x+1,y-1)) - arg(p(x-1,y+1) p*(x-1,y-1))
+//                - arg(p(x+1,y+1) p*(x-1,y+1)) + arg(p(x+1,y-1) p*(x-1,y-1)) ],  arg(0) := 0.
+// The arithmetic is done in fp64 for both storage types.
+// ---------------------------------------------------------------------------
+__device__ __forceinline__ double arg_prod_conj(double ar, double ai, double br, double bi) {
+    // arg(a * conj(b))
+    const double re = ar * br + ai * bi, im = ai * br - ar * bi;
+    return (re == 0.0 && im == 0.0) ? 0.0 : atan2(im, re);
+}
+
+template <typename T>
+__global__ void __launch_bounds__(128) vorticity_kernel(const typename vec2<T>::type* q, T* omega,
+                                                        int64_t nx, int64_t ny) {
+    using V = typename vec2<T>::type;
+    const int64_t n = nx * ny;
+    const int64_t r = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (r >= n) return;
+    const int64_t x = r % nx, y = r / nx;
+    const int64_t xp = (x == nx - 1) ? 0 : x + 1, xm = (x == 0) ? nx - 1 : x - 1;
+    const int64_t yp = (y == ny - 1) ? 0 : y + 1, ym = (y == 0) ? ny - 1 : y - 1;
+    const int64_t ipp = yp * nx + xp, ipm = ym * nx + xp, imp = yp * nx + xm, imm = ym * nx + xm;
+    for (int j = 0; j < 5; ++j) {
+        const V* p1 = q + (int64_t)(2 * j) * n;
+        const V* p2 = q + (int64_t)(2 * j + 1) * n;
+        V a, b;
+        a = p1[ipp]; b = p2[ipp]; const double ppr = (double)a.x + (double)b.x, ppi = (double)a.y + (double)b.y;
+        a = p1[ipm]; b = p2[ipm]; const double pmr = (double)a.x + (double)b.x, pmi = (double)a.y + (double)b.y;
+        a = p1[imp]; b = p2[imp]; const double mpr = (double)a.x + (double)b.x, mpi = (double)a.y + (double)b.y;
+        a = p1[imm]; b = p2[imm]; const double mmr = (double)a.x + (double)b.x, mmi = (double)a.y + (double)b.y;
+        // v_y(x+1,y), v_y(x-1,y), v_x(x,y+1), v_x(x,y-1)   (each is half the wrapped phase difference)
+        const double vy_p = 0.5 * arg_prod_conj(ppr, ppi, pmr, pmi);
+        const double vy_m = 0.5 * arg_prod_conj(mpr, mpi, mmr, mmi);
+        const double vx_p = 0.5 * arg_prod_conj(ppr, ppi, mpr, mpi);
+        const double vx_m = 0.5 * arg_prod_conj(pmr, pmi, mmr, mmi);
+        omega[(int64_t)j * n + r] = (T)(0.5 * (vy_p - vy_m - vx_p + vx_m));
+    }
+}
+
+cudaError_t launch_vorticity(const Launch& L, qlga_prec prec, const void* q, void* omega,
+                             int64_t nx, int64_t ny) {
+    const int64_t n = nx * ny;
+    const unsigned blocks = (unsigned)((n + 127) / 128);
+    if (prec == QLGA_F64)
+        vorticity_kernel<double><<<blocks, 128, 0, L.stream>>>((const double2*)q, (double*)omega, nx, ny);
+    else
+        vorticity_kernel<float><<<blocks, 128, 0, L.stream>>>((const float2*)q, (float*)omega, nx, ny);
+    ++*L.counter;
+    return cudaGetLastError();
+}
+
+// ---------------------------------------------------------------------------
+// psi <-> q.  `psi` points at a chunk holding sites [offset, offset+count) of all
+// five channels, packed as [5][count]; q is the full [5][2][nsites] state.
+// ---------------------------------------------------------------------------
+template <typename T>
+__global__ void split_psi_kernel(const typename vec2<T>::type* psi, typename vec2<T>::type* q,
+                                 int64_t nsites, int64_t offset, int64_t count) {
+    const int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= 5 * count) return;
+    const int64_t j = k / count, r = k % count;
+    typename vec2<T>::type v = psi[k];
+    v.x *= (T)0.5; v.y *= (T)0.5;                 // q1 = q2 = psi/2  (reading R6)
+    q[(2 * j) * nsites + offset + r] = v;
+    q[(2 * j + 1) * nsites + offset + r] = v;
+}
+
+template <typename T>
+__global__ void sum_psi_kernel(const typename vec2<T>::type* q, typename vec2<T>::type* psi,
+                               int64_t nsites, int64_t offset, int64_t count) {
+    const int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= 5 * count) return;
+    const int64_t j = k / count, r = k % count;
+    const typename vec2<T>::type a = q[(2 * j) * nsites + offset + r], b = q[(2 * j + 1) * nsites + offset + r];
+    typename vec2<T>::type v; v.x = a.x + b.x; v.y = a.y + b.y;
+    psi[k] = v;
+}
+
+cudaError_t launch_split_psi(const Launch& L, qlga_prec prec, const void* psi, void* q,
+                             int64_t nsites, int64_t offset, int64_t count) {
+    const unsigned blocks = (unsigned)((5 * count + 255) / 256);
+    if (prec == QLGA_F64)
+        split_psi_kernel<double><<<blocks, 256, 0, L.stream>>>((const double2*)psi, (double2*)q, nsites, offset, count);
+    else
+        split_psi_kernel<float><<<blocks, 256, 0, L.stream>>>((const float2*)psi, (float2*)q, nsites, offset, count);
+    ++*L.counter;
+    return cudaGetLastError();
+}
+
+cudaError_t launch_sum_psi(const Launch& L, qlga_prec prec, const void* q, void* psi,
+                           int64_t nsites, int64_t offset, int64_t count) {
+    const unsigned blocks = (unsigned)((5 * count + 255) / 256);
+    if (prec == QLGA_F64)
+        sum_psi_kernel<double><<<blocks, 256, 0, L.stream>>>((const double2*)q, (double2*)psi, nsites, offset, count);
+    else
+        sum_psi_kernel<float><<<blocks, 256, 0, L.stream>>>((const float2*)q, (float2*)psi, nsites, offset, count);
+    ++*L.counter;
+    return cudaGetLastError();
+}
+
+}  // namespace qlga

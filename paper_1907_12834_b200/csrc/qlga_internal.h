@@ -1,0 +1,92 @@
+// qlga_internal.h -- context and kernel-launcher declarations shared by the
+// translation units of libqlga.so.  Not part of the public ABI (include/qlga.h).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <stddef.h>
+#include "../../include/qlga.h"
+#include "qlga_math.cuh"
+
+namespace qlga {
+
+// Parameters of one fused directional pass (4 kinetic factors per fused time
+// step, with the interaction interleaved as `umode` says).
+struct PassParams {
+    const void* src;
+    void* dst;
+    int64_t nx, ny;
+    int ksteps;            // time steps fused in this launch (1 in 2D)
+    int umode;             // 0: no U in this pass, 1: U before the first factor of each step,
+                           // 2: U before every factor
+    double g[4][3];        // per factor: (s c0, s c1, s c2/5) * 4^-e  (e = deferred halvings so far)
+    double out_scale;      // 2^-4, applied after the 4 factors of a step
+    ExpTable tab;
+};
+
+struct Launch {
+    cudaStream_t stream;
+    int64_t* counter;      // incremented per kernel launched
+};
+
+// fused passes (qlga_step.cu); dir = 0 (x) or 1 (y).  `threads` / `cx` are tunables
+// (0 = default).  Returns cudaGetLastError().
+cudaError_t launch_pass(const Launch& L, qlga_prec prec, int dir, const PassParams& P,
+                        int threads, int cx);
+// widest ksteps the x pass supports with the given CTA size
+int max_ksteps(int threads);
+
+// one kernel per operator (reference path on the GPU)
+cudaError_t launch_interaction(const Launch& L, qlga_prec prec, void* q, int64_t nx, int64_t ny,
+                               const double g[3], const ExpTable& tab);
+cudaError_t launch_kinetic(const Launch& L, qlga_prec prec, const void* src, void* dst,
+                           int64_t nx, int64_t ny, int dir, int sigma);
+
+// diagnostics and state conversion (qlga_diag.cu)
+constexpr int OBS_NACC = 19;   // accumulators per block, see qlga_diag.cu
+cudaError_t launch_observables(const Launch& L, qlga_prec prec, const void* q, const void* qprev,
+                               int64_t nx, int64_t ny, int ndim, double* partials, int nblocks,
+                               double* sums);
+cudaError_t launch_vorticity(const Launch& L, qlga_prec prec, const void* q, void* omega,
+                             int64_t nx, int64_t ny);
+cudaError_t launch_split_psi(const Launch& L, qlga_prec prec, const void* psi, void* q,
+                             int64_t nsites, int64_t offset, int64_t count);
+cudaError_t launch_sum_psi(const Launch& L, qlga_prec prec, const void* q, void* psi,
+                           int64_t nsites, int64_t offset, int64_t count);
+
+}  // namespace qlga
+
+struct qlga_ctx {
+    int ndim;
+    int64_t nx, ny;
+    double c[3];
+    qlga_order order;
+    qlga_prec prec;
+    void* buf[3];
+    size_t buf_bytes;
+    cudaStream_t stream;
+    int cur;               // index of the buffer holding the current state
+    int prev;              // index of the buffer holding the previous step's state, or -1
+    int have_state;
+    int64_t step;
+    int64_t launches;
+    // options
+    int path;              // 0 fused, 1 per-operator
+    int steps_per_launch;  // 1D temporal blocking, 0 = auto
+    int tol_log2;
+    int threads_x;
+    int tile_y;
+    qlga::ExpTable tab;
+    // scratch owned by the library
+    double* d_partials;    // [obs_blocks][OBS_NACC]
+    double* d_sums;        // [OBS_NACC]
+    int obs_blocks;
+    void* d_stage;         // staging for psi transfers
+    size_t stage_bytes;
+    // kernel timing hooks (qlga_profile_*)
+    int prof_on;
+    int prof_n;
+    cudaEvent_t* prof_ev;  // [PROF_CAP], created on first enable
+    signed char* prof_kind;
+    char err[512];
+};
+constexpr int PROF_CAP = 4097;

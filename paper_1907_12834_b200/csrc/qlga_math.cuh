@@ -1,0 +1,213 @@
+// qlga_math.cuh -- per-site device arithmetic of the spin-2 QLGA step (sm_100a).
+//
+// Everything here works on one lattice site held in registers:
+//   * kinetic messages of I'_{d,sigma} = S C S^T C (eq. 107)
+//     written as a radius-1 stencil,
+//   * the interaction unitary U^{(s)} = exp(-i s H_int[psi]) (reading R4,
+//     eq. 34) as scalar phase x Horner polynomial of
+//     K = c1 F.f + (c2/5)|chi><chi| applied to the two spinor 5-vectors.
+// No code is shared with oracle/.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace qlga {
+
+template <typename T> struct vec2;
+template <> struct vec2<double> { using type = double2; };
+template <> struct vec2<float>  { using type = float2; };
+
+template <typename T> struct cx {
+    T re, im;
+};
+
+template <typename T> __device__ __forceinline__ cx<T> mk(T re, T im) { cx<T> z; z.re = re; z.im = im; return z; }
+template <typename T> __device__ __forceinline__ cx<T> operator+(cx<T> a, cx<T> b) { return mk<T>(a.re + b.re, a.im + b.im); }
+template <typename T> __device__ __forceinline__ cx<T> operator-(cx<T> a, cx<T> b) { return mk<T>(a.re - b.re, a.im - b.im); }
+template <typename T> __device__ __forceinline__ cx<T> cmul(cx<T> a, cx<T> b) {
+    return mk<T>(a.re * b.re - a.im * b.im, a.re * b.im + a.im * b.re);
+}
+// acc + a*b
+template <typename T> __device__ __forceinline__ cx<T> cfma(cx<T> a, cx<T> b, cx<T> acc) {
+    acc.re = fma(a.re, b.re, acc.re); acc.re = fma(-a.im, b.im, acc.re);
+    acc.im = fma(a.re, b.im, acc.im); acc.im = fma(a.im, b.re, acc.im);
+    return acc;
+}
+// acc + conj(a)*b
+template <typename T> __device__ __forceinline__ cx<T> cfma_conj(cx<T> a, cx<T> b, cx<T> acc) {
+    acc.re = fma(a.re, b.re, acc.re); acc.re = fma(a.im, b.im, acc.re);
+    acc.im = fma(a.re, b.im, acc.im); acc.im = fma(-a.im, b.re, acc.im);
+    return acc;
+}
+
+__device__ __forceinline__ void sincos_t(double x, double* s, double* c) { sincos(x, s, c); }
+__device__ __forceinline__ void sincos_t(float x, float* s, float* c) { sincosf(x, s, c); }
+
+// Site state: q[j][sigma], j = 0..4 <-> m = +2..-2.
+template <typename T> struct Site {
+    cx<T> q[5][2];
+};
+
+// ---------------------------------------------------------------------------
+// Kinetic factor I'_{d,sigma} as a stencil, halvings deferred.
+// With a = streamed component sigma, b = the other one:
+//   Fw = i a + b   (goes to the site at r + e)      Bw = a + i b   (goes to r - e)
+//   a'(r) = -i Bw(r) + Fw(r - e)                    b'(r) = -i Fw(r) + Bw(r + e)
+// and the true result is (a', b')/2; the caller folds the power of two into the
+// interaction constants and into one final scaling (exact in binary floating point).
+// ---------------------------------------------------------------------------
+template <typename T>
+__device__ __forceinline__ void kin_messages(const Site<T>& s, int sigma, cx<T> Fw[5], cx<T> Bw[5]) {
+#pragma unroll
+    for (int j = 0; j < 5; ++j) {
+        cx<T> a = s.q[j][sigma], b = s.q[j][1 - sigma];
+        Fw[j] = mk<T>(b.re - a.im, b.im + a.re);
+        Bw[j] = mk<T>(a.re - b.im, a.im + b.re);
+    }
+}
+
+template <typename T>
+__device__ __forceinline__ void kin_update(Site<T>& s, int sigma, const cx<T> Fw[5], const cx<T> Bw[5],
+                                           const cx<T> Fprev[5], const cx<T> Bnext[5]) {
+#pragma unroll
+    for (int j = 0; j < 5; ++j) {
+        s.q[j][sigma]     = mk<T>(Fprev[j].re + Bw[j].im, Fprev[j].im - Bw[j].re);
+        s.q[j][1 - sigma] = mk<T>(Bnext[j].re + Fw[j].im, Bnext[j].im - Fw[j].re);
+    }
+}
+
+// ---------------------------------------------------------------------------
+// Interaction.  Constants of one application (already multiplied by the
+// sub-step fraction s and by the deferred-scaling factor 4^-e):
+//   g0 = s c0, g1 = s c1, g2 = s c2 / 5.
+// thr[p-1] = largest angle for which a degree-p polynomial meets the tolerance.
+// ---------------------------------------------------------------------------
+constexpr int QLGA_PMAX = 18;
+
+template <typename T> struct UConst {
+    T g0, g1, g2;
+};
+
+struct ExpTable {
+    double rcp[QLGA_PMAX + 2];  // rcp[k] = 1/k
+    float thr[QLGA_PMAX];       // thresholds in float: order selection only
+    float theta_split;          // angles above this are split into equal sub-angles
+};
+
+// w = (s K) u  with  s K = g1 F.f + g2 |chi><chi|,
+//   (F.f u)_m = m F_z u_m + (1/2) F_- alpha_{m-1} u_{m-1} + (1/2) F_+ alpha_m u_{m+1},
+//   alpha_1 = alpha_-2 = 2, alpha_0 = alpha_-1 = sqrt(6)   (f_+|m> = sqrt(6 - m(m+1))|m+1>),
+//   <chi|u> = sum_m (-1)^m psi_{-m} u_m,   chi_m = (-1)^m conj(psi_{-m}).
+// Inputs are pre-scaled: az = g1 F_z, a1 = g1 F_+ (coefficient 2/2), a6 = g1 (sqrt6/2) F_+.
+template <typename T>
+__device__ __forceinline__ void apply_sK(const cx<T> u[5], cx<T> w[5], T az, cx<T> a1, cx<T> a6,
+                                         T g2, const cx<T> psi[5]) {
+    // rank-one part: t = g2 <chi|u>
+    cx<T> t = cmul(psi[4], u[0]);
+    t = cfma(psi[2], u[2], t);
+    t = cfma(psi[0], u[4], t);
+    cx<T> t2 = cmul(psi[3], u[1]);
+    t2 = cfma(psi[1], u[3], t2);
+    t = t - t2;
+    t.re *= g2; t.im *= g2;
+    // spin part, rows m = +2..-2 (j = 0..4); raising uses conj(F_+) on u_{m-1} (j+1),
+    // lowering uses F_+ on u_{m+1} (j-1)
+    const T two = (T)2;
+    cx<T> r0 = mk<T>(two * az * u[0].re, two * az * u[0].im);
+    r0 = cfma_conj(a1, u[1], r0);
+    cx<T> r1 = mk<T>(az * u[1].re, az * u[1].im);
+    r1 = cfma(a1, u[0], r1);
+    r1 = cfma_conj(a6, u[2], r1);
+    cx<T> r2 = cmul(a6, u[1]);
+    r2 = cfma_conj(a6, u[3], r2);
+    cx<T> r3 = mk<T>(-az * u[3].re, -az * u[3].im);
+    r3 = cfma(a6, u[2], r3);
+    r3 = cfma_conj(a1, u[4], r3);
+    cx<T> r4 = mk<T>(-two * az * u[4].re, -two * az * u[4].im);
+    r4 = cfma(a1, u[3], r4);
+    // add t * chi_m,  chi_m = (-1)^m conj(psi_{-m})
+    w[0] = cfma_conj(psi[4], t, r0);
+    w[1] = r1 - cfma_conj(psi[3], t, mk<T>((T)0, (T)0));
+    w[2] = cfma_conj(psi[2], t, r2);
+    w[3] = r3 - cfma_conj(psi[1], t, mk<T>((T)0, (T)0));
+    w[4] = cfma_conj(psi[0], t, r4);
+}
+
+// Apply U^{(s)} to one site.  The site may carry a power-of-two scale 2^e; the
+// caller passes constants multiplied by 4^-e, which makes the result identical
+// (bit for bit, barring under/overflow) to applying U to the unscaled site.
+template <typename T>
+__device__ __forceinline__ void interaction(Site<T>& s, const UConst<T>& uc, const ExpTable& tab) {
+    cx<T> psi[5];
+    T n[5];
+#pragma unroll
+    for (int j = 0; j < 5; ++j) {
+        psi[j] = s.q[j][0] + s.q[j][1];
+        n[j] = fma(psi[j].re, psi[j].re, psi[j].im * psi[j].im);
+    }
+    const T rho = (n[0] + n[4]) + (n[1] + n[3]) + n[2];
+    const T Fz = (T)2 * (n[0] - n[4]) + (n[1] - n[3]);
+    // F_+ = sum_m alpha_m conj(psi_{m+1}) psi_m = 2(conj(psi_2) psi_1 + conj(psi_-1) psi_-2)
+    //                                           + sqrt6 (conj(psi_1) psi_0 + conj(psi_0) psi_-1)
+    cx<T> fa = cfma_conj(psi[0], psi[1], mk<T>((T)0, (T)0));
+    fa = cfma_conj(psi[3], psi[4], fa);
+    cx<T> fb = cfma_conj(psi[1], psi[2], mk<T>((T)0, (T)0));
+    fb = cfma_conj(psi[2], psi[3], fb);
+    const T rt6 = (T)2.4494897427831780981972840747059;
+    const cx<T> Fp = mk<T>(fma(rt6, fb.re, (T)2 * fa.re), fma(rt6, fb.im, (T)2 * fa.im));
+
+    // angle bound theta = 2 |g1| |F| + |g2| rho  (spectral norms of the two parts)
+    const float Fabs = sqrtf((float)(Fz * Fz + Fp.re * Fp.re + Fp.im * Fp.im));
+    float theta = 2.0f * fabsf((float)uc.g1) * Fabs + fabsf((float)uc.g2) * (float)rho;
+    theta *= 1.0009765625f;                       // cover the float rounding of the estimate
+    int nsub = 1;
+    if (theta > tab.theta_split) {
+        nsub = (int)ceilf(theta / tab.theta_split);
+        theta = theta / (float)nsub * 1.0009765625f;
+    }
+    int p = 1;
+#pragma unroll
+    for (int k = 0; k < QLGA_PMAX - 1; ++k) p += (theta > tab.thr[k]) ? 1 : 0;
+    p = __reduce_max_sync(0xffffffffu, p);       // warp-uniform trip count
+    nsub = __reduce_max_sync(0xffffffffu, nsub);
+
+    const T inv_nsub = (T)1 / (T)nsub;
+    const T g1 = uc.g1 * inv_nsub, g2 = uc.g2 * inv_nsub;
+    const T az = g1 * Fz;
+    const cx<T> a1 = mk<T>(g1 * Fp.re, g1 * Fp.im);
+    const T h6 = g1 * (T)1.2247448713915890490986420373529;      // sqrt(6)/2
+    const cx<T> a6 = mk<T>(h6 * Fp.re, h6 * Fp.im);
+
+    // scalar phase exp(-i s c0 rho)
+    T sn, cs;
+    sincos_t(uc.g0 * rho, &sn, &cs);
+    const cx<T> ph = mk<T>(cs, -sn);
+
+#pragma unroll
+    for (int sg = 0; sg < 2; ++sg) {
+        cx<T> v[5], u[5], w[5];
+#pragma unroll
+        for (int j = 0; j < 5; ++j) { v[j] = s.q[j][sg]; u[j] = v[j]; }
+        for (int rep = 0; rep < nsub; ++rep) {
+            if (rep > 0) {
+#pragma unroll
+                for (int j = 0; j < 5; ++j) v[j] = u[j];
+            }
+            // Horner: u_{k-1} = v + (-i/k) (sK) u_k ; psi (hence K) is frozen at its
+            // value before the application (reading R4)
+            for (int k = p; k >= 1; --k) {
+                apply_sK<T>(u, w, az, a1, a6, g2, psi);
+                const T ik = (T)tab.rcp[k];
+#pragma unroll
+                for (int j = 0; j < 5; ++j) {
+                    u[j].re = fma(ik, w[j].im, v[j].re);
+                    u[j].im = fma(-ik, w[j].re, v[j].im);
+                }
+            }
+        }
+#pragma unroll
+        for (int j = 0; j < 5; ++j) s.q[j][sg] = cmul(ph, u[j]);
+    }
+}
+
+}  // namespace qlga

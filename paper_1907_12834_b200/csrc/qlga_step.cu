@@ -1,0 +1,303 @@
+// qlga_step.cu -- fused directional pass kernels of the QLGA time step (sm_100a).
+//
+// One pass = the four kinetic factors of one lattice direction,
+//     I'_{d,1} I'_{d,1} I'_{d,2} I'_{d,2}          (eq. 108 / 112)
+// with the interaction U interleaved before every factor (eq. 112), before the
+// first factor only (eq. 108: U is the rightmost operator of the step), or not at
+// all.  A 1D step is one x pass; a 2D step is a y pass followed by an x pass (R7).
+//
+// Design: one lattice site per thread, the 10 complex
+// amplitudes live in registers for the whole pass.  A CTA owns a line of TS sites
+// along the pass direction (x pass) or CX adjacent such lines (y pass: CX columns,
+// so a warp reads CX*16 B contiguous segments).  The only neighbour traffic of a
+// kinetic factor is one 5-vector to the site at r+e and one to r-e; it moves by
+// warp shuffle (distance CX) and, for the lanes on a warp edge, through a few
+// hundred bytes of shared memory.  Lines overlap by a halo of 4 sites per fused
+// time step on each side and the halo threads recompute (TS-8)/TS efficiency);
+// nothing but the final state goes back to HBM: 320 B per site per pass in fp64.
+#include "qlga_internal.h"
+
+namespace qlga {
+
+template <typename T>
+struct PassArgs {
+    const typename vec2<T>::type* src;
+    typename vec2<T>::type* dst;
+    int64_t nx, ny;
+    int ksteps, umode;
+    UConst<T> uc[4];
+    T out_scale;
+    ExpTable tab;
+};
+
+__device__ __forceinline__ int64_t pmod(int64_t a, int64_t n) {
+    int64_t r = a % n;
+    return r < 0 ? r + n : r;
+}
+
+template <typename T, int DIR, int CX, int NT>
+__global__ void __launch_bounds__(NT) pass_kernel(const __grid_constant__ PassArgs<T> P) {
+    using V = typename vec2<T>::type;
+    constexpr int TS = NT / CX;              // sites per line handled by the CTA
+    constexpr int NW = NT / 32;
+    constexpr int EDGE = 32 - CX;
+    static_assert(NT % 32 == 0 && 32 % CX == 0 && CX < 32, "bad tile");
+    static_assert(DIR == 1 || CX == 1, "x pass uses one line per CTA");
+
+    __shared__ cx<T> edgeF[2][NW][CX][5];
+    __shared__ cx<T> edgeB[2][NW][CX][5];
+
+    const int t = threadIdx.x;
+    const int lane = t & 31, warp = t >> 5;
+    const int c = t % CX, i = t / CX;
+    const int H = 4 * P.ksteps;
+    const int wout = TS - 2 * H;
+    const int64_t n = P.nx * P.ny;
+
+    int64_t x, y, spos, extent;
+    bool col_ok = true;
+    if (DIR == 0) {
+        const int64_t tiles = (P.nx + wout - 1) / wout;
+        const int64_t tile = blockIdx.x % tiles;
+        y = blockIdx.x / tiles;
+        spos = tile * wout - H + i;
+        extent = P.nx;
+        x = pmod(spos, P.nx);
+    } else {
+        const int64_t tiles_c = (P.nx + CX - 1) / CX;
+        const int64_t tc = blockIdx.x % tiles_c;
+        const int64_t ts = blockIdx.x / tiles_c;
+        x = tc * CX + c;
+        col_ok = x < P.nx;
+        if (!col_ok) x = P.nx - 1;
+        spos = ts * wout - H + i;
+        extent = P.ny;
+        y = pmod(spos, P.ny);
+    }
+    const int64_t idx = y * P.nx + x;
+
+    // slot 0 = the component that streams in the current factor, slot 1 = the other.
+    // The pass starts with component 2 (plane sigma = 1) streaming.
+    Site<T> s;
+#pragma unroll
+    for (int j = 0; j < 5; ++j) {
+        V a = P.src[(int64_t)(2 * j + 1) * n + idx];
+        V b = P.src[(int64_t)(2 * j + 0) * n + idx];
+        s.q[j][0] = mk<T>(a.x, a.y);
+        s.q[j][1] = mk<T>(b.x, b.y);
+    }
+
+    const int nsub = 4 * P.ksteps;
+    int pb = 0;
+#pragma unroll 1
+    for (int sub = 0; sub < nsub; ++sub) {
+        const int f = sub & 3;
+        if (P.umode == 2 || (P.umode == 1 && f == 0)) interaction<T>(s, P.uc[f], P.tab);
+
+        cx<T> Fw[5], Bw[5], Fp[5], Bn[5];
+        kin_messages<T>(s, 0, Fw, Bw);
+        if (lane >= EDGE) {
+#pragma unroll
+            for (int j = 0; j < 5; ++j) edgeF[pb][warp][lane - EDGE][j] = Fw[j];
+        }
+        if (lane < CX) {
+#pragma unroll
+            for (int j = 0; j < 5; ++j) edgeB[pb][warp][lane][j] = Bw[j];
+        }
+#pragma unroll
+        for (int j = 0; j < 5; ++j) {
+            Fp[j].re = __shfl_up_sync(0xffffffffu, Fw[j].re, CX);
+            Fp[j].im = __shfl_up_sync(0xffffffffu, Fw[j].im, CX);
+            Bn[j].re = __shfl_down_sync(0xffffffffu, Bw[j].re, CX);
+            Bn[j].im = __shfl_down_sync(0xffffffffu, Bw[j].im, CX);
+        }
+        __syncthreads();
+        if (lane < CX && warp > 0) {
+#pragma unroll
+            for (int j = 0; j < 5; ++j) Fp[j] = edgeF[pb][warp - 1][lane][j];
+        }
+        if (lane >= EDGE && warp < NW - 1) {
+#pragma unroll
+            for (int j = 0; j < 5; ++j) Bn[j] = edgeB[pb][warp + 1][lane - EDGE][j];
+        }
+        pb ^= 1;
+        kin_update<T>(s, 0, Fw, Bw, Fp, Bn);
+
+        if (sub & 1) {                       // factors come in pairs: 2,2,1,1 -> swap roles
+#pragma unroll
+            for (int j = 0; j < 5; ++j) { cx<T> tmp = s.q[j][0]; s.q[j][0] = s.q[j][1]; s.q[j][1] = tmp; }
+        }
+        if (f == 3) {                        // undo the four deferred halvings (exact)
+#pragma unroll
+            for (int j = 0; j < 5; ++j) {
+                s.q[j][0].re *= P.out_scale; s.q[j][0].im *= P.out_scale;
+                s.q[j][1].re *= P.out_scale; s.q[j][1].im *= P.out_scale;
+            }
+        }
+    }
+
+    // after a whole number of steps slot 0 is component 2 again
+    if (i >= H && i < TS - H && spos < extent && col_ok) {
+#pragma unroll
+        for (int j = 0; j < 5; ++j) {
+            V a, b;
+            a.x = s.q[j][0].re; a.y = s.q[j][0].im;
+            b.x = s.q[j][1].re; b.y = s.q[j][1].im;
+            P.dst[(int64_t)(2 * j + 1) * n + idx] = a;
+            P.dst[(int64_t)(2 * j + 0) * n + idx] = b;
+        }
+    }
+}
+
+template <typename T>
+static PassArgs<T> make_args(const PassParams& P) {
+    PassArgs<T> A;
+    A.src = (const typename vec2<T>::type*)P.src;
+    A.dst = (typename vec2<T>::type*)P.dst;
+    A.nx = P.nx; A.ny = P.ny; A.ksteps = P.ksteps; A.umode = P.umode;
+    for (int f = 0; f < 4; ++f) {
+        A.uc[f].g0 = (T)P.g[f][0]; A.uc[f].g1 = (T)P.g[f][1]; A.uc[f].g2 = (T)P.g[f][2];
+    }
+    A.out_scale = (T)P.out_scale;
+    A.tab = P.tab;
+    return A;
+}
+
+template <typename T, int DIR, int CX, int NT>
+static cudaError_t run_pass(const Launch& L, const PassParams& P) {
+    constexpr int TS = NT / CX;
+    const int wout = TS - 8 * P.ksteps;
+    if (wout <= 0) return cudaErrorInvalidValue;
+    int64_t blocks;
+    if (DIR == 0) blocks = ((P.nx + wout - 1) / wout) * P.ny;
+    else blocks = ((P.nx + CX - 1) / CX) * ((P.ny + wout - 1) / wout);
+    if (blocks <= 0 || blocks > 2147483647LL) return cudaErrorInvalidValue;
+    PassArgs<T> A = make_args<T>(P);
+    pass_kernel<T, DIR, CX, NT><<<(unsigned)blocks, NT, 0, L.stream>>>(A);
+    ++*L.counter;
+    return cudaGetLastError();
+}
+
+int max_ksteps(int threads) { return (threads - 8) / 8; }
+
+template <typename T>
+static cudaError_t launch_pass_t(const Launch& L, int dir, const PassParams& P, int threads, int cxw) {
+    if (dir == 0) {
+        if (threads == 0) threads = 128;
+        switch (threads) {
+            case 128: return run_pass<T, 0, 1, 128>(L, P);
+            case 256: return run_pass<T, 0, 1, 256>(L, P);
+            default: return cudaErrorInvalidValue;
+        }
+    }
+    if (cxw == 0) cxw = 4;
+    switch (cxw) {
+        case 1: return run_pass<T, 1, 1, 128>(L, P);
+        case 2: return run_pass<T, 1, 2, 256>(L, P);
+        case 4: return run_pass<T, 1, 4, 256>(L, P);
+        case 8: return run_pass<T, 1, 8, 256>(L, P);
+        default: return cudaErrorInvalidValue;
+    }
+}
+
+cudaError_t launch_pass(const Launch& L, qlga_prec prec, int dir, const PassParams& P,
+                        int threads, int cxw) {
+    return prec == QLGA_F64 ? launch_pass_t<double>(L, dir, P, threads, cxw)
+                            : launch_pass_t<float>(L, dir, P, threads, cxw);
+}
+
+// ---------------------------------------------------------------------------
+// One kernel per operator: U in place, I'_{d,sigma} out of place straight from
+// global memory.  Slow (one HBM round trip per operator); kept as the GPU-side
+// cross-check of the fused passes and selectable with QLGA_OPT_PATH = 1.
+// ---------------------------------------------------------------------------
+template <typename T>
+__global__ void __launch_bounds__(128) interaction_kernel(typename vec2<T>::type* q, int64_t n,
+                                                          UConst<T> uc, const __grid_constant__ ExpTable tab) {
+    using V = typename vec2<T>::type;
+    // every thread of the CTA takes part (the order selection is a warp reduction);
+    // threads past the end work on a copy of the last site and do not store
+    int64_t r = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    const bool ok = r < n;
+    if (!ok) r = n - 1;
+    Site<T> s;
+#pragma unroll
+    for (int j = 0; j < 5; ++j)
+#pragma unroll
+        for (int sg = 0; sg < 2; ++sg) {
+            V v = q[(int64_t)(2 * j + sg) * n + r];
+            s.q[j][sg] = mk<T>(v.x, v.y);
+        }
+    interaction<T>(s, uc, tab);
+    if (ok) {
+#pragma unroll
+        for (int j = 0; j < 5; ++j)
+#pragma unroll
+            for (int sg = 0; sg < 2; ++sg) {
+                V v; v.x = s.q[j][sg].re; v.y = s.q[j][sg].im;
+                q[(int64_t)(2 * j + sg) * n + r] = v;
+            }
+    }
+}
+
+template <typename T>
+__global__ void __launch_bounds__(128) kinetic_kernel(const typename vec2<T>::type* src,
+                                                      typename vec2<T>::type* dst,
+                                                      int64_t nx, int64_t ny, int dir, int sigma) {
+    using V = typename vec2<T>::type;
+    const int64_t n = nx * ny;
+    const int64_t r = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (r >= n) return;
+    const int64_t x = r % nx, y = r / nx;
+    int64_t rm, rp;
+    if (dir == 0) {
+        rm = y * nx + (x == 0 ? nx - 1 : x - 1);
+        rp = y * nx + (x == nx - 1 ? 0 : x + 1);
+    } else {
+        rm = (y == 0 ? ny - 1 : y - 1) * nx + x;
+        rp = (y == ny - 1 ? 0 : y + 1) * nx + x;
+    }
+    const T half = (T)0.5;
+    for (int j = 0; j < 5; ++j) {
+        const V* pa = src + (int64_t)(2 * j + sigma) * n;
+        const V* pb = src + (int64_t)(2 * j + 1 - sigma) * n;
+        const V a = pa[r], b = pb[r], am = pa[rm], bm = pb[rm], ap = pa[rp], bp = pb[rp];
+        // a'(r) = (1/2)[-i a + b + i a(r-e) + b(r-e)],  b'(r) = (1/2)[a(r+e) + i b(r+e) + a - i b]
+        V za, zb;
+        za.x = half * ((a.y + b.x) + (bm.x - am.y));
+        za.y = half * ((b.y - a.x) + (am.x + bm.y));
+        zb.x = half * ((ap.x - bp.y) + (a.x + b.y));
+        zb.y = half * ((ap.y + bp.x) + (a.y - b.x));
+        dst[(int64_t)(2 * j + sigma) * n + r] = za;
+        dst[(int64_t)(2 * j + 1 - sigma) * n + r] = zb;
+    }
+}
+
+cudaError_t launch_interaction(const Launch& L, qlga_prec prec, void* q, int64_t nx, int64_t ny,
+                               const double g[3], const ExpTable& tab) {
+    const int64_t n = nx * ny;
+    const unsigned blocks = (unsigned)((n + 127) / 128);
+    if (prec == QLGA_F64) {
+        UConst<double> uc{g[0], g[1], g[2]};
+        interaction_kernel<double><<<blocks, 128, 0, L.stream>>>((double2*)q, n, uc, tab);
+    } else {
+        UConst<float> uc{(float)g[0], (float)g[1], (float)g[2]};
+        interaction_kernel<float><<<blocks, 128, 0, L.stream>>>((float2*)q, n, uc, tab);
+    }
+    ++*L.counter;
+    return cudaGetLastError();
+}
+
+cudaError_t launch_kinetic(const Launch& L, qlga_prec prec, const void* src, void* dst,
+                           int64_t nx, int64_t ny, int dir, int sigma) {
+    const int64_t n = nx * ny;
+    const unsigned blocks = (unsigned)((n + 127) / 128);
+    if (prec == QLGA_F64)
+        kinetic_kernel<double><<<blocks, 128, 0, L.stream>>>((const double2*)src, (double2*)dst, nx, ny, dir, sigma);
+    else
+        kinetic_kernel<float><<<blocks, 128, 0, L.stream>>>((const float2*)src, (float2*)dst, nx, ny, dir, sigma);
+    ++*L.counter;
+    return cudaGetLastError();
+}
+
+}  // namespace qlga

@@ -1,0 +1,223 @@
+"""Thin Python binding of the C ABI in include/qlga.h (argument marshalling only).
+
+Every step of the path runs in the CUDA kernels of libqlga.so; torch is used for
+device memory and streams.  Importing this module fails loudly if the shared
+library has not been built (python -m paper_1907_12834_b200.build): there is no
+CPU fallback.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_LIB_PATH = os.path.join(_HERE, "libqlga.so")
+
+QLGA_OK, QLGA_EINVAL, QLGA_ENOMEM, QLGA_ECUDA, QLGA_ESTATE, QLGA_EUNSUP = range(6)
+QLGA_F64, QLGA_F32 = 0, 1
+QLGA_PLAIN, QLGA_INTERLEAVED = 0, 1
+OPT_PATH, OPT_STEPS_PER_LAUNCH, OPT_EXP_TOL_LOG2, OPT_THREADS_X, OPT_TILE_Y = range(5)
+
+ABI_SYMBOLS = (
+    "qlga_init", "qlga_state_bytes", "qlga_set_option", "qlga_set_state_psi", "qlga_set_state_q",
+    "qlga_get_state_q", "qlga_get_state_psi", "qlga_step", "qlga_observables", "qlga_vorticity",
+    "qlga_launch_count", "qlga_last_error", "qlga_destroy", "qlga_version",
+    "qlga_profile_enable", "qlga_profile_read",
+)
+
+
+class QlgaObs(ctypes.Structure):
+    _fields_ = [("n_m", ctypes.c_double * 5), ("norm_psi", ctypes.c_double), ("norm_q", ctypes.c_double),
+                ("F", ctypes.c_double * 3), ("A00_re", ctypes.c_double), ("A00_im", ctypes.c_double),
+                ("A00_abs2", ctypes.c_double), ("e_kin", ctypes.c_double), ("e_c0", ctypes.c_double),
+                ("e_c1", ctypes.c_double), ("e_c2", ctypes.c_double), ("e_total", ctypes.c_double),
+                ("e_dt_re", ctypes.c_double), ("e_dt_im", ctypes.c_double), ("step", ctypes.c_int64)]
+
+
+class QlgaProfile(ctypes.Structure):
+    _fields_ = [("ms", ctypes.c_double * 3), ("launches", ctypes.c_int64 * 3)]
+
+
+class QlgaError(RuntimeError):
+    def __init__(self, status, text):
+        super().__init__(f"qlga status {status}: {text}")
+        self.status = status
+
+
+def load_library():
+    if not os.path.exists(_LIB_PATH):
+        raise ImportError(f"{_LIB_PATH} is missing: build it with "
+                          "`python -m paper_1907_12834_b200.build` (needs nvcc); there is no CPU fallback")
+    lib = ctypes.CDLL(_LIB_PATH)
+    P, I, I64, D, SZ = ctypes.c_void_p, ctypes.c_int, ctypes.c_int64, ctypes.c_double, ctypes.c_size_t
+    lib.qlga_init.argtypes = [ctypes.POINTER(P), I, ctypes.POINTER(I64), D, D, D, I, I, P, P, P, SZ, P]
+    lib.qlga_init.restype = I
+    lib.qlga_state_bytes.argtypes = [I, ctypes.POINTER(I64), I]
+    lib.qlga_state_bytes.restype = SZ
+    lib.qlga_set_option.argtypes = [P, I, I64]
+    lib.qlga_set_option.restype = I
+    for name in ("qlga_set_state_psi", "qlga_set_state_q", "qlga_get_state_q", "qlga_get_state_psi",
+                 "qlga_vorticity"):
+        fn = getattr(lib, name)
+        fn.argtypes = [P, P, I]
+        fn.restype = I
+    lib.qlga_step.argtypes = [P, I64]
+    lib.qlga_step.restype = I
+    lib.qlga_observables.argtypes = [P, ctypes.POINTER(QlgaObs)]
+    lib.qlga_observables.restype = I
+    lib.qlga_launch_count.argtypes = [P]
+    lib.qlga_launch_count.restype = I64
+    lib.qlga_last_error.argtypes = [P]
+    lib.qlga_last_error.restype = ctypes.c_char_p
+    lib.qlga_destroy.argtypes = [P]
+    lib.qlga_destroy.restype = I
+    lib.qlga_profile_enable.argtypes = [P, I]
+    lib.qlga_profile_enable.restype = I
+    lib.qlga_profile_read.argtypes = [P, ctypes.POINTER(QlgaProfile)]
+    lib.qlga_profile_read.restype = I
+    lib.qlga_version.argtypes = []
+    lib.qlga_version.restype = ctypes.c_char_p
+    return lib
+
+
+_lib = load_library()
+
+
+def version() -> str:
+    return _lib.qlga_version().decode()
+
+
+def state_bytes(ndim, dims, prec) -> int:
+    d = (ctypes.c_int64 * 2)(int(dims[0]), int(dims[1]))
+    return int(_lib.qlga_state_bytes(int(ndim), d, int(prec)))
+
+
+class Qlga:
+    """One lattice on one GPU.  dims = (Nx, Ny) (Ny = 1 in 1D); couplings = (c0, c1, c2)
+    = the paper's (g0, g1, g2); order "plain" (eq. 108) or "interleaved" (eq. 112);
+    precision "f64" or "f32".  `keep_previous=True` allocates the third buffer that
+    eq. (85)'s energy needs in 2D."""
+
+    def __init__(self, ndim, dims, couplings, order="interleaved", precision="f64",
+                 device="cuda:0", stream=None, keep_previous=False):
+        import torch
+        if not torch.cuda.is_available():
+            raise RuntimeError("qlga needs a CUDA device (B200, sm_100a); there is no CPU fallback")
+        self.torch = torch
+        self.ndim = int(ndim)
+        self.nx, self.ny = int(dims[0]), int(dims[1])
+        self.prec = QLGA_F64 if precision in ("f64", "fp64", "double") else QLGA_F32
+        self.order = QLGA_INTERLEAVED if order in ("interleaved", 1) else QLGA_PLAIN
+        self.device = torch.device(device)
+        self.rdtype = torch.float64 if self.prec == QLGA_F64 else torch.float32
+        self.np_cdtype = np.complex128 if self.prec == QLGA_F64 else np.complex64
+        self.np_rdtype = np.float64 if self.prec == QLGA_F64 else np.float32
+        nbytes = state_bytes(self.ndim, (self.nx, self.ny), self.prec)
+        if nbytes == 0:
+            raise QlgaError(QLGA_EINVAL, "bad ndim/dims")
+        nreal = nbytes // (8 if self.prec == QLGA_F64 else 4)
+        with torch.cuda.device(self.device):
+            nbuf = 3 if (keep_previous and self.ndim == 2) else 2
+            self.bufs = [torch.empty(nreal, dtype=self.rdtype, device=self.device) for _ in range(nbuf)]
+            self.stream = stream if stream is not None else torch.cuda.current_stream(self.device)
+            dims_c = (ctypes.c_int64 * 2)(self.nx, self.ny)
+            ctx = ctypes.c_void_p()
+            c0, c1, c2 = (float(v) for v in couplings)
+            st = _lib.qlga_init(ctypes.byref(ctx), self.ndim, dims_c, c0, c1, c2, self.order, self.prec,
+                                self.bufs[0].data_ptr(), self.bufs[1].data_ptr(),
+                                self.bufs[2].data_ptr() if nbuf == 3 else None, nbytes,
+                                ctypes.c_void_p(self.stream.cuda_stream))
+        if st != QLGA_OK:
+            raise QlgaError(st, _lib.qlga_last_error(None).decode())
+        self.ctx = ctx
+
+    # -- plumbing ----------------------------------------------------------
+    def _check(self, st):
+        if st != QLGA_OK:
+            raise QlgaError(st, _lib.qlga_last_error(self.ctx).decode())
+
+    def _ptr(self, a):
+        """(pointer, on_device) of a numpy array or torch tensor."""
+        if isinstance(a, np.ndarray):
+            assert a.flags["C_CONTIGUOUS"]
+            return a.ctypes.data, 0
+        assert a.is_contiguous()
+        return a.data_ptr(), int(a.is_cuda)
+
+    def close(self):
+        if getattr(self, "ctx", None):
+            _lib.qlga_destroy(self.ctx)
+            self.ctx = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def set_option(self, key, value):
+        self._check(_lib.qlga_set_option(self.ctx, int(key), int(value)))
+
+    # -- state -------------------------------------------------------------
+    def set_state_psi(self, psi):
+        if isinstance(psi, np.ndarray):
+            psi = np.ascontiguousarray(psi, dtype=self.np_cdtype)
+            assert psi.shape == (5, self.ny, self.nx), psi.shape
+        p, dev = self._ptr(psi)
+        self._check(_lib.qlga_set_state_psi(self.ctx, p, dev))
+
+    def set_state_q(self, q):
+        if isinstance(q, np.ndarray):
+            q = np.ascontiguousarray(q, dtype=self.np_cdtype)
+            assert q.shape == (5, 2, self.ny, self.nx), q.shape
+        p, dev = self._ptr(q)
+        self._check(_lib.qlga_set_state_q(self.ctx, p, dev))
+
+    def get_state_q(self, out=None):
+        if out is None:
+            out = np.empty((5, 2, self.ny, self.nx), dtype=self.np_cdtype)
+        p, dev = self._ptr(out)
+        self._check(_lib.qlga_get_state_q(self.ctx, p, dev))
+        return out
+
+    def get_state_psi(self, out=None):
+        if out is None:
+            out = np.empty((5, self.ny, self.nx), dtype=self.np_cdtype)
+        p, dev = self._ptr(out)
+        self._check(_lib.qlga_get_state_psi(self.ctx, p, dev))
+        return out
+
+    # -- evolution and diagnostics -----------------------------------------
+    def step(self, n=1):
+        self._check(_lib.qlga_step(self.ctx, int(n)))
+
+    def observables(self):
+        ob = QlgaObs()
+        self._check(_lib.qlga_observables(self.ctx, ctypes.byref(ob)))
+        return {"n_p2": ob.n_m[0], "n_p1": ob.n_m[1], "n_0": ob.n_m[2], "n_m1": ob.n_m[3], "n_m2": ob.n_m[4],
+                "norm_psi": ob.norm_psi, "norm_q": ob.norm_q, "F_x": ob.F[0], "F_y": ob.F[1], "F_z": ob.F[2],
+                "A00_re": ob.A00_re, "A00_im": ob.A00_im, "A00_abs2": ob.A00_abs2, "e_kin": ob.e_kin,
+                "e_c0": ob.e_c0, "e_c1": ob.e_c1, "e_c2": ob.e_c2, "e_total": ob.e_total,
+                "e_dt_re": ob.e_dt_re, "e_dt_im": ob.e_dt_im, "step": ob.step}
+
+    def vorticity(self, out=None):
+        if out is None:
+            out = np.empty((5, self.ny, self.nx), dtype=self.np_rdtype)
+        p, dev = self._ptr(out)
+        self._check(_lib.qlga_vorticity(self.ctx, p, dev))
+        return out
+
+    def profile_enable(self, on=True):
+        self._check(_lib.qlga_profile_enable(self.ctx, int(bool(on))))
+
+    def profile_read(self):
+        """{'x_pass': (ms, launches), 'y_pass': ..., 'per_operator': ...} since the last read."""
+        pr = QlgaProfile()
+        self._check(_lib.qlga_profile_read(self.ctx, ctypes.byref(pr)))
+        names = ("x_pass", "y_pass", "per_operator")
+        return {n: (pr.ms[k], int(pr.launches[k])) for k, n in enumerate(names)}
+
+    def launch_count(self):
+        return int(_lib.qlga_launch_count(self.ctx))

@@ -1,0 +1,326 @@
+"""Parity of the CUDA path (through the C ABI, libqlga.so) with the CPU oracle,
+element by element on the same seeded inputs.  Needs a B200: run with -m gpu.
+
+Bar (BASELINE.json north_star): max relative L2 field error 1e-12 (fp64) and
+1e-5 (fp32) over all 10 spinor planes after the stated step counts."""
+import numpy as np
+import pytest
+
+from paper_1907_12834_b200 import inputs
+from conftest import rel_l2, norm2
+
+pytestmark = pytest.mark.gpu
+
+TOL64 = 1e-12
+TOL32 = 1e-5
+ORDERS = {"plain": 0, "interleaved": 1}
+
+
+@pytest.fixture(scope="module")
+def qlga():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    from paper_1907_12834_b200 import qlga as mod      # fails loudly if libqlga.so is missing
+    return mod
+
+
+def run_gpu(qlga, q0, ndim, couplings, order, steps, precision="f64", options=(), keep_previous=False):
+    ny, nx = q0.shape[2], q0.shape[3]
+    sim = qlga.Qlga(ndim, (nx, ny), couplings, order=order, precision=precision, keep_previous=keep_previous)
+    for k, v in options:
+        sim.set_option(k, v)
+    sim.set_state_q(q0)
+    sim.step(steps)
+    out = sim.get_state_q().astype(np.complex128)
+    sim.close()
+    return out
+
+
+# ---------------------------------------------------------------------------
+# generic lattices: several tiles and a ragged tail, tiny and degenerate sizes
+# ---------------------------------------------------------------------------
+@pytest.mark.parametrize("order", ["plain", "interleaved"])
+@pytest.mark.parametrize("L", [1, 2, 7, 119, 120, 121, 1000])
+def test_1d_random_state_matches_oracle(qlga, oracle, order, L):
+    c = (1.0, 0.3, -0.1)
+    q0 = inputs.random_spinor_state((L, 1), seed=100 + L, amplitude=0.3)
+    ref = oracle.step(q0, 1, c, ORDERS[order], 3)
+    out = run_gpu(qlga, q0, 1, c, order, 3)
+    assert rel_l2(out, ref) < TOL64
+
+
+@pytest.mark.parametrize("order", ["plain", "interleaved"])
+@pytest.mark.parametrize("dims", [(1, 1), (5, 3), (4, 57), (130, 9), (100, 70), (67, 130)])
+def test_2d_random_state_matches_oracle(qlga, oracle, order, dims):
+    c = (0.8, -0.25, 0.4)
+    q0 = inputs.random_spinor_state(dims, seed=7 + dims[0], amplitude=0.3)
+    ref = oracle.step(q0, 2, c, ORDERS[order], 2)
+    out = run_gpu(qlga, q0, 2, c, order, 2)
+    assert rel_l2(out, ref) < TOL64
+
+
+@pytest.mark.parametrize("tile_y", [1, 2, 4, 8])
+def test_2d_all_y_tilings(qlga, oracle, tile_y):
+    c = (1.0, 0.3, -0.1)
+    q0 = inputs.random_spinor_state((37, 150), seed=3, amplitude=0.2)
+    ref = oracle.step(q0, 2, c, 1, 2)
+    out = run_gpu(qlga, q0, 2, c, "interleaved", 2, options=[(qlga.OPT_TILE_Y, tile_y)])
+    assert rel_l2(out, ref) < TOL64
+    out = run_gpu(qlga, q0, 2, c, "interleaved", 2, options=[(qlga.OPT_TILE_Y, tile_y), (qlga.OPT_THREADS_X, 256)])
+    assert rel_l2(out, ref) < TOL64
+
+
+def test_large_angles_use_the_split_exponential(qlga, oracle):
+    # O(1) amplitudes and couplings: interaction angles of several radians
+    c = (0.7, -0.4, 0.9)
+    q0 = inputs.random_spinor_state((64, 1), seed=5, amplitude=1.5)
+    for order in ("plain", "interleaved"):
+        ref = oracle.step(q0, 1, c, ORDERS[order], 2)
+        assert rel_l2(run_gpu(qlga, q0, 1, c, order, 2), ref) < TOL64
+
+
+@pytest.mark.parametrize("order", ["plain", "interleaved"])
+def test_per_operator_path_matches_oracle_and_fused(qlga, oracle, order):
+    c = (1.0, 0.3, -0.1)
+    for ndim, dims in ((1, (333, 1)), (2, (40, 33))):
+        q0 = inputs.random_spinor_state(dims, seed=21, amplitude=0.3)
+        ref = oracle.step(q0, ndim, c, ORDERS[order], 2)
+        a = run_gpu(qlga, q0, ndim, c, order, 2, options=[(qlga.OPT_PATH, 1)])
+        b = run_gpu(qlga, q0, ndim, c, order, 2)
+        assert rel_l2(a, ref) < TOL64 and rel_l2(b, ref) < TOL64
+        assert rel_l2(a, b) < 1e-14
+
+
+def test_temporal_blocking_is_bit_identical(qlga):
+    c = (1.0, 0.3, -0.1)
+    w = inputs.config3(L=5000)
+    q0 = np.repeat(w.psi[:, None] / 2, 2, axis=1)
+    base = run_gpu(qlga, q0, 1, c, "interleaved", 13, options=[(qlga.OPT_STEPS_PER_LAUNCH, 1)])
+    for k in (2, 3, 5, 7):
+        out = run_gpu(qlga, q0, 1, c, "interleaved", 13, options=[(qlga.OPT_STEPS_PER_LAUNCH, k)])
+        assert np.array_equal(out, base)
+    out = run_gpu(qlga, q0, 1, c, "interleaved", 13, options=[(qlga.OPT_THREADS_X, 256), (qlga.OPT_STEPS_PER_LAUNCH, 4)])
+    assert np.array_equal(out, base)
+
+
+# ---------------------------------------------------------------------------
+# the five BASELINE.json configurations (full size where the oracle finishes in
+# seconds, reduced step counts / lattices otherwise)
+# ---------------------------------------------------------------------------
+def _q_of(w):
+    return np.repeat(w.psi[:, None] / 2, 2, axis=1)
+
+
+@pytest.mark.parametrize("order", ["plain", "interleaved"])
+def test_config1_full_length(qlga, oracle, order):
+    w = inputs.config1()
+    q0 = _q_of(w)
+    ref = oracle.step(q0, 1, w.couplings, ORDERS[order], w.steps)
+    out = run_gpu(qlga, q0, 1, w.couplings, order, w.steps)
+    assert rel_l2(out, ref) < TOL64
+    assert abs(norm2(out) / norm2(q0) - 1) < 1e-13
+    d0 = np.abs(w.psi[0, 0]) ** 2
+    dn = np.abs(out[0, 0, 0] + out[0, 1, 0]) ** 2
+    assert np.sqrt(np.sum((dn - d0) ** 2) / np.sum(d0 ** 2)) < 5e-3        # stationary profile
+
+
+def test_config2_reduced_steps_and_collision_variant(qlga, oracle):
+    w = inputs.config2()                                  # full L = 65536, 25 of 50000 steps
+    q0 = _q_of(w)
+    ref = oracle.step(q0, 1, w.couplings, 1, 25)
+    assert rel_l2(run_gpu(qlga, q0, 1, w.couplings, "interleaved", 25), ref) < TOL64
+    w = inputs.config2(L=8192, centres=(8192 / 2 - 100, 8192 / 2 + 100))   # overlapping solitons
+    q0 = _q_of(w)
+    ref = oracle.step(q0, 1, w.couplings, 1, 300)
+    assert rel_l2(run_gpu(qlga, q0, 1, w.couplings, "interleaved", 300), ref) < TOL64
+
+
+def test_config3_reduced_fp64_and_fp32(qlga, oracle):
+    w = inputs.config3(L=1 << 16)
+    q0 = _q_of(w)
+    ref = oracle.step(q0, 1, w.couplings, 1, 40)
+    assert rel_l2(run_gpu(qlga, q0, 1, w.couplings, "interleaved", 40), ref) < TOL64
+    q32 = q0.astype(np.complex64)
+    ref32 = oracle.step(q32.astype(np.complex128), 1, w.couplings, 1, 40)
+    assert rel_l2(run_gpu(qlga, q32, 1, w.couplings, "interleaved", 40, precision="f32"), ref32) < TOL32
+
+
+def test_config4_reduced(qlga, oracle):
+    w = inputs.config4(L=192, core=8.0)
+    q0 = _q_of(w)
+    for order in ("plain", "interleaved"):
+        ref = oracle.step(q0, 2, w.couplings, ORDERS[order], 12)
+        assert rel_l2(run_gpu(qlga, q0, 2, w.couplings, order, 12), ref) < TOL64
+
+
+def test_config5_reduced_fp64_and_fp32(qlga, oracle):
+    w = inputs.config5(L=160, core=6.0, spacing=24.0, offset=32.0)
+    q0 = _q_of(w)
+    ref = oracle.step(q0, 2, w.couplings, 1, 10)
+    assert rel_l2(run_gpu(qlga, q0, 2, w.couplings, "interleaved", 10), ref) < TOL64
+    q32 = q0.astype(np.complex64)
+    ref32 = oracle.step(q32.astype(np.complex128), 2, w.couplings, 1, 10)
+    assert rel_l2(run_gpu(qlga, q32, 2, w.couplings, "interleaved", 10, precision="f32"), ref32) < TOL32
+
+
+def test_fp32_plain_and_1d_random(qlga, oracle):
+    c = (1.0, 0.3, -0.1)
+    q32 = inputs.random_spinor_state((777, 1), seed=2, amplitude=0.2).astype(np.complex64)
+    for order in ("plain", "interleaved"):
+        ref = oracle.step(q32.astype(np.complex128), 1, c, ORDERS[order], 20)
+        assert rel_l2(run_gpu(qlga, q32, 1, c, order, 20, precision="f32"), ref) < TOL32
+
+
+# ---------------------------------------------------------------------------
+# full-size lattices in the launch configuration bench.py times: windowed parity
+# (the domain of dependence of a site is exactly 4 sites per step per direction)
+# ---------------------------------------------------------------------------
+def _windowed_parity(qlga, oracle, ndim, dims, couplings, q_dev_in, steps, windows, P, precision, tol):
+    import torch
+    nx, ny = dims
+    sim = qlga.Qlga(ndim, dims, couplings, order="interleaved", precision=precision)
+    sim.set_state_q(q_dev_in)
+    sim.step(steps)
+    cdt = torch.complex128 if precision == "f64" else torch.complex64
+    out_dev = torch.empty((5, 2, ny, nx), dtype=cdt, device="cuda")
+    sim.get_state_q(out_dev)
+    h = 4 * steps
+    worst = 0.0
+    for (cx, cy) in windows:
+        xs = (np.arange(cx - h, cx + P + h)) % nx
+        ys = (np.arange(cy - h, cy + P + h)) % ny if ndim == 2 else np.array([0])
+        xi = torch.as_tensor(xs, device="cuda"); yi = torch.as_tensor(ys, device="cuda")
+        patch_in = q_dev_in[:, :, yi][:, :, :, xi].cpu().numpy().astype(np.complex128)
+        patch_out = out_dev[:, :, yi][:, :, :, xi].cpu().numpy().astype(np.complex128)
+        ref = oracle.step(patch_in, ndim, couplings, 1, steps)          # periodic patch: only the centre is valid
+        if ndim == 2:
+            a, b = patch_out[:, :, h:h + P, h:h + P], ref[:, :, h:h + P, h:h + P]
+        else:
+            a, b = patch_out[:, :, :, h:h + P], ref[:, :, :, h:h + P]
+        worst = max(worst, rel_l2(a, b))
+    sim.close()
+    assert worst < tol, worst
+
+
+def test_config5_full_size_windowed(qlga, oracle):
+    import torch
+    L = 8192
+    w = inputs.config5(L=L)
+    psi = torch.from_numpy(w.psi).cuda()
+    q_dev = (psi[:, None] / 2).expand(5, 2, L, L).contiguous()
+    del psi
+    windows = [(0, 0), (L // 2 + 40, L // 2 - 260), (L - 20, L - 20), (1234, 4321)]   # wrap corners, a vortex core, bulk
+    _windowed_parity(qlga, oracle, 2, (L, L), w.couplings, q_dev, 2, windows, 24, "f64", TOL64)
+    q32 = q_dev.to(torch.complex64)
+    del q_dev
+    _windowed_parity(qlga, oracle, 2, (L, L), w.couplings, q32, 2, windows, 24, "f32", TOL32)
+
+
+def test_config3_full_size_windowed(qlga, oracle):
+    import torch
+    L = 1 << 22
+    w = inputs.config3(L=L)
+    q_dev = torch.from_numpy(_q_of(w)).cuda()
+    windows = [(0, 0), (L // 4 - 50, 0), (L - 30, 0), (3 * L // 4, 0)]
+    _windowed_parity(qlga, oracle, 1, (L, 1), w.couplings, q_dev, 5, windows, 100, "f64", TOL64)
+
+
+# ---------------------------------------------------------------------------
+# observables, vorticity, boundary behaviour
+# ---------------------------------------------------------------------------
+def test_observables_match_oracle(qlga, oracle):
+    c = (1.0, 0.3, -0.1)
+    for ndim, dims, keep in ((1, (3000, 1), False), (2, (70, 45), True), (2, (70, 45), False)):
+        q0 = inputs.random_spinor_state(dims, seed=9, amplitude=0.3)
+        sim = qlga.Qlga(ndim, dims, c, order="interleaved", keep_previous=keep)
+        sim.set_state_q(q0)
+        ob0 = sim.observables()
+        ref0 = oracle.observables(q0, ndim, c)
+        assert np.isnan(ob0["e_dt_re"]) and ob0["step"] == 0
+        for k, v in ref0.items():
+            if not k.startswith("e_dt"):
+                assert abs(ob0[k] - v) <= 1e-11 * max(1.0, abs(v)), k
+        sim.step(3)
+        q3 = sim.get_state_q()
+        q2 = oracle.step(q0, ndim, c, 1, 2)
+        ob = sim.observables()
+        ref = oracle.observables(q3, ndim, c, qprev=q2)
+        assert ob["step"] == 3
+        for k, v in ref.items():
+            if k.startswith("e_dt"):
+                if ndim == 1 or keep:
+                    assert abs(ob[k] - v) < 1e-10, k
+                else:
+                    assert np.isnan(ob[k])
+            else:
+                assert abs(ob[k] - v) <= 1e-11 * max(1.0, abs(v)), k
+        sim.close()
+
+
+def test_psi_roundtrip_and_device_transfers(qlga, oracle):
+    import torch
+    c = (1.0, 0.3, -0.1)
+    psi = inputs.random_field((50, 20), seed=4)
+    sim = qlga.Qlga(2, (50, 20), c)
+    sim.set_state_psi(psi)
+    q = sim.get_state_q()
+    assert np.array_equal(q[:, 0], psi / 2) and np.array_equal(q[:, 1], psi / 2)      # reading R6
+    assert np.array_equal(sim.get_state_psi(), psi)
+    sim.set_state_psi(torch.from_numpy(psi).cuda())
+    out = torch.empty((5, 20, 50), dtype=torch.complex128, device="cuda")
+    sim.get_state_psi(out)
+    assert np.array_equal(out.cpu().numpy(), psi)
+    sim.close()
+
+
+def test_vorticity_matches_oracle(qlga, oracle):
+    c = (1.0, 0.3, -0.1)
+    w = inputs.config4(L=96, core=6.0)
+    q0 = _q_of(w)
+    q0 += inputs.random_spinor_state((96, 96), seed=1, amplitude=1e-3)
+    for precision, tol in (("f64", 1e-12), ("f32", 1e-6)):
+        sim = qlga.Qlga(2, (96, 96), c, precision=precision)
+        qin = q0 if precision == "f64" else q0.astype(np.complex64)
+        sim.set_state_q(qin)
+        om = sim.vorticity()
+        ref = oracle.vorticity(qin.astype(np.complex128))
+        assert np.abs(om - ref).max() < tol
+        sim.step(5)
+        om = sim.vorticity()
+        ref = oracle.vorticity(sim.get_state_q().astype(np.complex128))
+        assert np.abs(om - ref).max() < tol
+        assert abs(om.sum()) < 1e-3
+        sim.close()
+
+
+def test_error_paths(qlga):
+    c = (1.0, 0.3, -0.1)
+    sim = qlga.Qlga(1, (64, 1), c)
+    with pytest.raises(qlga.QlgaError) as e:
+        sim.step(1)
+    assert e.value.status == qlga.QLGA_ESTATE
+    sim.set_state_psi(inputs.random_field((64, 1), seed=1))
+    with pytest.raises(qlga.QlgaError) as e:
+        sim.vorticity()
+    assert e.value.status == qlga.QLGA_EUNSUP
+    with pytest.raises(qlga.QlgaError) as e:
+        sim.step(-1)
+    assert e.value.status == qlga.QLGA_EINVAL
+    with pytest.raises(qlga.QlgaError):
+        sim.set_option(qlga.OPT_TILE_Y, 3)
+    before = sim.get_state_q()
+    sim.step(0)
+    assert np.array_equal(sim.get_state_q(), before)
+    assert sim.launch_count() >= 1
+    sim.close()
+    with pytest.raises(qlga.QlgaError):
+        qlga.Qlga(1, (64, 2), c)
+
+
+def test_gpu_unitarity_1000_steps(qlga):
+    c = (1.0, 0.3, -0.1)
+    psi = inputs.smooth_random_field((4096, 1), seed=4, amplitude=0.08)
+    q0 = np.repeat(psi[:, None] / 2, 2, axis=1) + inputs.random_spinor_state((4096, 1), seed=6, amplitude=1e-3)
+    for order in ("plain", "interleaved"):
+        out = run_gpu(qlga, q0, 1, c, order, 1000)
+        assert abs(norm2(out) / norm2(q0) - 1) < 1e-13

@@ -32,7 +32,7 @@ def test_pade_default_coefficients_are_table3_at_E_equal_g():
     s = np.array([0.0, 0.5, 3.0, 50.0])
     ref = np.sqrt((a2 * s**4 + a1 * s**2) / (a2 * s**4 + b1 * s**2 + 1))
     assert np.allclose(inputs.pade_profile(s), ref)
-    assert inputs.pade_profile(np.array([1e3]))[0] < 1.0      # b1 > a1: approaches 1 from below
+    assert abs(inputs.pade_profile(np.array([1e3]))[0] - 1.0) < 1e-5 and inputs.pade_profile(np.array([0.0]))[0] == 0.0
 
 
 def test_configs_shapes_seeds_and_structure():
