@@ -231,3 +231,192 @@ def run_reference(args, w, ndim, config):
             "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
     print(json.dumps(line))
+
+
+# ---------------------------------------------------------------------------
+# this repo's arm
+# ---------------------------------------------------------------------------
+def main():
+    args = parse_args()
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    wl = WORKLOADS[args.workload]
+    ndim = wl["ndim"]
+
+    if args.impl == "reference" and rank != 0:
+        return                                              # rank 0 alone runs the oracle arm
+    w = wl["gen"](args.lattice)
+    nx, ny = w.dims
+    sites = nx * ny
+    inner = args.inner or max(1, min(1000, int(6.0e8 / sites)))   # ~0.5 s of GPU work per bench step
+    config = {"workload": f"{w.name} (BASELINE.json configs[{int(args.workload[3]) - 1}]): "
+                          f"{'2D' if ndim == 2 else '1D'} periodic {nx}x{ny}, {args.precision}, "
+                          f"{args.order} ordering (eq. {'112' if args.order == 'interleaved' else '108'})",
+              "lattice": [nx, ny], "precision": args.precision, "order": args.order,
+              "couplings": list(w.couplings), "time_steps_per_bench_step": inner,
+              "per_bench_step": f"{inner} time steps + 1 observables reduction" + (" + 1 vorticity map" if ndim == 2 else ""),
+              "l2_policy": "state (%.1f GB per buffer) larger than the 126 MB L2" % (sites * 160 / 1e9 * (1 if args.precision == 'f64' else 0.5))
+                           if sites * 80 > 126e6 else "state fits in L2 (latency-bound workload; no HBM claim)",
+              "parallelism": f"replicas x{args.gpus} (one lattice per GPU, no data-path collective)"}
+    if args.impl == "reference":
+        run_reference(args, w, ndim, config)
+        return
+
+    import torch
+    from paper_1907_12834_b200 import qlga                  # fails loudly without libqlga.so
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device; there is no CPU fallback")
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=dev)
+
+    def barrier():
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    cdt = torch.complex128 if args.precision == "f64" else torch.complex64
+    # host input in pinned memory: q1 = q2 = psi/2 (reading R6)
+    q_host = torch.empty((5, 2, ny, nx), dtype=cdt, pin_memory=True)
+    half = torch.from_numpy(w.psi / 2).to(cdt)
+    q_host[:, 0] = half
+    q_host[:, 1] = half
+    del half
+    out_host = torch.empty_like(q_host, pin_memory=True) if not args.no_e2e else None
+
+    sim = qlga.Qlga(ndim, (nx, ny), w.couplings, order=args.order, precision=args.precision, device=dev)
+    if args.tile_y:
+        sim.set_option(qlga.OPT_TILE_Y, args.tile_y)
+    if args.threads_x:
+        sim.set_option(qlga.OPT_THREADS_X, args.threads_x)
+    omega_dev = (torch.empty((5, ny, nx), dtype=torch.float64 if args.precision == "f64" else torch.float32,
+                             device=dev) if ndim == 2 else None)
+    state_bytes = q_host.numel() * q_host.element_size()
+
+    def hot_path_step():
+        sim.step(inner)
+        obs = sim.observables()
+        if omega_dev is not None:
+            sim.vorticity(omega_dev)
+        return obs
+
+    # ---- device-resident measurement -------------------------------------------------
+    sim.set_state_q(q_host.numpy())
+    obs0 = sim.observables()
+    for _ in range(max(3, args.warmup)):
+        hot_path_step()
+    sim.profile_enable(True)
+    sampler = ClockSampler(local_rank)
+    barrier()
+    sampler.start()
+    launches0 = sim.launch_count()
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    ev0.record()
+    for _ in range(args.steps):
+        obs = hot_path_step()
+    ev1.record()
+    barrier()
+    clocks = sampler.stop()
+    launches = sim.launch_count() - launches0
+    ms = ev0.elapsed_time(ev1)
+    prof = sim.profile_read()
+    sim.profile_enable(False)
+    if world > 1:
+        t = torch.tensor([ms], device=dev, dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms = float(t.item())
+    value = sites * inner * args.steps * world / (ms * 1e-3) / 1e9
+
+    # ---- end to end through the C ABI with host buffers ---------------------------------
+    e2e = None
+    if not args.no_e2e:
+        def e2e_step():
+            sim.set_state_q(q_host.numpy())                 # H2D from pinned host memory
+            sim.step(inner)
+            o = sim.observables()
+            sim.get_state_q(out_host.numpy())               # D2H of the step's result
+            return o
+        e2e_step()
+        barrier()
+        t0 = time.perf_counter()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for _ in range(args.e2e_steps):
+            e2e_step()
+        e1.record()
+        barrier()
+        wall = time.perf_counter() - t0
+        ems = max(e0.elapsed_time(e1), 0.0)
+        if world > 1:
+            t = torch.tensor([ems], device=dev, dtype=torch.float64)
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            ems = float(t.item())
+        e2e = {"value": sites * inner * args.e2e_steps * world / (ems * 1e-3) / 1e9, "unit": UNIT,
+               "h2d_bytes_per_step": state_bytes, "d2h_bytes_per_step": state_bytes + 168,
+               "steps": args.e2e_steps, "ms_per_step": ems / args.e2e_steps,
+               "wall_ms_per_step": wall * 1e3 / args.e2e_steps,
+               "call": "qlga_set_state_q(host) + qlga_step(n) + qlga_observables + qlga_get_state_q(host)"}
+
+    if rank != 0:
+        return
+
+    # ---- roofline of the dominant kernel (the pass kernels) -----------------------------
+    hbm_peak, peak_kind, sm_max = load_peaks()
+    bps = bytes_per_site_update(args.precision)
+    kinds = {k: v for k, v in prof.items() if v[1] > 0}
+    dom = max(kinds, key=lambda k: kinds[k][0]) if kinds else None
+    pass_ms = sum(v[0] for v in kinds.values())
+    roof = None
+    roof_hbm = None
+    if dom:
+        dms, dn = kinds[dom]
+        per_launch_ms = dms / dn
+        # a pass launch advances every site by 1/ndim of a time step (times the fused steps in 1D)
+        units = sites * inner * args.steps / (ndim * dn)      # site-updates per launch
+        deg = expected_degree(w, ndim, args.order, args.precision)
+        fpi = fp_instr_per_site_update(ndim, args.order, deg)
+        lanes = 64 if args.precision == "f64" else 128       # FP64 / FP32 FMA lanes per SM per clock
+        clk = (clocks.get("sm_mhz") or sm_max) * 1e6
+        alu_peak = 148 * lanes * clk / 1e12                  # T instr/s at the clock seen under load
+        alu_ach = units * fpi / (per_launch_ms * 1e-3) / 1e12
+        hbm_ach = units * bps / (per_launch_ms * 1e-3) / 1e9
+        roof_hbm = {"bound": "hbm", "achieved": hbm_ach, "peak": hbm_peak, "unit": "GB/s",
+                    "frac": hbm_ach / hbm_peak, "traffic": None, "peak_kind": peak_kind,
+                    "kernel": dom, "ms_per_launch": per_launch_ms,
+                    "model": f"{bps:.0f} B per site-update x {units:.3g} site-updates per launch"}
+        roof_alu = {"bound": "alu", "achieved": alu_ach, "peak": alu_peak, "unit": "Tinstr/s",
+                    "frac": alu_ach / alu_peak, "traffic": None, "kernel": dom,
+                    "ms_per_launch": per_launch_ms,
+                    "model": f"{fpi:.0f} FP instr per site-update (degree {deg:.0f}) x {units:.3g} site-updates per launch; "
+                             f"peak = 148 SMs x {lanes} lanes x {clk / 1e6:.0f} MHz (median clock under load)"}
+        # the binding roofline is the one with the larger fraction
+        roof = roof_alu if roof_alu["frac"] > roof_hbm["frac"] else roof_hbm
+        if roof is roof_alu:
+            roof["hbm_model"] = roof_hbm
+        else:
+            roof["alu_model"] = roof_alu
+
+    cpu = None
+    if world == 1 and not args.no_cpu_baseline:
+        rate, sample, _, _ = time_oracle(w, ndim, args.order, args.cpu_seconds)
+        cpu = {"value": rate / 1e9, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample}
+
+    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": max(3, args.warmup), "ms_per_step": ms / args.steps, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": args.precision, "data": "synthetic",
+            "config": config, "clocks": clocks, "e2e": e2e, "gpu_launches": launches,
+            "roofline": roof, "cpu_baseline": cpu,
+            "hbm_model_frac": value / world * 1e9 * bps / (hbm_peak * 1e9),
+            "kernel_ms": {k: {"ms_total": v[0], "launches": v[1]} for k, v in prof.items()},
+            "pass_kernel_share_of_step": pass_ms / ms if ms > 0 else None,
+            "norm_q_drift": obs["norm_q"] / obs0["norm_q"] - 1.0,
+            "sim_step": obs["step"]}
+    print(json.dumps(line))
+
+
+if __name__ == "__main__":
+    main()
