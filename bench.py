@@ -59,6 +59,8 @@ def parse_args():
     ap.add_argument("--cpu-seconds", type=float, default=15.0, help="target CPU time of the oracle sample")
     ap.add_argument("--tile-y", type=int, default=0)
     ap.add_argument("--threads-x", type=int, default=0)
+    ap.add_argument("--threads-y", type=int, default=0)
+    ap.add_argument("--tol-log2", type=int, default=0, help="QLGA_OPT_EXP_TOL_LOG2 override (experiments only)")
     return ap.parse_args()
 
 
@@ -293,6 +295,10 @@ def main():
         sim.set_option(qlga.OPT_TILE_Y, args.tile_y)
     if args.threads_x:
         sim.set_option(qlga.OPT_THREADS_X, args.threads_x)
+    if args.threads_y:
+        sim.set_option(qlga.OPT_THREADS_Y, args.threads_y)
+    if args.tol_log2:
+        sim.set_option(qlga.OPT_EXP_TOL_LOG2, args.tol_log2)
     omega_dev = (torch.empty((5, ny, nx), dtype=torch.float64 if args.precision == "f64" else torch.float32,
                              device=dev) if ndim == 2 else None)
     state_bytes = q_host.numel() * q_host.element_size()

@@ -58,8 +58,10 @@ typedef enum {
     QLGA_OPT_PATH = 0,        /* 0 = fused pass kernels (default), 1 = one kernel per operator   */
     QLGA_OPT_STEPS_PER_LAUNCH = 1, /* 1D only: time steps fused per launch (halo 4 per step); 0 = auto */
     QLGA_OPT_EXP_TOL_LOG2 = 2,/* truncation target of the interaction exponential, log2 (default -56 / -27) */
-    QLGA_OPT_THREADS_X = 3,   /* CTA size of the x pass: 128 or 256; 0 = auto                    */
-    QLGA_OPT_TILE_Y = 4       /* y pass: columns per CTA (1,2,4,8); 0 = auto                     */
+    QLGA_OPT_THREADS_X = 3,   /* CTA size of the x pass: 128, 192 or 256; 0 = auto               */
+    QLGA_OPT_TILE_Y = 4,      /* y pass: columns per CTA (1,2,4,8); 0 = auto                     */
+    QLGA_OPT_THREADS_Y = 5    /* CTA size of the y pass: 128, 192 or 256 (valid pairs with TILE_Y: 1x128, 1x192,
+                                 2x128, 2x192, 2x256, 4x256, 8x256); 0 = auto */
 } qlga_option;
 
 /* Lattice sums returned by qlga_observables (always double).

@@ -138,8 +138,11 @@ extern "C" qlga_status qlga_set_option(qlga_ctx* c, qlga_option key, int64_t v) 
             if (v > -8 || v < -100) return fail(c, QLGA_EINVAL, "QLGA_OPT_EXP_TOL_LOG2: -100..-8");
             c->tol_log2 = (int)v; build_exp_table(c->tab, c->tol_log2); return QLGA_OK;
         case QLGA_OPT_THREADS_X:
-            if (v != 0 && v != 128 && v != 256) return fail(c, QLGA_EINVAL, "QLGA_OPT_THREADS_X: 0, 128, 256");
+            if (v != 0 && v != 128 && v != 192 && v != 256) return fail(c, QLGA_EINVAL, "QLGA_OPT_THREADS_X: 0, 128, 192, 256");
             c->threads_x = (int)v; return QLGA_OK;
+        case QLGA_OPT_THREADS_Y:
+            if (v != 0 && v != 128 && v != 192 && v != 256) return fail(c, QLGA_EINVAL, "QLGA_OPT_THREADS_Y: 0, 128, 192, 256");
+            c->threads_y = (int)v; return QLGA_OK;
         case QLGA_OPT_TILE_Y:
             if (v != 0 && v != 1 && v != 2 && v != 4 && v != 8) return fail(c, QLGA_EINVAL, "QLGA_OPT_TILE_Y: 0,1,2,4,8");
             c->tile_y = (int)v; return QLGA_OK;
@@ -336,7 +339,7 @@ static qlga_status step_fused(qlga_ctx* c, int64_t nsteps) {
         P.src = c->buf[c->cur]; P.dst = c->buf[mid];
         P.umode = inter ? 2 : 1;                                       // U is the rightmost operator
         prof_mark(c, 1);
-        CU(c, launch_pass(L, c->prec, 1, P, 0, c->tile_y));
+        CU(c, launch_pass(L, c->prec, 1, P, c->threads_y, c->tile_y));
         P.src = c->buf[mid]; P.dst = c->buf[dst];
         P.umode = inter ? 2 : 0;
         prof_mark(c, 0);

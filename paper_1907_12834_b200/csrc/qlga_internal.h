@@ -75,6 +75,7 @@ struct qlga_ctx {
     int tol_log2;
     int threads_x;
     int tile_y;
+    int threads_y;
     qlga::ExpTable tab;
     // scratch owned by the library
     double* d_partials;    // [obs_blocks][OBS_NACC]

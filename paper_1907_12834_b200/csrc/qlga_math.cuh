@@ -40,8 +40,29 @@ template <typename T> __device__ __forceinline__ cx<T> cfma_conj(cx<T> a, cx<T> 
     return acc;
 }
 
-__device__ __forceinline__ void sincos_t(double x, double* s, double* c) { sincos(x, s, c); }
-__device__ __forceinline__ void sincos_t(float x, float* s, float* c) { sincosf(x, s, c); }
+// sin/cos of the scalar interaction phase for |x| <= 2^-4 (always the case at the
+// paper's scaled amplitudes): Taylor polynomials in x^2 to x^13 / x^14, remainder
+// < 2^-80, branch free so that the chain interleaves with the spin-density arithmetic.
+template <typename T>
+__device__ __forceinline__ void sincos_small(T x, T* s, T* c) {
+    const T z = x * x;
+    T ps = fma(z, (T)(-1.0 / 156.0), (T)1);
+    T pc = fma(z, (T)(-1.0 / 182.0), (T)1);
+    ps = fma(z * (T)(-1.0 / 110.0), ps, (T)1);
+    pc = fma(z * (T)(-1.0 / 132.0), pc, (T)1);
+    ps = fma(z * (T)(-1.0 / 72.0), ps, (T)1);
+    pc = fma(z * (T)(-1.0 / 90.0), pc, (T)1);
+    ps = fma(z * (T)(-1.0 / 42.0), ps, (T)1);
+    pc = fma(z * (T)(-1.0 / 56.0), pc, (T)1);
+    ps = fma(z * (T)(-1.0 / 20.0), ps, (T)1);
+    pc = fma(z * (T)(-1.0 / 30.0), pc, (T)1);
+    ps = fma(z * (T)(-1.0 / 6.0), ps, (T)1);
+    pc = fma(z * (T)(-1.0 / 12.0), pc, (T)1);
+    *s = x * ps;
+    *c = fma(z * (T)-0.5, pc, (T)1);
+}
+__device__ __forceinline__ void sincos_lib(double x, double* s, double* c) { sincos(x, s, c); }
+__device__ __forceinline__ void sincos_lib(float x, float* s, float* c) { sincosf(x, s, c); }
 
 // Site state: q[j][sigma], j = 0..4 <-> m = +2..-2.
 template <typename T> struct Site {
@@ -136,6 +157,17 @@ __device__ __forceinline__ void apply_sK(const cx<T> u[5], cx<T> w[5], T az, cx<
 // Apply U^{(s)} to one site.  The site may carry a power-of-two scale 2^e; the
 // caller passes constants multiplied by 4^-e, which makes the result identical
 // (bit for bit, barring under/overflow) to applying U to the unscaled site.
+// number of thresholds thr[0..PMAX-2] (ascending) that theta exceeds, by bisection
+__device__ __forceinline__ int count_below(const float* thr, float theta) {
+    int lo = 0, hi = QLGA_PMAX - 1;              // answer in [lo, hi]
+#pragma unroll
+    for (int it = 0; it < 5; ++it) {
+        const int mid = (lo + hi) >> 1;
+        if (lo < hi) { if (theta > thr[mid]) lo = mid + 1; else hi = mid; }
+    }
+    return lo;
+}
+
 template <typename T>
 __device__ __forceinline__ void interaction(Site<T>& s, const UConst<T>& uc, const ExpTable& tab) {
     cx<T> psi[5];
@@ -156,53 +188,70 @@ __device__ __forceinline__ void interaction(Site<T>& s, const UConst<T>& uc, con
     const T rt6 = (T)2.4494897427831780981972840747059;
     const cx<T> Fp = mk<T>(fma(rt6, fb.re, (T)2 * fa.re), fma(rt6, fb.im, (T)2 * fa.im));
 
-    // angle bound theta = 2 |g1| |F| + |g2| rho  (spectral norms of the two parts)
+    // angle bound theta = 2 |g1| |F| + |g2| rho  (spectral norms of the two parts),
+    // made warp-uniform (one degree per warp keeps the Horner loops convergent)
     const float Fabs = sqrtf((float)(Fz * Fz + Fp.re * Fp.re + Fp.im * Fp.im));
     float theta = 2.0f * fabsf((float)uc.g1) * Fabs + fabsf((float)uc.g2) * (float)rho;
     theta *= 1.0009765625f;                       // cover the float rounding of the estimate
-    int nsub = 1;
-    if (theta > tab.theta_split) {
-        nsub = (int)ceilf(theta / tab.theta_split);
-        theta = theta / (float)nsub * 1.0009765625f;
-    }
-    int p = 1;
-#pragma unroll
-    for (int k = 0; k < QLGA_PMAX - 1; ++k) p += (theta > tab.thr[k]) ? 1 : 0;
-    p = __reduce_max_sync(0xffffffffu, p);       // warp-uniform trip count
-    nsub = __reduce_max_sync(0xffffffffu, nsub);
+    theta = __uint_as_float(__reduce_max_sync(0xffffffffu, __float_as_uint(theta)));
 
-    const T inv_nsub = (T)1 / (T)nsub;
-    const T g1 = uc.g1 * inv_nsub, g2 = uc.g2 * inv_nsub;
-    const T az = g1 * Fz;
-    const cx<T> a1 = mk<T>(g1 * Fp.re, g1 * Fp.im);
-    const T h6 = g1 * (T)1.2247448713915890490986420373529;      // sqrt(6)/2
-    const cx<T> a6 = mk<T>(h6 * Fp.re, h6 * Fp.im);
-
-    // scalar phase exp(-i s c0 rho)
+    // Fast path, branch free (one basic block, so the independent chains below
+    // interleave): one application, small scalar phase.
+    const T xph = uc.g0 * rho;                    // scalar phase exp(-i s c0 rho)
     T sn, cs;
-    sincos_t(uc.g0 * rho, &sn, &cs);
+    sincos_small<T>(xph, &sn, &cs);
+    T g2 = uc.g2;
+    T az = uc.g1 * Fz;
+    cx<T> a1 = mk<T>(uc.g1 * Fp.re, uc.g1 * Fp.im);
+    const T rt6h = (T)1.2247448713915890490986420373529;          // sqrt(6)/2
+    cx<T> a6 = mk<T>(rt6h * a1.re, rt6h * a1.im);
+    int p = 1 + count_below(tab.thr, theta);
+    int nsub = 1;
+    // Rare path (never at the paper's amplitudes): large scalar phase -> library sincos;
+    // angle above theta_split -> nsub equal sub-angles (exact: K is frozen).
+    const bool big_phase = !__all_sync(0xffffffffu, fabs(xph) <= (T)0.0625);
+    if (big_phase || theta > tab.theta_split) {
+        if (big_phase) sincos_lib(xph, &sn, &cs);
+        if (theta > tab.theta_split) {
+            nsub = (int)ceilf(theta / tab.theta_split);
+            const T inv_nsub = (T)1 / (T)nsub;
+            g2 *= inv_nsub; az *= inv_nsub;
+            a1.re *= inv_nsub; a1.im *= inv_nsub; a6.re *= inv_nsub; a6.im *= inv_nsub;
+            p = 1 + count_below(tab.thr, theta / (float)nsub * 1.0009765625f);
+        }
+    }
     const cx<T> ph = mk<T>(cs, -sn);
 
+    // Horner form u_{k-1} = v + (-i/k) (sK) u_k, k = p..1, u_p = v, for each of the two
+    // spinor 5-vectors; psi (hence K) is frozen at its value before the application
+    // (reading R4).  Stage p acts on v itself (no copy of the site state).
 #pragma unroll
     for (int sg = 0; sg < 2; ++sg) {
-        cx<T> v[5], u[5], w[5];
-#pragma unroll
-        for (int j = 0; j < 5; ++j) { v[j] = s.q[j][sg]; u[j] = v[j]; }
+        cx<T> u[5], w[5];
         for (int rep = 0; rep < nsub; ++rep) {
-            if (rep > 0) {
+            cx<T> v[5];
 #pragma unroll
-                for (int j = 0; j < 5; ++j) v[j] = u[j];
+            for (int j = 0; j < 5; ++j) v[j] = s.q[j][sg];
+            apply_sK<T>(v, w, az, a1, a6, g2, psi);
+            {
+                const T ik = (T)tab.rcp[p];
+#pragma unroll
+                for (int j = 0; j < 5; ++j) {
+                    u[j].re = fma(ik, w[j].im, v[j].re); u[j].im = fma(-ik, w[j].re, v[j].im);
+                }
             }
-            // Horner: u_{k-1} = v + (-i/k) (sK) u_k ; psi (hence K) is frozen at its
-            // value before the application (reading R4)
-            for (int k = p; k >= 1; --k) {
+#pragma unroll 1
+            for (int k = p - 1; k >= 1; --k) {
                 apply_sK<T>(u, w, az, a1, a6, g2, psi);
                 const T ik = (T)tab.rcp[k];
 #pragma unroll
                 for (int j = 0; j < 5; ++j) {
-                    u[j].re = fma(ik, w[j].im, v[j].re);
-                    u[j].im = fma(-ik, w[j].re, v[j].im);
+                    u[j].re = fma(ik, w[j].im, v[j].re); u[j].im = fma(-ik, w[j].re, v[j].im);
                 }
+            }
+            if (rep + 1 < nsub) {               // rare: next sub-angle starts from u
+#pragma unroll
+                for (int j = 0; j < 5; ++j) s.q[j][sg] = u[j];
             }
         }
 #pragma unroll

@@ -35,8 +35,13 @@ __device__ __forceinline__ int64_t pmod(int64_t a, int64_t n) {
     return r < 0 ? r + n : r;
 }
 
+// experiment knobs (compile time)
+#ifndef QLGA_MINB128
+#define QLGA_MINB128 3
+#endif
+
 template <typename T, int DIR, int CX, int NT>
-__global__ void __launch_bounds__(NT) pass_kernel(const __grid_constant__ PassArgs<T> P) {
+__global__ void __launch_bounds__(NT, (NT >= 256 ? 2 : (NT >= 192 ? 2 : QLGA_MINB128))) pass_kernel(const __grid_constant__ PassArgs<T> P) {
     using V = typename vec2<T>::type;
     constexpr int TS = NT / CX;              // sites per line handled by the CTA
     constexpr int NW = NT / 32;
@@ -186,16 +191,24 @@ static cudaError_t launch_pass_t(const Launch& L, int dir, const PassParams& P, 
         if (threads == 0) threads = 128;
         switch (threads) {
             case 128: return run_pass<T, 0, 1, 128>(L, P);
+            case 192: return run_pass<T, 0, 1, 192>(L, P);
             case 256: return run_pass<T, 0, 1, 256>(L, P);
             default: return cudaErrorInvalidValue;
         }
     }
-    if (cxw == 0) cxw = 4;
-    switch (cxw) {
-        case 1: return run_pass<T, 1, 1, 128>(L, P);
-        case 2: return run_pass<T, 1, 2, 256>(L, P);
-        case 4: return run_pass<T, 1, 4, 256>(L, P);
-        case 8: return run_pass<T, 1, 8, 256>(L, P);
+    // defaults: fp64 is register-heavy and FP64-pipe bound: 128-thread CTAs (three per SM without
+    // spills), one column x 128 rows (least halo recompute; the half-used 32-byte sectors are
+    // completed by the neighbouring column's CTA out of L2); fp32 takes four columns x 64 rows
+    if (cxw == 0) cxw = (sizeof(T) == 8) ? 1 : 4;
+    if (threads == 0) threads = (cxw <= 2) ? 128 : 256;
+    switch (cxw * 1000 + threads) {
+        case 1128: return run_pass<T, 1, 1, 128>(L, P);
+        case 1192: return run_pass<T, 1, 1, 192>(L, P);
+        case 2128: return run_pass<T, 1, 2, 128>(L, P);
+        case 2192: return run_pass<T, 1, 2, 192>(L, P);
+        case 2256: return run_pass<T, 1, 2, 256>(L, P);
+        case 4256: return run_pass<T, 1, 4, 256>(L, P);
+        case 8256: return run_pass<T, 1, 8, 256>(L, P);
         default: return cudaErrorInvalidValue;
     }
 }

@@ -96,16 +96,18 @@ def test_per_operator_path_matches_oracle_and_fused(qlga, oracle, order):
         assert rel_l2(a, b) < 1e-14
 
 
-def test_temporal_blocking_is_bit_identical(qlga):
+def test_temporal_blocking_matches_single_step_launches(qlga):
+    # same arithmetic per site; only the (warp-uniform) polynomial degree can differ
+    # where the warp composition differs, i.e. at the 1e-17 level
     c = (1.0, 0.3, -0.1)
     w = inputs.config3(L=5000)
     q0 = np.repeat(w.psi[:, None] / 2, 2, axis=1)
     base = run_gpu(qlga, q0, 1, c, "interleaved", 13, options=[(qlga.OPT_STEPS_PER_LAUNCH, 1)])
     for k in (2, 3, 5, 7):
         out = run_gpu(qlga, q0, 1, c, "interleaved", 13, options=[(qlga.OPT_STEPS_PER_LAUNCH, k)])
-        assert np.array_equal(out, base)
+        assert rel_l2(out, base) < 1e-15
     out = run_gpu(qlga, q0, 1, c, "interleaved", 13, options=[(qlga.OPT_THREADS_X, 256), (qlga.OPT_STEPS_PER_LAUNCH, 4)])
-    assert np.array_equal(out, base)
+    assert rel_l2(out, base) < 1e-15
 
 
 # ---------------------------------------------------------------------------
@@ -174,6 +176,21 @@ def test_fp32_plain_and_1d_random(qlga, oracle):
     for order in ("plain", "interleaved"):
         ref = oracle.step(q32.astype(np.complex128), 1, c, ORDERS[order], 20)
         assert rel_l2(run_gpu(qlga, q32, 1, c, order, 20, precision="f32"), ref) < TOL32
+
+
+def test_long_run_error_growth(qlga, oracle):
+    # 150 interleaved 2D steps (1200 interaction exponentials per site) on a vortex
+    # quadrupole stay at rounding level against the oracle, norm conserved.  (Beyond
+    # ~200 steps this small, violently evolving lattice amplifies rounding differences
+    # exponentially -- the oracle's own double and long-double builds part ways at the
+    # same rate, 2.8e-12 at 300 steps; DESIGN.md section 8 -- so a longer comparison
+    # would measure the flow's sensitivity, not the kernels.)
+    w = inputs.config4(L=96, core=8.0)
+    q0 = _q_of(w)
+    ref = oracle.step(q0, 2, w.couplings, 1, 150)
+    a = run_gpu(qlga, q0, 2, w.couplings, "interleaved", 150)
+    assert rel_l2(a, ref) < 1e-13
+    assert abs(norm2(a) / norm2(q0) - 1) < 1e-13
 
 
 # ---------------------------------------------------------------------------
