@@ -143,8 +143,9 @@ def fp_instr_per_site_update(ndim, order, degree):
 
 
 def expected_degree(w, ndim, order, precision):
-    """Degree the kernel's order selection picks on the workload's background state
-    (same rule as build_exp_table / interaction(): theta = s (2|c1||F| + |c2| rho / 5))."""
+    """Degree the kernel's order selection picks on the workload's initial state (same
+    rule as interaction(): theta = s (2|c1||F| + |c2| rho / 5) against the library's
+    thresholds, qlga_exp_polynomial)."""
     psi = w.psi.reshape(5, -1)
     idx = np.linspace(0, psi.shape[1] - 1, 4096).astype(np.int64)
     p5 = psi[:, idx]
@@ -157,13 +158,11 @@ def expected_degree(w, ndim, order, precision):
     s = 1.0 / (4 * ndim) if order == "interleaved" else 1.0
     c0, c1, c2 = w.couplings
     theta = s * (2 * abs(c1) * fabs + abs(c2) / 5 * rho)
-    tol = 2.0 ** (-56 if precision == "f64" else -27)
+    from paper_1907_12834_b200 import qlga
+    tol_log2 = -56 if precision == "f64" else -27
     deg = np.ones_like(theta)
-    fact = 2.0
-    for p in range(1, 18):
-        fact_p = float(np.prod(np.arange(1, p + 2)))
-        thr = (tol * fact_p) ** (1.0 / (p + 1)) * 0.999
-        deg += theta > thr
+    for p in range(1, 12):
+        deg += theta * 1.001 > qlga.exp_polynomial(tol_log2, p)[0]
     return float(np.percentile(deg, 90))
 
 

@@ -139,6 +139,12 @@ typedef struct { double ms[3]; int64_t launches[3]; } qlga_profile;
 qlga_status qlga_profile_enable(qlga_ctx*, int on);
 qlga_status qlga_profile_read(qlga_ctx*, qlga_profile* host_out);
 
+/* The polynomial the kernels use for the interaction exponential (host only, needs no GPU):
+ * exp(-i s K) v = P_p(y) v, y = -i s K, P_p(y) = b0 (1 + r[1] y (1 + r[2] y (... (1 + r[p] y)))),
+ * the Chebyshev-economised Taylor polynomial of degree p, valid for ||s K|| <= *theta_max within
+ * 2^tol_log2.  p = 1..12.  Exposed so that the table can be tested on the CPU. */
+qlga_status qlga_exp_polynomial(int tol_log2, int p, double* theta_max, double* b0, double* r);
+
 /* Number of kernels this context has launched so far (for bench.py's gpu_launches). */
 int64_t qlga_launch_count(const qlga_ctx*);
 

@@ -29,22 +29,83 @@ static qlga_status cuda_fail(qlga_ctx* c, const char* what, cudaError_t e) {
 
 static size_t real_size(qlga_prec p) { return p == QLGA_F64 ? sizeof(double) : sizeof(float); }
 
-// thresholds of the interaction polynomial: a degree-p Taylor polynomial of
-// exp(-i s K) has remainder <= theta^(p+1)/(p+1)!; thr[p-1] is the largest theta
-// for which that is below tol = 2^tol_log2.
+// ---------------------------------------------------------------------------
+// The interaction polynomial.  exp(-i s K) v is evaluated as P_p(-i s K) v with P_p a
+// degree-p polynomial with real coefficients b_j close to 1/j!.  A plain Taylor
+// polynomial wastes accuracy at small |x|; Chebyshev economisation (Lanczos) of the
+// degree-(p+4) Taylor polynomial on [-theta, theta] spreads the error evenly and buys
+// a factor ~2^p: the remainder is  sum_{n>p} |beta_n| 2^(1-n)  with beta_n the scaled
+// coefficient at the moment its degree is removed, ~ theta^(p+1) / ((p+1)! 2^p).
+// With y = -i x the even part of P_p is a polynomial for cos x and the odd part for
+// -i sin x, so the real polynomial A(x) = sum_j sigma_j b_j x^j, sigma_j = (-1)^(j/2),
+// (Taylor: cos x + sin x) is economised; T_n has the parity of n, so parities never mix.
+// ---------------------------------------------------------------------------
+static long double economise(int p, long double theta, long double* b /*[p+1]*/) {
+    const int N = p + 4;
+    long double beta[QLGA_PMAX + 8], fact = 1.0L, pw = 1.0L;
+    for (int n = 0; n <= N; ++n) {
+        if (n > 0) { fact *= (long double)n; pw *= theta; }
+        const long double sigma = ((n / 2) % 2 == 0) ? 1.0L : -1.0L;
+        beta[n] = sigma * pw / fact;                       // a_n theta^n
+    }
+    long double err = pw * theta / (fact * (long double)(N + 1));   // Taylor remainder of degree N
+    long double tc[QLGA_PMAX + 8][QLGA_PMAX + 8];          // T_n(t) = sum_k tc[n][k] t^k
+    for (int n = 0; n <= N; ++n) for (int k = 0; k <= N; ++k) tc[n][k] = 0.0L;
+    tc[0][0] = 1.0L; tc[1][1] = 1.0L;
+    for (int n = 2; n <= N; ++n)
+        for (int k = 0; k <= n; ++k)
+            tc[n][k] = (k > 0 ? 2.0L * tc[n - 1][k - 1] : 0.0L) - tc[n - 2][k];
+    for (int n = N; n > p; --n) {                          // remove degree n
+        const long double lam = beta[n] / tc[n][n];
+        for (int k = 0; k <= n; ++k) beta[k] -= lam * tc[n][k];
+        beta[n] = 0.0L;
+        err += fabsl(lam);
+    }
+    pw = 1.0L;
+    for (int j = 0; j <= p; ++j) {
+        if (j > 0) pw *= theta;
+        const long double sigma = ((j / 2) % 2 == 0) ? 1.0L : -1.0L;
+        b[j] = sigma * beta[j] / pw;
+    }
+    // the constant term is stored in double: a correction below half an ulp of 1 is lost
+    err += fabsl(b[0] - (long double)(double)b[0]);
+    return err;
+}
+
+// thr[p-1]: largest theta for which the economised degree-p polynomial stays within
+// tol = 2^tol_log2 (bisection on the monotone error bound); coefficients at that theta.
 static void build_exp_table(ExpTable& tab, int tol_log2) {
-    const double tol = ldexp(1.0, tol_log2);
-    tab.rcp[0] = 0.0;
-    for (int k = 1; k < QLGA_PMAX + 2; ++k) tab.rcp[k] = 1.0 / (double)k;
-    double fact = 1.0;                       // (p+1)!
+    const long double tol = ldexpl(1.0L, tol_log2);
     for (int p = 1; p <= QLGA_PMAX; ++p) {
-        fact = 1.0;
-        for (int k = 2; k <= p + 1; ++k) fact *= (double)k;
-        const double th = pow(tol * fact, 1.0 / (double)(p + 1));
-        tab.thr[p - 1] = (float)(th * 0.999);
+        long double b[QLGA_PMAX + 1];
+        long double lo = 0.0L, hi = 4.0L;
+        for (int it = 0; it < 200; ++it) {
+            const long double mid = 0.5L * (lo + hi);
+            if (economise(p, mid, b) <= tol) lo = mid; else hi = mid;
+        }
+        long double th = lo * 0.999L;                      // margin for the fp32 angle estimate
+        economise(p, th, b);
+        tab.thr[p - 1] = (float)th;
+        if ((long double)tab.thr[p - 1] > th) tab.thr[p - 1] = nextafterf(tab.thr[p - 1], 0.0f);
+        tab.b0[p - 1] = (double)b[0];
+        for (int k = 0; k <= QLGA_PMAX; ++k) tab.r[p - 1][k] = 0.0;
+        for (int k = 1; k <= p; ++k) tab.r[p - 1][k] = (double)(b[k] / b[k - 1]);
     }
     const double top = tab.thr[QLGA_PMAX - 1];
     tab.theta_split = (float)(top < 0.5 ? top : 0.5);
+}
+
+// Introspection of the polynomial table (host only, no GPU): used by the CPU tests.
+extern "C" qlga_status qlga_exp_polynomial(int tol_log2, int p, double* theta_max, double* b0,
+                                           double* r /* [p+1], r[0] unused */) {
+    if (p < 1 || p > QLGA_PMAX || tol_log2 > -8 || tol_log2 < -100 || !theta_max || !b0 || !r)
+        return QLGA_EINVAL;
+    static ExpTable tab;                                   // 1.3 KB: keep it off the stack
+    build_exp_table(tab, tol_log2);
+    *theta_max = tab.thr[p - 1];
+    *b0 = tab.b0[p - 1];
+    for (int k = 0; k <= p; ++k) r[k] = tab.r[p - 1][k];
+    return QLGA_OK;
 }
 
 extern "C" const char* qlga_version(void) { return "qlga-b200 0.1 (sm_100a)"; }

@@ -103,15 +103,19 @@ __device__ __forceinline__ void kin_update(Site<T>& s, int sigma, const cx<T> Fw
 //   g0 = s c0, g1 = s c1, g2 = s c2 / 5.
 // thr[p-1] = largest angle for which a degree-p polynomial meets the tolerance.
 // ---------------------------------------------------------------------------
-constexpr int QLGA_PMAX = 18;
+constexpr int QLGA_PMAX = 12;
 
 template <typename T> struct UConst {
     T g0, g1, g2;
 };
 
 struct ExpTable {
-    double rcp[QLGA_PMAX + 2];  // rcp[k] = 1/k
-    float thr[QLGA_PMAX];       // thresholds in float: order selection only
+    // Horner ratios of the degree-p polynomial P_p(y) = b0 (1 + r1 y (1 + r2 y (... (1 + rp y)))),
+    // y = -i s K: r[p-1][k] = b_k / b_{k-1} (close to 1/k), b0[p-1] close to 1.  P_p is the
+    // Chebyshev-economised Taylor polynomial of exp(y) on |y| <= thr[p-1].
+    double r[QLGA_PMAX][QLGA_PMAX + 1];
+    double b0[QLGA_PMAX];
+    float thr[QLGA_PMAX];       // thr[p-1] = largest angle degree p serves within the tolerance
     float theta_split;          // angles above this are split into equal sub-angles
 };
 
@@ -220,7 +224,8 @@ __device__ __forceinline__ void interaction(Site<T>& s, const UConst<T>& uc, con
             p = 1 + count_below(tab.thr, theta / (float)nsub * 1.0009765625f);
         }
     }
-    const cx<T> ph = mk<T>(cs, -sn);
+    const T pb0 = (T)tab.b0[p - 1];                // constant term of the polynomial (1 - O(tol))
+    const cx<T> ph = mk<T>(pb0 * cs, -(pb0 * sn));
 
     // Horner form u_{k-1} = v + (-i/k) (sK) u_k, k = p..1, u_p = v, for each of the two
     // spinor 5-vectors; psi (hence K) is frozen at its value before the application
@@ -234,7 +239,7 @@ __device__ __forceinline__ void interaction(Site<T>& s, const UConst<T>& uc, con
             for (int j = 0; j < 5; ++j) v[j] = s.q[j][sg];
             apply_sK<T>(v, w, az, a1, a6, g2, psi);
             {
-                const T ik = (T)tab.rcp[p];
+                const T ik = (T)tab.r[p - 1][p];
 #pragma unroll
                 for (int j = 0; j < 5; ++j) {
                     u[j].re = fma(ik, w[j].im, v[j].re); u[j].im = fma(-ik, w[j].re, v[j].im);
@@ -243,7 +248,7 @@ __device__ __forceinline__ void interaction(Site<T>& s, const UConst<T>& uc, con
 #pragma unroll 1
             for (int k = p - 1; k >= 1; --k) {
                 apply_sK<T>(u, w, az, a1, a6, g2, psi);
-                const T ik = (T)tab.rcp[k];
+                const T ik = (T)tab.r[p - 1][k];
 #pragma unroll
                 for (int j = 0; j < 5; ++j) {
                     u[j].re = fma(ik, w[j].im, v[j].re); u[j].im = fma(-ik, w[j].re, v[j].im);

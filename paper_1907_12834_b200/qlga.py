@@ -24,7 +24,7 @@ ABI_SYMBOLS = (
     "qlga_init", "qlga_state_bytes", "qlga_set_option", "qlga_set_state_psi", "qlga_set_state_q",
     "qlga_get_state_q", "qlga_get_state_psi", "qlga_step", "qlga_observables", "qlga_vorticity",
     "qlga_launch_count", "qlga_last_error", "qlga_destroy", "qlga_version",
-    "qlga_profile_enable", "qlga_profile_read",
+    "qlga_profile_enable", "qlga_profile_read", "qlga_exp_polynomial",
 )
 
 
@@ -77,6 +77,8 @@ def load_library():
     lib.qlga_profile_enable.restype = I
     lib.qlga_profile_read.argtypes = [P, ctypes.POINTER(QlgaProfile)]
     lib.qlga_profile_read.restype = I
+    lib.qlga_exp_polynomial.argtypes = [I, I, ctypes.POINTER(D), ctypes.POINTER(D), ctypes.POINTER(D)]
+    lib.qlga_exp_polynomial.restype = I
     lib.qlga_version.argtypes = []
     lib.qlga_version.restype = ctypes.c_char_p
     return lib
@@ -87,6 +89,16 @@ _lib = load_library()
 
 def version() -> str:
     return _lib.qlga_version().decode()
+
+
+def exp_polynomial(tol_log2, p):
+    """(theta_max, b0, r[0..p]) of the degree-p interaction polynomial (host only)."""
+    th, b0 = ctypes.c_double(), ctypes.c_double()
+    r = (ctypes.c_double * (p + 1))()
+    st = _lib.qlga_exp_polynomial(int(tol_log2), int(p), ctypes.byref(th), ctypes.byref(b0), r)
+    if st != QLGA_OK:
+        raise QlgaError(st, "qlga_exp_polynomial: bad arguments")
+    return th.value, b0.value, list(r)
 
 
 def state_bytes(ndim, dims, prec) -> int:

@@ -1,0 +1,58 @@
+"""The interaction polynomial table of the CUDA library (host-side, no GPU): the
+economised polynomial P_p(-ix) must reproduce exp(-ix) within the stated tolerance
+on the whole interval it is used for.  Checked in 50-digit arithmetic (mpmath)."""
+import math
+
+import mpmath as mp
+import pytest
+
+mp.mp.dps = 50
+
+
+def _poly(b0, r, p, y):
+    acc = mp.mpf(1)
+    for k in range(p, 0, -1):
+        acc = 1 + mp.mpf(r[k]) * y * acc
+    return mp.mpf(b0) * acc
+
+
+@pytest.mark.parametrize("tol_log2", [-56, -27])
+def test_polynomial_meets_tolerance_on_its_interval(tol_log2):
+    from paper_1907_12834_b200 import qlga
+    tol = mp.mpf(2) ** tol_log2
+    prev = 0.0
+    for p in range(1, 13):
+        theta, b0, r = qlga.exp_polynomial(tol_log2, p)
+        assert theta > prev                      # thresholds ascend
+        prev = theta
+        worst = mp.mpf(0)
+        for i in range(0, 201):
+            x = mp.mpf(theta) * (mp.mpf(i) / 100 - 1)
+            err = abs(_poly(b0, r, p, -1j * x) - mp.e ** (-1j * x))
+            worst = max(worst, err)
+        # (coefficients are doubles: allow their rounding, 2^-53 * theta, on top of the tolerance)
+        assert worst <= tol * mp.mpf("1.02") + mp.mpf(2) ** -52 * theta, (p, float(worst / tol))
+        # the economised polynomial reaches ~1.5-2x further than the Taylor polynomial of equal degree
+        taylor_theta = float((tol * mp.factorial(p + 1)) ** (mp.mpf(1) / (p + 1)))
+        assert theta > (1.25 if p >= 2 else 0.99) * taylor_theta
+        # coefficients stay close to 1/k and b0 to 1
+        assert abs(b0 - 1.0) <= 2.0 * float(tol) + 1e-18
+        for k in range(1, p + 1):
+            assert abs(r[k] * k - 1.0) < 0.3
+
+
+def test_polynomial_is_nearly_unitary():
+    # |P_p(-ix)| - 1 stays within the tolerance (the norm drift per application)
+    from paper_1907_12834_b200 import qlga
+    for p in (3, 5, 6, 8):
+        theta, b0, r = qlga.exp_polynomial(-56, p)
+        for i in range(0, 41):
+            x = mp.mpf(theta) * (mp.mpf(i) / 20 - 1)
+            assert abs(abs(_poly(b0, r, p, -1j * x)) - 1) <= mp.mpf(2) ** -56 * mp.mpf("1.02") + mp.mpf(2) ** -52 * theta
+
+
+def test_bad_arguments():
+    from paper_1907_12834_b200 import qlga
+    for args in ((-56, 0), (-56, 13), (-4, 3), (-200, 3)):
+        with pytest.raises(qlga.QlgaError):
+            qlga.exp_polynomial(*args)
