@@ -60,6 +60,7 @@ def parse_args():
     ap.add_argument("--tile-y", type=int, default=0)
     ap.add_argument("--threads-x", type=int, default=0)
     ap.add_argument("--threads-y", type=int, default=0)
+    ap.add_argument("--steps-per-launch", type=int, default=0, help="QLGA_OPT_STEPS_PER_LAUNCH (1D)")
     ap.add_argument("--tol-log2", type=int, default=0, help="QLGA_OPT_EXP_TOL_LOG2 override (experiments only)")
     return ap.parse_args()
 
@@ -296,6 +297,8 @@ def main():
         sim.set_option(qlga.OPT_THREADS_X, args.threads_x)
     if args.threads_y:
         sim.set_option(qlga.OPT_THREADS_Y, args.threads_y)
+    if args.steps_per_launch:
+        sim.set_option(qlga.OPT_STEPS_PER_LAUNCH, args.steps_per_launch)
     if args.tol_log2:
         sim.set_option(qlga.OPT_EXP_TOL_LOG2, args.tol_log2)
     omega_dev = (torch.empty((5, ny, nx), dtype=torch.float64 if args.precision == "f64" else torch.float32,

@@ -199,10 +199,10 @@ extern "C" qlga_status qlga_set_option(qlga_ctx* c, qlga_option key, int64_t v) 
             if (v > -8 || v < -100) return fail(c, QLGA_EINVAL, "QLGA_OPT_EXP_TOL_LOG2: -100..-8");
             c->tol_log2 = (int)v; build_exp_table(c->tab, c->tol_log2); return QLGA_OK;
         case QLGA_OPT_THREADS_X:
-            if (v != 0 && v != 128 && v != 192 && v != 256) return fail(c, QLGA_EINVAL, "QLGA_OPT_THREADS_X: 0, 128, 192, 256");
+            if (v != 0 && v != 64 && v != 96 && v != 128 && v != 192 && v != 256) return fail(c, QLGA_EINVAL, "QLGA_OPT_THREADS_X: 0, 64, 96, 128, 192, 256");
             c->threads_x = (int)v; return QLGA_OK;
         case QLGA_OPT_THREADS_Y:
-            if (v != 0 && v != 128 && v != 192 && v != 256) return fail(c, QLGA_EINVAL, "QLGA_OPT_THREADS_Y: 0, 128, 192, 256");
+            if (v != 0 && v != 64 && v != 96 && v != 128 && v != 192 && v != 256) return fail(c, QLGA_EINVAL, "QLGA_OPT_THREADS_Y: 0, 64, 96, 128, 192, 256");
             c->threads_y = (int)v; return QLGA_OK;
         case QLGA_OPT_TILE_Y:
             if (v != 0 && v != 1 && v != 2 && v != 4 && v != 8) return fail(c, QLGA_EINVAL, "QLGA_OPT_TILE_Y: 0,1,2,4,8");

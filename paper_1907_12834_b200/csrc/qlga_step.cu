@@ -41,7 +41,7 @@ __device__ __forceinline__ int64_t pmod(int64_t a, int64_t n) {
 #endif
 
 template <typename T, int DIR, int CX, int NT>
-__global__ void __launch_bounds__(NT, (NT >= 256 ? 2 : (NT >= 192 ? 2 : QLGA_MINB128))) pass_kernel(const __grid_constant__ PassArgs<T> P) {
+__global__ void __launch_bounds__(NT, (NT >= 192 ? 2 : (NT >= 128 ? QLGA_MINB128 : (NT >= 96 ? 4 : 6)))) pass_kernel(const __grid_constant__ PassArgs<T> P) {
     using V = typename vec2<T>::type;
     constexpr int TS = NT / CX;              // sites per line handled by the CTA
     constexpr int NW = NT / 32;
@@ -190,6 +190,8 @@ static cudaError_t launch_pass_t(const Launch& L, int dir, const PassParams& P, 
     if (dir == 0) {
         if (threads == 0) threads = 128;
         switch (threads) {
+            case 64: return run_pass<T, 0, 1, 64>(L, P);
+            case 96: return run_pass<T, 0, 1, 96>(L, P);
             case 128: return run_pass<T, 0, 1, 128>(L, P);
             case 192: return run_pass<T, 0, 1, 192>(L, P);
             case 256: return run_pass<T, 0, 1, 256>(L, P);
@@ -202,6 +204,8 @@ static cudaError_t launch_pass_t(const Launch& L, int dir, const PassParams& P, 
     if (cxw == 0) cxw = (sizeof(T) == 8) ? 1 : 4;
     if (threads == 0) threads = (cxw <= 2) ? 128 : 256;
     switch (cxw * 1000 + threads) {
+        case 1064: return run_pass<T, 1, 1, 64>(L, P);
+        case 1096: return run_pass<T, 1, 1, 96>(L, P);
         case 1128: return run_pass<T, 1, 1, 128>(L, P);
         case 1192: return run_pass<T, 1, 1, 192>(L, P);
         case 2128: return run_pass<T, 1, 2, 128>(L, P);
