@@ -236,6 +236,26 @@ def run_reference(args, w, ndim, config):
 
 
 # ---------------------------------------------------------------------------
+# multi-GPU plumbing: replicas only -- one lattice per rank, no
+# data-path collective; torch.distributed serves the barrier and the max over ranks
+# ---------------------------------------------------------------------------
+def max_over_ranks(ms, world, device=None):
+    """Largest per-rank duration (the job is as slow as its slowest replica)."""
+    if world <= 1:
+        return float(ms)
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([float(ms)], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def aggregate_gsups(sites_per_rank, time_steps, world, ms):
+    """Whole-job site-updates per second (GSUP/s): every rank advances its own lattice."""
+    return sites_per_rank * time_steps * world / (ms * 1e-3) / 1e9
+
+
+# ---------------------------------------------------------------------------
 # this repo's arm
 # ---------------------------------------------------------------------------
 def main():
@@ -333,11 +353,8 @@ def main():
     ms = ev0.elapsed_time(ev1)
     prof = sim.profile_read()
     sim.profile_enable(False)
-    if world > 1:
-        t = torch.tensor([ms], device=dev, dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms = float(t.item())
-    value = sites * inner * args.steps * world / (ms * 1e-3) / 1e9
+    ms = max_over_ranks(ms, world, dev)
+    value = aggregate_gsups(sites, inner * args.steps, world, ms)
 
     # ---- end to end through the C ABI with host buffers ---------------------------------
     e2e = None
@@ -359,11 +376,8 @@ def main():
         barrier()
         wall = time.perf_counter() - t0
         ems = max(e0.elapsed_time(e1), 0.0)
-        if world > 1:
-            t = torch.tensor([ems], device=dev, dtype=torch.float64)
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            ems = float(t.item())
-        e2e = {"value": sites * inner * args.e2e_steps * world / (ems * 1e-3) / 1e9, "unit": UNIT,
+        ems = max_over_ranks(ems, world, dev)
+        e2e = {"value": aggregate_gsups(sites, inner * args.e2e_steps, world, ems), "unit": UNIT,
                "h2d_bytes_per_step": state_bytes, "d2h_bytes_per_step": state_bytes + 168,
                "steps": args.e2e_steps, "ms_per_step": ems / args.e2e_steps,
                "wall_ms_per_step": wall * 1e3 / args.e2e_steps,
