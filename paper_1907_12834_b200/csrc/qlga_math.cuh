@@ -158,107 +158,141 @@ __device__ __forceinline__ void apply_sK(const cx<T> u[5], cx<T> w[5], T az, cx<
     w[4] = cfma_conj(psi[0], t, r4);
 }
 
-// Apply U^{(s)} to one site.  The site may carry a power-of-two scale 2^e; the
-// caller passes constants multiplied by 4^-e, which makes the result identical
-// (bit for bit, barring under/overflow) to applying U to the unscaled site.
-// number of thresholds thr[0..PMAX-2] (ascending) that theta exceeds, by bisection
+// number of thresholds thr[0..PMAX-2] (ascending) that theta exceeds: independent
+// compares summed as a tree (a bisection has fewer instructions but is a chain of
+// dependent constant-bank loads, and this sits on the critical path of every factor)
 __device__ __forceinline__ int count_below(const float* thr, float theta) {
-    int lo = 0, hi = QLGA_PMAX - 1;              // answer in [lo, hi]
+    int c[QLGA_PMAX - 1];
 #pragma unroll
-    for (int it = 0; it < 5; ++it) {
-        const int mid = (lo + hi) >> 1;
-        if (lo < hi) { if (theta > thr[mid]) lo = mid + 1; else hi = mid; }
-    }
-    return lo;
+    for (int k = 0; k < QLGA_PMAX - 1; ++k) c[k] = (theta > thr[k]) ? 1 : 0;
+#pragma unroll
+    for (int w = 1; w < QLGA_PMAX - 1; w *= 2)
+#pragma unroll
+        for (int k = 0; k + w < QLGA_PMAX - 1; k += 2 * w) c[k] += c[k + w];
+    return c[0];
 }
 
-template <typename T>
-__device__ __forceinline__ void interaction(Site<T>& s, const UConst<T>& uc, const ExpTable& tab) {
+// Site-local coefficients of sK = g1 F.f + g2 |chi><chi| (pre-scaled, see apply_sK).
+template <typename T> struct KCoef {
+    T az, g2;
+    cx<T> a1, a6;
     cx<T> psi[5];
+    T rho;
+    float theta;                                   // 2|g1||F| + |g2| rho, this lane
+};
+
+template <typename T>
+__device__ __forceinline__ void site_coefficients(const Site<T>& s, const UConst<T>& uc, KCoef<T>& kc) {
     T n[5];
 #pragma unroll
     for (int j = 0; j < 5; ++j) {
-        psi[j] = s.q[j][0] + s.q[j][1];
-        n[j] = fma(psi[j].re, psi[j].re, psi[j].im * psi[j].im);
+        kc.psi[j] = s.q[j][0] + s.q[j][1];
+        n[j] = fma(kc.psi[j].re, kc.psi[j].re, kc.psi[j].im * kc.psi[j].im);
     }
-    const T rho = (n[0] + n[4]) + (n[1] + n[3]) + n[2];
+    kc.rho = (n[0] + n[4]) + (n[1] + n[3]) + n[2];
     const T Fz = (T)2 * (n[0] - n[4]) + (n[1] - n[3]);
     // F_+ = sum_m alpha_m conj(psi_{m+1}) psi_m = 2(conj(psi_2) psi_1 + conj(psi_-1) psi_-2)
     //                                           + sqrt6 (conj(psi_1) psi_0 + conj(psi_0) psi_-1)
-    cx<T> fa = cfma_conj(psi[0], psi[1], mk<T>((T)0, (T)0));
-    fa = cfma_conj(psi[3], psi[4], fa);
-    cx<T> fb = cfma_conj(psi[1], psi[2], mk<T>((T)0, (T)0));
-    fb = cfma_conj(psi[2], psi[3], fb);
+    cx<T> fa = cfma_conj(kc.psi[0], kc.psi[1], mk<T>((T)0, (T)0));
+    fa = cfma_conj(kc.psi[3], kc.psi[4], fa);
+    cx<T> fb = cfma_conj(kc.psi[1], kc.psi[2], mk<T>((T)0, (T)0));
+    fb = cfma_conj(kc.psi[2], kc.psi[3], fb);
     const T rt6 = (T)2.4494897427831780981972840747059;
     const cx<T> Fp = mk<T>(fma(rt6, fb.re, (T)2 * fa.re), fma(rt6, fb.im, (T)2 * fa.im));
-
-    // angle bound theta = 2 |g1| |F| + |g2| rho  (spectral norms of the two parts),
-    // made warp-uniform (one degree per warp keeps the Horner loops convergent)
-    const float Fabs = sqrtf((float)(Fz * Fz + Fp.re * Fp.re + Fp.im * Fp.im));
-    float theta = 2.0f * fabsf((float)uc.g1) * Fabs + fabsf((float)uc.g2) * (float)rho;
-    theta *= 1.0009765625f;                       // cover the float rounding of the estimate
-    theta = __uint_as_float(__reduce_max_sync(0xffffffffu, __float_as_uint(theta)));
-
-    // Fast path, branch free (one basic block, so the independent chains below
-    // interleave): one application, small scalar phase.
-    const T xph = uc.g0 * rho;                    // scalar phase exp(-i s c0 rho)
-    T sn, cs;
-    sincos_small<T>(xph, &sn, &cs);
-    T g2 = uc.g2;
-    T az = uc.g1 * Fz;
-    cx<T> a1 = mk<T>(uc.g1 * Fp.re, uc.g1 * Fp.im);
+    // angle bound theta = 2 |g1| |F| + |g2| rho (the exact spectral norms of the two parts);
+    // |F| by the approximate reciprocal square root (2 ulp; the 2^-10 margin covers it)
+    const float f2 = fmaxf((float)(Fz * Fz + Fp.re * Fp.re + Fp.im * Fp.im), 1e-37f);
+    const float Fabs = f2 * __frsqrt_rn(f2);
+    kc.theta = (2.0f * fabsf((float)uc.g1) * Fabs + fabsf((float)uc.g2) * (float)kc.rho) * 1.0009765625f;
+    kc.g2 = uc.g2;
+    kc.az = uc.g1 * Fz;
+    kc.a1 = mk<T>(uc.g1 * Fp.re, uc.g1 * Fp.im);
     const T rt6h = (T)1.2247448713915890490986420373529;          // sqrt(6)/2
-    cx<T> a6 = mk<T>(rt6h * a1.re, rt6h * a1.im);
-    int p = 1 + count_below(tab.thr, theta);
-    int nsub = 1;
-    // Rare path (never at the paper's amplitudes): large scalar phase -> library sincos;
-    // angle above theta_split -> nsub equal sub-angles (exact: K is frozen).
-    const bool big_phase = !__all_sync(0xffffffffu, fabs(xph) <= (T)0.0625);
-    if (big_phase || theta > tab.theta_split) {
-        if (big_phase) sincos_lib(xph, &sn, &cs);
-        if (theta > tab.theta_split) {
-            nsub = (int)ceilf(theta / tab.theta_split);
-            const T inv_nsub = (T)1 / (T)nsub;
-            g2 *= inv_nsub; az *= inv_nsub;
-            a1.re *= inv_nsub; a1.im *= inv_nsub; a6.re *= inv_nsub; a6.im *= inv_nsub;
-            p = 1 + count_below(tab.thr, theta / (float)nsub * 1.0009765625f);
+    kc.a6 = mk<T>(rt6h * kc.a1.re, rt6h * kc.a1.im);
+}
+
+// u <- P_p(-i sK) v in Horner form u_{k-1} = v + r_k (-i sK) u_k, k = p..1, u_p = v
+// (stage p acts on v itself: no copy).  psi, hence K, is frozen (reading R4).
+template <typename T>
+__device__ __forceinline__ void horner(const cx<T> v[5], cx<T> u[5], const KCoef<T>& kc,
+                                       const double* __restrict__ r, int p) {
+    cx<T> w[5];
+    apply_sK<T>(v, w, kc.az, kc.a1, kc.a6, kc.g2, kc.psi);
+    {
+        const T ik = (T)r[p];
+#pragma unroll
+        for (int j = 0; j < 5; ++j) {
+            u[j].re = fma(ik, w[j].im, v[j].re); u[j].im = fma(-ik, w[j].re, v[j].im);
         }
     }
+#pragma unroll 1
+    for (int k = p - 1; k >= 1; --k) {
+        apply_sK<T>(u, w, kc.az, kc.a1, kc.a6, kc.g2, kc.psi);
+        const T ik = (T)r[k];
+#pragma unroll
+        for (int j = 0; j < 5; ++j) {
+            u[j].re = fma(ik, w[j].im, v[j].re); u[j].im = fma(-ik, w[j].re, v[j].im);
+        }
+    }
+}
+
+// General path (never taken at the paper's amplitudes): scalar phase by the library
+// sincos; angles above theta_split in nsub equal sub-angles (exact: K is frozen).
+// Out of line and by value so that the common path keeps its registers.
+template <typename T>
+__device__ __noinline__ Site<T> interaction_general(Site<T> s, UConst<T> uc, const ExpTable& tab, float theta) {
+    KCoef<T> kc;
+    site_coefficients<T>(s, uc, kc);
+    int nsub = 1;
+    if (theta > tab.theta_split) nsub = (int)ceilf(theta / tab.theta_split);
+    const T inv_nsub = (T)1 / (T)nsub;
+    kc.g2 *= inv_nsub; kc.az *= inv_nsub;
+    kc.a1.re *= inv_nsub; kc.a1.im *= inv_nsub; kc.a6.re *= inv_nsub; kc.a6.im *= inv_nsub;
+    const int p = 1 + count_below(tab.thr, theta / (float)nsub * 1.0009765625f);
+    T sn, cs;
+    sincos_lib(uc.g0 * kc.rho, &sn, &cs);
+    T b0n = (T)1;
+    for (int rep = 0; rep < nsub; ++rep) b0n *= (T)tab.b0[p - 1];
+    const cx<T> ph = mk<T>(b0n * cs, -(b0n * sn));
+    for (int sg = 0; sg < 2; ++sg) {
+        cx<T> v[5], u[5];
+        for (int j = 0; j < 5; ++j) v[j] = s.q[j][sg];
+        for (int rep = 0; rep < nsub; ++rep) {
+            horner<T>(v, u, kc, tab.r[p - 1], p);
+            for (int j = 0; j < 5; ++j) v[j] = u[j];
+        }
+        for (int j = 0; j < 5; ++j) s.q[j][sg] = cmul(ph, v[j]);
+    }
+    return s;
+}
+
+// Apply U^{(s)} to one site.  The site may carry a power-of-two scale 2^e; the
+// caller passes constants multiplied by 4^-e, which makes the result identical
+// (bit for bit, barring under/overflow) to applying U to the unscaled site.
+template <typename T>
+__device__ __forceinline__ void interaction(Site<T>& s, const UConst<T>& uc, const ExpTable& tab) {
+    KCoef<T> kc;
+    site_coefficients<T>(s, uc, kc);
+    // warp-uniform angle (one polynomial degree per warp keeps the Horner loops convergent)
+    const float theta = __uint_as_float(__reduce_max_sync(0xffffffffu, __float_as_uint(kc.theta)));
+    const T xph = uc.g0 * kc.rho;                  // scalar phase exp(-i s c0 rho)
+    const bool big_phase = !__all_sync(0xffffffffu, fabs(xph) <= (T)0.0625);
+    if (big_phase || theta > tab.theta_split) {
+        s = interaction_general<T>(s, uc, tab, theta);
+        return;
+    }
+    T sn, cs;
+    sincos_small<T>(xph, &sn, &cs);
+    const int p = 1 + count_below(tab.thr, theta);
     const T pb0 = (T)tab.b0[p - 1];                // constant term of the polynomial (1 - O(tol))
     const cx<T> ph = mk<T>(pb0 * cs, -(pb0 * sn));
-
-    // Horner form u_{k-1} = v + (-i/k) (sK) u_k, k = p..1, u_p = v, for each of the two
-    // spinor 5-vectors; psi (hence K) is frozen at its value before the application
-    // (reading R4).  Stage p acts on v itself (no copy of the site state).
+    const double* r = tab.r[p - 1];
 #pragma unroll
     for (int sg = 0; sg < 2; ++sg) {
-        cx<T> u[5], w[5];
-        for (int rep = 0; rep < nsub; ++rep) {
-            cx<T> v[5];
+        cx<T> v[5], u[5];
 #pragma unroll
-            for (int j = 0; j < 5; ++j) v[j] = s.q[j][sg];
-            apply_sK<T>(v, w, az, a1, a6, g2, psi);
-            {
-                const T ik = (T)tab.r[p - 1][p];
-#pragma unroll
-                for (int j = 0; j < 5; ++j) {
-                    u[j].re = fma(ik, w[j].im, v[j].re); u[j].im = fma(-ik, w[j].re, v[j].im);
-                }
-            }
-#pragma unroll 1
-            for (int k = p - 1; k >= 1; --k) {
-                apply_sK<T>(u, w, az, a1, a6, g2, psi);
-                const T ik = (T)tab.r[p - 1][k];
-#pragma unroll
-                for (int j = 0; j < 5; ++j) {
-                    u[j].re = fma(ik, w[j].im, v[j].re); u[j].im = fma(-ik, w[j].re, v[j].im);
-                }
-            }
-            if (rep + 1 < nsub) {               // rare: next sub-angle starts from u
-#pragma unroll
-                for (int j = 0; j < 5; ++j) s.q[j][sg] = u[j];
-            }
-        }
+        for (int j = 0; j < 5; ++j) v[j] = s.q[j][sg];
+        horner<T>(v, u, kc, r, p);
 #pragma unroll
         for (int j = 0; j < 5; ++j) s.q[j][sg] = cmul(ph, u[j]);
     }

@@ -35,6 +35,44 @@ __device__ __forceinline__ int64_t pmod(int64_t a, int64_t n) {
     return r < 0 ? r + n : r;
 }
 
+// One kinetic factor I'_{d,SIGMA} of the pass, preceded by the interaction if the
+// ordering asks for it.  SIGMA (compile time) = the spinor component that streams.
+template <typename T, int CX, int NW, int SIGMA>
+__device__ __forceinline__ void factor(Site<T>& s, const PassArgs<T>& P, int f, int lane, int warp, int& pb,
+                                       cx<T> (*edgeF)[NW][CX][5], cx<T> (*edgeB)[NW][CX][5]) {
+    constexpr int EDGE = 32 - CX;
+    if (P.umode == 2 || (P.umode == 1 && f == 0)) interaction<T>(s, P.uc[f], P.tab);
+
+    cx<T> Fw[5], Bw[5], Fp[5], Bn[5];
+    kin_messages<T>(s, SIGMA, Fw, Bw);
+    if (lane >= EDGE) {
+#pragma unroll
+        for (int j = 0; j < 5; ++j) edgeF[pb][warp][lane - EDGE][j] = Fw[j];
+    }
+    if (lane < CX) {
+#pragma unroll
+        for (int j = 0; j < 5; ++j) edgeB[pb][warp][lane][j] = Bw[j];
+    }
+#pragma unroll
+    for (int j = 0; j < 5; ++j) {
+        Fp[j].re = __shfl_up_sync(0xffffffffu, Fw[j].re, CX);
+        Fp[j].im = __shfl_up_sync(0xffffffffu, Fw[j].im, CX);
+        Bn[j].re = __shfl_down_sync(0xffffffffu, Bw[j].re, CX);
+        Bn[j].im = __shfl_down_sync(0xffffffffu, Bw[j].im, CX);
+    }
+    __syncthreads();
+    if (lane < CX && warp > 0) {
+#pragma unroll
+        for (int j = 0; j < 5; ++j) Fp[j] = edgeF[pb][warp - 1][lane][j];
+    }
+    if (lane >= EDGE && warp < NW - 1) {
+#pragma unroll
+        for (int j = 0; j < 5; ++j) Bn[j] = edgeB[pb][warp + 1][lane - EDGE][j];
+    }
+    pb ^= 1;
+    kin_update<T>(s, SIGMA, Fw, Bw, Fp, Bn);
+}
+
 // experiment knobs (compile time)
 #ifndef QLGA_MINB128
 #define QLGA_MINB128 3
@@ -45,7 +83,6 @@ __global__ void __launch_bounds__(NT, (NT >= 192 ? 2 : (NT >= 128 ? QLGA_MINB128
     using V = typename vec2<T>::type;
     constexpr int TS = NT / CX;              // sites per line handled by the CTA
     constexpr int NW = NT / 32;
-    constexpr int EDGE = 32 - CX;
     static_assert(NT % 32 == 0 && 32 % CX == 0 && CX < 32, "bad tile");
     static_assert(DIR == 1 || CX == 1, "x pass uses one line per CTA");
 
@@ -81,75 +118,43 @@ __global__ void __launch_bounds__(NT, (NT >= 192 ? 2 : (NT >= 128 ? QLGA_MINB128
     }
     const int64_t idx = y * P.nx + x;
 
-    // slot 0 = the component that streams in the current factor, slot 1 = the other.
-    // The pass starts with component 2 (plane sigma = 1) streaming.
+    // s.q[j][sigma]: sigma = 0,1 <-> spinor component 1,2 (the planes' own order)
     Site<T> s;
 #pragma unroll
     for (int j = 0; j < 5; ++j) {
-        V a = P.src[(int64_t)(2 * j + 1) * n + idx];
-        V b = P.src[(int64_t)(2 * j + 0) * n + idx];
+        V a = P.src[(int64_t)(2 * j + 0) * n + idx];
+        V b = P.src[(int64_t)(2 * j + 1) * n + idx];
         s.q[j][0] = mk<T>(a.x, a.y);
         s.q[j][1] = mk<T>(b.x, b.y);
     }
 
-    const int nsub = 4 * P.ksteps;
     int pb = 0;
 #pragma unroll 1
-    for (int sub = 0; sub < nsub; ++sub) {
-        const int f = sub & 3;
-        if (P.umode == 2 || (P.umode == 1 && f == 0)) interaction<T>(s, P.uc[f], P.tab);
-
-        cx<T> Fw[5], Bw[5], Fp[5], Bn[5];
-        kin_messages<T>(s, 0, Fw, Bw);
-        if (lane >= EDGE) {
-#pragma unroll
-            for (int j = 0; j < 5; ++j) edgeF[pb][warp][lane - EDGE][j] = Fw[j];
-        }
-        if (lane < CX) {
-#pragma unroll
-            for (int j = 0; j < 5; ++j) edgeB[pb][warp][lane][j] = Bw[j];
-        }
+    for (int st = 0; st < P.ksteps; ++st) {
+        // factors I'_{d,2} I'_{d,2} then I'_{d,1} I'_{d,1} (rightmost first): two code instances,
+        // one per streamed component, so that no register ever changes role
+#pragma unroll 1
+        for (int f = 0; f < 2; ++f)
+            factor<T, CX, NW, 1>(s, P, f, lane, warp, pb, edgeF, edgeB);
+#pragma unroll 1
+        for (int f = 2; f < 4; ++f)
+            factor<T, CX, NW, 0>(s, P, f, lane, warp, pb, edgeF, edgeB);
+        // undo the four deferred halvings (exact)
 #pragma unroll
         for (int j = 0; j < 5; ++j) {
-            Fp[j].re = __shfl_up_sync(0xffffffffu, Fw[j].re, CX);
-            Fp[j].im = __shfl_up_sync(0xffffffffu, Fw[j].im, CX);
-            Bn[j].re = __shfl_down_sync(0xffffffffu, Bw[j].re, CX);
-            Bn[j].im = __shfl_down_sync(0xffffffffu, Bw[j].im, CX);
-        }
-        __syncthreads();
-        if (lane < CX && warp > 0) {
-#pragma unroll
-            for (int j = 0; j < 5; ++j) Fp[j] = edgeF[pb][warp - 1][lane][j];
-        }
-        if (lane >= EDGE && warp < NW - 1) {
-#pragma unroll
-            for (int j = 0; j < 5; ++j) Bn[j] = edgeB[pb][warp + 1][lane - EDGE][j];
-        }
-        pb ^= 1;
-        kin_update<T>(s, 0, Fw, Bw, Fp, Bn);
-
-        if (sub & 1) {                       // factors come in pairs: 2,2,1,1 -> swap roles
-#pragma unroll
-            for (int j = 0; j < 5; ++j) { cx<T> tmp = s.q[j][0]; s.q[j][0] = s.q[j][1]; s.q[j][1] = tmp; }
-        }
-        if (f == 3) {                        // undo the four deferred halvings (exact)
-#pragma unroll
-            for (int j = 0; j < 5; ++j) {
-                s.q[j][0].re *= P.out_scale; s.q[j][0].im *= P.out_scale;
-                s.q[j][1].re *= P.out_scale; s.q[j][1].im *= P.out_scale;
-            }
+            s.q[j][0].re *= P.out_scale; s.q[j][0].im *= P.out_scale;
+            s.q[j][1].re *= P.out_scale; s.q[j][1].im *= P.out_scale;
         }
     }
 
-    // after a whole number of steps slot 0 is component 2 again
     if (i >= H && i < TS - H && spos < extent && col_ok) {
 #pragma unroll
         for (int j = 0; j < 5; ++j) {
             V a, b;
             a.x = s.q[j][0].re; a.y = s.q[j][0].im;
             b.x = s.q[j][1].re; b.y = s.q[j][1].im;
-            P.dst[(int64_t)(2 * j + 1) * n + idx] = a;
-            P.dst[(int64_t)(2 * j + 0) * n + idx] = b;
+            P.dst[(int64_t)(2 * j + 0) * n + idx] = a;
+            P.dst[(int64_t)(2 * j + 1) * n + idx] = b;
         }
     }
 }
