@@ -37,37 +37,36 @@ __device__ __forceinline__ int64_t pmod(int64_t a, int64_t n) {
 
 // One kinetic factor I'_{d,SIGMA} of the pass, preceded by the interaction if the
 // ordering asks for it.  SIGMA (compile time) = the spinor component that streams.
-template <typename T, int CX, int NW, int SIGMA>
-__device__ __forceinline__ void factor(Site<T>& s, const PassArgs<T>& P, int f, int lane, int warp, int& pb,
-                                       cx<T> (*edgeF)[NW][CX][5], cx<T> (*edgeB)[NW][CX][5]) {
-    constexpr int EDGE = 32 - CX;
+// The two message 5-vectors of a site go to its neighbours along the line through
+// shared memory, one 16-byte (8-byte in fp32) element per thread and plane
+// ([j][thread]: conflict free), double buffered so that one barrier per factor
+// suffices.  (A warp-shuffle exchange was measured first: SHFL.32 issues at 6 cycles
+// per warp on sm_100a and a factor needs 40 of them.)
+template <typename T, int CX, int NT, int SIGMA>
+__device__ __forceinline__ void factor(Site<T>& s, const PassArgs<T>& P, int f, int t, int& pb,
+                                       typename vec2<T>::type (*sF)[5][NT], typename vec2<T>::type (*sB)[5][NT]) {
+    using V = typename vec2<T>::type;
     if (P.umode == 2 || (P.umode == 1 && f == 0)) interaction<T>(s, P.uc[f], P.tab);
 
     cx<T> Fw[5], Bw[5], Fp[5], Bn[5];
     kin_messages<T>(s, SIGMA, Fw, Bw);
-    if (lane >= EDGE) {
-#pragma unroll
-        for (int j = 0; j < 5; ++j) edgeF[pb][warp][lane - EDGE][j] = Fw[j];
-    }
-    if (lane < CX) {
-#pragma unroll
-        for (int j = 0; j < 5; ++j) edgeB[pb][warp][lane][j] = Bw[j];
-    }
 #pragma unroll
     for (int j = 0; j < 5; ++j) {
-        Fp[j].re = __shfl_up_sync(0xffffffffu, Fw[j].re, CX);
-        Fp[j].im = __shfl_up_sync(0xffffffffu, Fw[j].im, CX);
-        Bn[j].re = __shfl_down_sync(0xffffffffu, Bw[j].re, CX);
-        Bn[j].im = __shfl_down_sync(0xffffffffu, Bw[j].im, CX);
+        V a, b;
+        a.x = Fw[j].re; a.y = Fw[j].im; b.x = Bw[j].re; b.y = Bw[j].im;
+        sF[pb][j][t] = a;
+        sB[pb][j][t] = b;
     }
     __syncthreads();
-    if (lane < CX && warp > 0) {
+    // the first / last CX threads of the CTA have no neighbour in the tile: they are halo
+    // threads whose values are never stored; they read their own slot
+    const int tm = (t >= CX) ? t - CX : t;
+    const int tp = (t + CX < NT) ? t + CX : t;
 #pragma unroll
-        for (int j = 0; j < 5; ++j) Fp[j] = edgeF[pb][warp - 1][lane][j];
-    }
-    if (lane >= EDGE && warp < NW - 1) {
-#pragma unroll
-        for (int j = 0; j < 5; ++j) Bn[j] = edgeB[pb][warp + 1][lane - EDGE][j];
+    for (int j = 0; j < 5; ++j) {
+        const V a = sF[pb][j][tm], b = sB[pb][j][tp];
+        Fp[j] = mk<T>(a.x, a.y);
+        Bn[j] = mk<T>(b.x, b.y);
     }
     pb ^= 1;
     kin_update<T>(s, SIGMA, Fw, Bw, Fp, Bn);
@@ -82,15 +81,14 @@ template <typename T, int DIR, int CX, int NT>
 __global__ void __launch_bounds__(NT, (NT >= 192 ? 2 : (NT >= 128 ? QLGA_MINB128 : (NT >= 96 ? 4 : 6)))) pass_kernel(const __grid_constant__ PassArgs<T> P) {
     using V = typename vec2<T>::type;
     constexpr int TS = NT / CX;              // sites per line handled by the CTA
-    constexpr int NW = NT / 32;
     static_assert(NT % 32 == 0 && 32 % CX == 0 && CX < 32, "bad tile");
     static_assert(DIR == 1 || CX == 1, "x pass uses one line per CTA");
 
-    __shared__ cx<T> edgeF[2][NW][CX][5];
-    __shared__ cx<T> edgeB[2][NW][CX][5];
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    V (*sF)[5][NT] = reinterpret_cast<V (*)[5][NT]>(smem_raw);
+    V (*sB)[5][NT] = sF + 2;
 
     const int t = threadIdx.x;
-    const int lane = t & 31, warp = t >> 5;
     const int c = t % CX, i = t / CX;
     const int H = 4 * P.ksteps;
     const int wout = TS - 2 * H;
@@ -135,10 +133,10 @@ __global__ void __launch_bounds__(NT, (NT >= 192 ? 2 : (NT >= 128 ? QLGA_MINB128
         // one per streamed component, so that no register ever changes role
 #pragma unroll 1
         for (int f = 0; f < 2; ++f)
-            factor<T, CX, NW, 1>(s, P, f, lane, warp, pb, edgeF, edgeB);
+            factor<T, CX, NT, 1>(s, P, f, t, pb, sF, sB);
 #pragma unroll 1
         for (int f = 2; f < 4; ++f)
-            factor<T, CX, NW, 0>(s, P, f, lane, warp, pb, edgeF, edgeB);
+            factor<T, CX, NT, 0>(s, P, f, t, pb, sF, sB);
         // undo the four deferred halvings (exact)
 #pragma unroll
         for (int j = 0; j < 5; ++j) {
@@ -183,7 +181,15 @@ static cudaError_t run_pass(const Launch& L, const PassParams& P) {
     else blocks = ((P.nx + CX - 1) / CX) * ((P.ny + wout - 1) / wout);
     if (blocks <= 0 || blocks > 2147483647LL) return cudaErrorInvalidValue;
     PassArgs<T> A = make_args<T>(P);
-    pass_kernel<T, DIR, CX, NT><<<(unsigned)blocks, NT, 0, L.stream>>>(A);
+    constexpr size_t smem = (size_t)4 * 5 * NT * sizeof(typename vec2<T>::type);   // sF[2], sB[2]
+    static bool configured = false;            // per instantiation; more than 48 KB needs the opt-in
+    if (!configured) {
+        cudaError_t e = cudaFuncSetAttribute(pass_kernel<T, DIR, CX, NT>,
+                                             cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return e;
+        configured = true;
+    }
+    pass_kernel<T, DIR, CX, NT><<<(unsigned)blocks, NT, smem, L.stream>>>(A);
     ++*L.counter;
     return cudaGetLastError();
 }
