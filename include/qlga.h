@@ -129,6 +129,23 @@ qlga_status qlga_observables(qlga_ctx*, qlga_obs* host_out);
  * omega: HOST or DEVICE [5][Ny][Nx] real of the context's real type.  QLGA_EUNSUP in 1D. */
 qlga_status qlga_vorticity(qlga_ctx*, void* omega, int dst_on_device);
 
+/* Total density rho(r) = sum_m |psi_m(r)|^2 = psi psi^dagger; rho: HOST or DEVICE [Ny][Nx] real. */
+qlga_status qlga_density(qlga_ctx*, void* rho, int dst_on_device);
+
+/* L2 error of eq. (115), PAPER.md:1074 (the paper's convergence measure, Figs. 23-24):
+ *   *host_eps = sum_r (rho_ref(r) - rho(r))^2,  rho_ref: HOST or DEVICE [Ny][Nx] real of the
+ * context's real type (e.g. the density of the initial eigenstate).  Synchronises the stream. */
+qlga_status qlga_density_l2_error(qlga_ctx*, const void* rho_ref, int src_on_device, double* host_eps);
+
+/* Vortex detection, 2D only (the paper tracks vortices of positive / negative winding number,
+ * Figs. 18, 21, 22; detector = reading R15 of DESIGN.md): winding number of
+ * every elementary plaquette, corners counter-clockwise a=(x,y), b=(x+1,y), c=(x+1,y+1), d=(x,y+1),
+ *   w = [arg(b a*) + arg(c b*) + arg(d c*) + arg(a d*)] / (2 pi)  in {-1, 0, +1}   (arg(0) := 0),
+ * per m.  Writes up to max_out records (j, x, y, w) of the plaquettes with w != 0 to
+ * host_out (HOST, int32 [max_out][4], order unspecified) and the total number found to
+ * *host_count (may exceed max_out).  Synchronises the stream.  QLGA_EUNSUP in 1D. */
+qlga_status qlga_vortices(qlga_ctx*, int32_t* host_out, int64_t max_out, int64_t* host_count);
+
 /* Kernel timing hooks (used by bench.py for the roofline of the dominant kernel).
  * While enabled, qlga_step records a CUDA event on the caller's stream before every
  * pass kernel and one after the last; qlga_profile_read synchronises the stream,

@@ -413,3 +413,61 @@ void orc_vorticity(const cplx *q, long nx, long ny, real *omega)
     }
     free(psi); free(vx); free(vy);
 }
+
+/* ------------------------------------------------------------------------
+ * Total density and the L2 error of eq. (115), PAPER.md:1074:
+ *   rho(r) = sum_m |psi_m(r)|^2 = psi psi^dagger,
+ *   epsilon = sum_lattice ( rho_ref(r) - rho(r) )^2 .
+ * (the convergence study of Figs. 23-24.)
+ * ---------------------------------------------------------------------- */
+void orc_density(const cplx *q, long nx, long ny, real *rho)
+{
+    long n = nx * ny;
+    for (long r = 0; r < n; ++r) {
+        real s = 0;
+        for (int j = 0; j < NM; ++j) {
+            cplx p = q[((size_t)j * NS + 0) * n + r] + q[((size_t)j * NS + 1) * n + r];
+            s += creal(p) * creal(p) + cimag(p) * cimag(p);
+        }
+        rho[r] = s;
+    }
+}
+
+double orc_density_l2_error(const cplx *q, const real *rho_ref, long nx, long ny)
+{
+    long n = nx * ny;
+    real *rho = (real *)malloc(sizeof(real) * (size_t)n);
+    orc_density(q, nx, ny, rho);
+    real e = 0;
+    for (long r = 0; r < n; ++r) { real d = rho_ref[r] - rho[r]; e += d * d; }
+    free(rho);
+    return (double)e;
+}
+
+/* ------------------------------------------------------------------------
+ * Plaquette winding numbers (vortex detection; the
+ * paper tracks "vortices with a positive / negative winding number", Figs. 18, 21,
+ * 22, without printing the detector)  [R15]:
+ * for the elementary plaquette with lower-left corner (x, y), corners taken
+ * counter-clockwise  a=(x,y), b=(x+1,y), c=(x+1,y+1), d=(x,y+1),
+ *   w(x,y) = [ arg(b a*) + arg(c b*) + arg(d c*) + arg(a d*) ] / (2 pi)  in {-1, 0, +1},
+ * every phase difference wrapped to (-pi, pi] by taking arg of the product and
+ * arg(0) := 0, rounded to the nearest integer.  wind: [5][ny][nx] int32.
+ * ---------------------------------------------------------------------- */
+void orc_winding(const cplx *q, long nx, long ny, int *wind)
+{
+    long n = nx * ny;
+    const real twopi = (real)6.283185307179586476925286766559005768L;
+    for (int j = 0; j < NM; ++j)
+        for (long y = 0; y < ny; ++y)
+            for (long x = 0; x < nx; ++x) {
+                long xp = wrapl(x + 1, nx), yp = wrapl(y + 1, ny);
+                long ia = y * nx + x, ib = y * nx + xp, ic = yp * nx + xp, id = yp * nx + x;
+                cplx a = q[((size_t)j * NS + 0) * n + ia] + q[((size_t)j * NS + 1) * n + ia];
+                cplx b = q[((size_t)j * NS + 0) * n + ib] + q[((size_t)j * NS + 1) * n + ib];
+                cplx c = q[((size_t)j * NS + 0) * n + ic] + q[((size_t)j * NS + 1) * n + ic];
+                cplx d = q[((size_t)j * NS + 0) * n + id] + q[((size_t)j * NS + 1) * n + id];
+                real circ = arg0(b * conj(a)) + arg0(c * conj(b)) + arg0(d * conj(c)) + arg0(a * conj(d));
+                wind[(size_t)j * n + ia] = (int)lrint((double)(circ / twopi));
+            }
+}

@@ -60,11 +60,16 @@ class Oracle:
             "orc_step": [P, L, L, I, R, R, R, I, L],
             "orc_observables": [P, P, L, L, I, R, R, R, P],
             "orc_vorticity": [P, L, L, P],
+            "orc_density": [P, L, L, P],
+            "orc_winding": [P, L, L, P],
         }
         for name, args in sig.items():
             fn = getattr(self.lib, name)
             fn.argtypes = args
             fn.restype = None
+
+        self.lib.orc_density_l2_error.argtypes = [P, P, L, L]
+        self.lib.orc_density_l2_error.restype = ctypes.c_double
 
     # -- helpers ---------------------------------------------------------
     def _c(self, a, shape=None):
@@ -164,3 +169,27 @@ class Oracle:
         om = np.empty((5, ny, nx), dtype=self.rtype)
         self.lib.orc_vorticity(self._p(q), nx, ny, self._p(om))
         return om
+
+    def density(self, q):
+        """rho(r) = sum_m |psi_m|^2, shape (Ny, Nx)."""
+        q = self._c(q)
+        nx, ny = self._dims(q)
+        rho = np.empty((ny, nx), dtype=self.rtype)
+        self.lib.orc_density(self._p(q), nx, ny, self._p(rho))
+        return rho
+
+    def density_l2_error(self, q, rho_ref):
+        """eq. (115): sum_r (rho_ref - rho)^2."""
+        q = self._c(q)
+        nx, ny = self._dims(q)
+        rho_ref = np.ascontiguousarray(rho_ref, dtype=self.rtype)
+        assert rho_ref.shape == (ny, nx)
+        return float(self.lib.orc_density_l2_error(self._p(q), self._p(rho_ref), nx, ny))
+
+    def winding(self, q):
+        """Plaquette winding numbers, int32 (5, Ny, Nx)."""
+        q = self._c(q)
+        nx, ny = self._dims(q)
+        w = np.empty((5, ny, nx), dtype=np.int32)
+        self.lib.orc_winding(self._p(q), nx, ny, self._p(w))
+        return w

@@ -509,3 +509,80 @@ extern "C" qlga_status qlga_vorticity(qlga_ctx* c, void* omega, int dst_on_devic
     if (e != cudaSuccess) return cuda_fail(c, "qlga_vorticity", e);
     return QLGA_OK;
 }
+
+// ---------------------------------------------------------------------------
+// density, eq. (115), vortex detection
+// ---------------------------------------------------------------------------
+extern "C" qlga_status qlga_density(qlga_ctx* c, void* rho, int dst_on_device) {
+    if (!c || !rho) return c ? fail(c, QLGA_EINVAL, "qlga_density: NULL") : QLGA_EINVAL;
+    if (!c->have_state) return fail(c, QLGA_ESTATE, "qlga_density: no state set");
+    Launch L{c->stream, &c->launches};
+    const int64_t n = c->nx * c->ny;
+    const size_t bytes = (size_t)n * real_size(c->prec);
+    if (dst_on_device) {
+        CU(c, launch_density(L, c->prec, c->buf[c->cur], rho, n));
+        return QLGA_OK;
+    }
+    void* tmp = nullptr;
+    if (cudaMalloc(&tmp, bytes) != cudaSuccess) { cudaGetLastError(); return fail(c, QLGA_ENOMEM, "qlga_density: cudaMalloc failed"); }
+    cudaError_t e = launch_density(L, c->prec, c->buf[c->cur], tmp, n);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(rho, tmp, bytes, cudaMemcpyDeviceToHost, c->stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
+    cudaFree(tmp);
+    if (e != cudaSuccess) return cuda_fail(c, "qlga_density", e);
+    return QLGA_OK;
+}
+
+extern "C" qlga_status qlga_density_l2_error(qlga_ctx* c, const void* rho_ref, int src_on_device, double* host_eps) {
+    if (!c || !rho_ref || !host_eps) return c ? fail(c, QLGA_EINVAL, "qlga_density_l2_error: NULL") : QLGA_EINVAL;
+    if (!c->have_state) return fail(c, QLGA_ESTATE, "qlga_density_l2_error: no state set");
+    Launch L{c->stream, &c->launches};
+    const int64_t n = c->nx * c->ny;
+    const size_t bytes = (size_t)n * real_size(c->prec);
+    void* tmp = nullptr;
+    const void* ref = rho_ref;
+    if (!src_on_device) {
+        if (cudaMalloc(&tmp, bytes) != cudaSuccess) { cudaGetLastError(); return fail(c, QLGA_ENOMEM, "qlga_density_l2_error: cudaMalloc failed"); }
+        cudaError_t e0 = cudaMemcpyAsync(tmp, rho_ref, bytes, cudaMemcpyHostToDevice, c->stream);
+        if (e0 != cudaSuccess) { cudaFree(tmp); return cuda_fail(c, "qlga_density_l2_error: H2D", e0); }
+        ref = tmp;
+    }
+    int blocks = c->obs_blocks;
+    if ((int64_t)blocks * 256 > n) blocks = (int)((n + 255) / 256);
+    double h = 0.0;
+    cudaError_t e = launch_l2_error(L, c->prec, c->buf[c->cur], ref, n, c->d_partials, blocks, c->d_sums);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(&h, c->d_sums, sizeof(double), cudaMemcpyDeviceToHost, c->stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
+    if (tmp) cudaFree(tmp);
+    if (e != cudaSuccess) return cuda_fail(c, "qlga_density_l2_error", e);
+    *host_eps = h;
+    return QLGA_OK;
+}
+
+extern "C" qlga_status qlga_vortices(qlga_ctx* c, int32_t* host_out, int64_t max_out, int64_t* host_count) {
+    if (!c || !host_count || max_out < 0 || (max_out > 0 && !host_out))
+        return c ? fail(c, QLGA_EINVAL, "qlga_vortices: bad arguments") : QLGA_EINVAL;
+    if (c->ndim != 2) return fail(c, QLGA_EUNSUP, "qlga_vortices: 2D lattices only");
+    if (!c->have_state) return fail(c, QLGA_ESTATE, "qlga_vortices: no state set");
+    Launch L{c->stream, &c->launches};
+    int* list = nullptr;
+    unsigned long long* counter = nullptr;
+    const size_t lbytes = (size_t)(max_out > 0 ? max_out : 1) * 4 * sizeof(int);
+    if (cudaMalloc(&list, lbytes) != cudaSuccess || cudaMalloc(&counter, sizeof(unsigned long long)) != cudaSuccess) {
+        cudaGetLastError(); cudaFree(list);
+        return fail(c, QLGA_ENOMEM, "qlga_vortices: cudaMalloc failed");
+    }
+    unsigned long long hc = 0;
+    cudaError_t e = cudaMemsetAsync(counter, 0, sizeof(unsigned long long), c->stream);
+    if (e == cudaSuccess) e = launch_vortices(L, c->prec, c->buf[c->cur], c->nx, c->ny, list, (long long)max_out, counter);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(&hc, counter, sizeof(hc), cudaMemcpyDeviceToHost, c->stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
+    if (e == cudaSuccess && max_out > 0) {
+        const unsigned long long ncopy = hc < (unsigned long long)max_out ? hc : (unsigned long long)max_out;
+        if (ncopy) e = cudaMemcpy(host_out, list, (size_t)ncopy * 4 * sizeof(int), cudaMemcpyDeviceToHost);
+    }
+    cudaFree(list); cudaFree(counter);
+    if (e != cudaSuccess) return cuda_fail(c, "qlga_vortices", e);
+    *host_count = (int64_t)hc;
+    return QLGA_OK;
+}

@@ -245,3 +245,114 @@ cudaError_t launch_sum_psi(const Launch& L, qlga_prec prec, const void* q, void*
 }
 
 }  // namespace qlga
+
+// ---------------------------------------------------------------------------
+// Total density, the L2 error of eq. (115) and plaquette winding numbers
+// (definitions in include/qlga.h).
+// ---------------------------------------------------------------------------
+namespace qlga {
+
+template <typename T>
+__device__ __forceinline__ double site_density(const typename vec2<T>::type* q, int64_t n, int64_t r) {
+    double s = 0.0;
+#pragma unroll
+    for (int j = 0; j < 5; ++j) {
+        const typename vec2<T>::type a = q[(int64_t)(2 * j) * n + r], b = q[(int64_t)(2 * j + 1) * n + r];
+        const double pr = (double)a.x + (double)b.x, pi = (double)a.y + (double)b.y;
+        s += pr * pr + pi * pi;
+    }
+    return s;
+}
+
+template <typename T>
+__global__ void density_kernel(const typename vec2<T>::type* q, T* rho, int64_t n) {
+    const int64_t r = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (r < n) rho[r] = (T)site_density<T>(q, n, r);
+}
+
+template <typename T>
+__global__ void __launch_bounds__(256) l2_error_kernel(const typename vec2<T>::type* q, const T* rho_ref,
+                                                       int64_t n, double* partials) {
+    double acc = 0.0;
+    for (int64_t r = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; r < n; r += (int64_t)gridDim.x * blockDim.x) {
+        const double d = (double)rho_ref[r] - site_density<T>(q, n, r);
+        acc += d * d;
+    }
+    __shared__ double sm[8];
+    for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
+    if ((threadIdx.x & 31) == 0) sm[threadIdx.x >> 5] = acc;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double s = 0.0;
+        for (int w = 0; w < 8; ++w) s += sm[w];
+        partials[(int64_t)blockIdx.x * OBS_NACC] = s;
+        for (int k = 1; k < OBS_NACC; ++k) partials[(int64_t)blockIdx.x * OBS_NACC + k] = 0.0;
+    }
+}
+
+template <typename T>
+__global__ void __launch_bounds__(128) vortices_kernel(const typename vec2<T>::type* q, int64_t nx, int64_t ny,
+                                                       int* list, long long max_out, unsigned long long* counter) {
+    using V = typename vec2<T>::type;
+    const int64_t n = nx * ny;
+    const int64_t r = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (r >= n) return;
+    const int64_t x = r % nx, y = r / nx;
+    const int64_t xp = (x == nx - 1) ? 0 : x + 1, yp = (y == ny - 1) ? 0 : y + 1;
+    const int64_t ia = r, ib = y * nx + xp, ic = yp * nx + xp, id = yp * nx + x;
+    for (int j = 0; j < 5; ++j) {
+        const V* p1 = q + (int64_t)(2 * j) * n;
+        const V* p2 = q + (int64_t)(2 * j + 1) * n;
+        V u, v;
+        u = p1[ia]; v = p2[ia]; const double ar = (double)u.x + (double)v.x, ai = (double)u.y + (double)v.y;
+        u = p1[ib]; v = p2[ib]; const double br = (double)u.x + (double)v.x, bi = (double)u.y + (double)v.y;
+        u = p1[ic]; v = p2[ic]; const double cr = (double)u.x + (double)v.x, ci = (double)u.y + (double)v.y;
+        u = p1[id]; v = p2[id]; const double dr = (double)u.x + (double)v.x, di = (double)u.y + (double)v.y;
+        const double circ = arg_prod_conj(br, bi, ar, ai) + arg_prod_conj(cr, ci, br, bi)
+                          + arg_prod_conj(dr, di, cr, ci) + arg_prod_conj(ar, ai, dr, di);
+        const int w = (int)rint(circ * 0.15915494309189533576888376337251);      // 1/(2 pi)
+        if (w != 0) {
+            const unsigned long long slot = atomicAdd(counter, 1ULL);
+            if ((long long)slot < max_out) {
+                int4 rec; rec.x = j; rec.y = (int)x; rec.z = (int)y; rec.w = w;
+                reinterpret_cast<int4*>(list)[slot] = rec;
+            }
+        }
+    }
+}
+
+cudaError_t launch_density(const Launch& L, qlga_prec prec, const void* q, void* rho, int64_t n) {
+    const unsigned blocks = (unsigned)((n + 255) / 256);
+    if (prec == QLGA_F64) density_kernel<double><<<blocks, 256, 0, L.stream>>>((const double2*)q, (double*)rho, n);
+    else density_kernel<float><<<blocks, 256, 0, L.stream>>>((const float2*)q, (float*)rho, n);
+    ++*L.counter;
+    return cudaGetLastError();
+}
+
+cudaError_t launch_l2_error(const Launch& L, qlga_prec prec, const void* q, const void* rho_ref, int64_t n,
+                            double* partials, int nblocks, double* sums) {
+    if (prec == QLGA_F64)
+        l2_error_kernel<double><<<nblocks, 256, 0, L.stream>>>((const double2*)q, (const double*)rho_ref, n, partials);
+    else
+        l2_error_kernel<float><<<nblocks, 256, 0, L.stream>>>((const float2*)q, (const float*)rho_ref, n, partials);
+    ++*L.counter;
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return e;
+    reduce_partials_kernel<<<1, 256, 0, L.stream>>>(partials, nblocks, sums);
+    ++*L.counter;
+    return cudaGetLastError();
+}
+
+cudaError_t launch_vortices(const Launch& L, qlga_prec prec, const void* q, int64_t nx, int64_t ny,
+                            int* list, long long max_out, unsigned long long* counter) {
+    const int64_t n = nx * ny;
+    const unsigned blocks = (unsigned)((n + 127) / 128);
+    if (prec == QLGA_F64)
+        vortices_kernel<double><<<blocks, 128, 0, L.stream>>>((const double2*)q, nx, ny, list, max_out, counter);
+    else
+        vortices_kernel<float><<<blocks, 128, 0, L.stream>>>((const float2*)q, nx, ny, list, max_out, counter);
+    ++*L.counter;
+    return cudaGetLastError();
+}
+
+}  // namespace qlga

@@ -48,6 +48,11 @@ cudaError_t launch_observables(const Launch& L, qlga_prec prec, const void* q, c
                                double* sums);
 cudaError_t launch_vorticity(const Launch& L, qlga_prec prec, const void* q, void* omega,
                              int64_t nx, int64_t ny);
+cudaError_t launch_density(const Launch& L, qlga_prec prec, const void* q, void* rho, int64_t nsites);
+cudaError_t launch_l2_error(const Launch& L, qlga_prec prec, const void* q, const void* rho_ref, int64_t nsites,
+                            double* partials, int nblocks, double* sums);
+cudaError_t launch_vortices(const Launch& L, qlga_prec prec, const void* q, int64_t nx, int64_t ny,
+                            int* list, long long max_out, unsigned long long* counter);
 cudaError_t launch_split_psi(const Launch& L, qlga_prec prec, const void* psi, void* q,
                              int64_t nsites, int64_t offset, int64_t count);
 cudaError_t launch_sum_psi(const Launch& L, qlga_prec prec, const void* q, void* psi,

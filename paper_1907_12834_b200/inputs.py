@@ -49,7 +49,8 @@ def seed_for(config_number: int) -> int:
 # closed-form profiles
 # --------------------------------------------------------------------------
 def sech(x):
-    return 1.0 / np.cosh(x)
+    with np.errstate(over="ignore"):          # cosh overflows to inf far from the soliton: sech -> 0
+        return 1.0 / np.cosh(x)
 
 
 def pade_profile(s, a1=11.0 / 32.0, b1=1.0 / 3.0, a2=11.0 / 384.0):

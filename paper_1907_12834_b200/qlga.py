@@ -25,6 +25,7 @@ ABI_SYMBOLS = (
     "qlga_get_state_q", "qlga_get_state_psi", "qlga_step", "qlga_observables", "qlga_vorticity",
     "qlga_launch_count", "qlga_last_error", "qlga_destroy", "qlga_version",
     "qlga_profile_enable", "qlga_profile_read", "qlga_exp_polynomial",
+    "qlga_density", "qlga_density_l2_error", "qlga_vortices",
 )
 
 
@@ -77,6 +78,12 @@ def load_library():
     lib.qlga_profile_enable.restype = I
     lib.qlga_profile_read.argtypes = [P, ctypes.POINTER(QlgaProfile)]
     lib.qlga_profile_read.restype = I
+    lib.qlga_density.argtypes = [P, P, I]
+    lib.qlga_density.restype = I
+    lib.qlga_density_l2_error.argtypes = [P, P, I, ctypes.POINTER(D)]
+    lib.qlga_density_l2_error.restype = I
+    lib.qlga_vortices.argtypes = [P, P, I64, ctypes.POINTER(I64)]
+    lib.qlga_vortices.restype = I
     lib.qlga_exp_polynomial.argtypes = [I, I, ctypes.POINTER(D), ctypes.POINTER(D), ctypes.POINTER(D)]
     lib.qlga_exp_polynomial.restype = I
     lib.qlga_version.argtypes = []
@@ -220,6 +227,31 @@ class Qlga:
         p, dev = self._ptr(out)
         self._check(_lib.qlga_vorticity(self.ctx, p, dev))
         return out
+
+    def density(self, out=None):
+        if out is None:
+            out = np.empty((self.ny, self.nx), dtype=self.np_rdtype)
+        p, dev = self._ptr(out)
+        self._check(_lib.qlga_density(self.ctx, p, dev))
+        return out
+
+    def density_l2_error(self, rho_ref):
+        """eq. (115): sum_r (rho_ref - rho)^2 against a reference density (numpy or torch)."""
+        if isinstance(rho_ref, np.ndarray):
+            rho_ref = np.ascontiguousarray(rho_ref, dtype=self.np_rdtype)
+            assert rho_ref.shape == (self.ny, self.nx)
+        p, dev = self._ptr(rho_ref)
+        eps = ctypes.c_double()
+        self._check(_lib.qlga_density_l2_error(self.ctx, p, dev, ctypes.byref(eps)))
+        return eps.value
+
+    def vortices(self, max_out=65536):
+        """(records, count): records int32 (k, 4) = (j, x, y, winding) of the plaquettes with
+        non-zero winding (order unspecified), count = total number found."""
+        out = np.empty((max_out, 4), dtype=np.int32)
+        cnt = ctypes.c_int64()
+        self._check(_lib.qlga_vortices(self.ctx, out.ctypes.data, int(max_out), ctypes.byref(cnt)))
+        return out[:min(cnt.value, max_out)].copy(), cnt.value
 
     def profile_enable(self, on=True):
         self._check(_lib.qlga_profile_enable(self.ctx, int(bool(on))))

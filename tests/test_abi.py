@@ -11,7 +11,7 @@ from conftest import ROOT
 def _declared_symbols():
     text = open(os.path.join(ROOT, "include", "qlga.h")).read()
     text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
-    return sorted(set(re.findall(r"\b(qlga_[a-z_]+)\s*\(", text)))
+    return sorted(set(re.findall(r"\b(qlga_[a-z0-9_]+)\s*\(", text)))
 
 
 def test_library_builds_loads_and_exports_every_declared_symbol():
