@@ -273,6 +273,13 @@ template <typename T>
 __device__ __forceinline__ void interaction(Site<T>& s, const UConst<T>& uc, const ExpTable& tab) {
     KCoef<T> kc;
     site_coefficients<T>(s, uc, kc);
+    // The first Horner stage of component 1 needs neither the degree nor the phase: it is
+    // issued before the warp-wide reductions below so that their latency (rsqrt, REDUX,
+    // vote, the branch on their result) is covered by 88 independent FP64 instructions.
+    cx<T> va[5], wa[5];
+#pragma unroll
+    for (int j = 0; j < 5; ++j) va[j] = s.q[j][0];
+    apply_sK<T>(va, wa, kc.az, kc.a1, kc.a6, kc.g2, kc.psi);
     // warp-uniform angle (one polynomial degree per warp keeps the Horner loops convergent)
     const float theta = __uint_as_float(__reduce_max_sync(0xffffffffu, __float_as_uint(kc.theta)));
     const T xph = uc.g0 * kc.rho;                  // scalar phase exp(-i s c0 rho)
@@ -287,14 +294,32 @@ __device__ __forceinline__ void interaction(Site<T>& s, const UConst<T>& uc, con
     const T pb0 = (T)tab.b0[p - 1];                // constant term of the polynomial (1 - O(tol))
     const cx<T> ph = mk<T>(pb0 * cs, -(pb0 * sn));
     const double* r = tab.r[p - 1];
+    {
+        cx<T> u[5];
+        const T ik = (T)r[p];
 #pragma unroll
-    for (int sg = 0; sg < 2; ++sg) {
+        for (int j = 0; j < 5; ++j) {
+            u[j].re = fma(ik, wa[j].im, va[j].re); u[j].im = fma(-ik, wa[j].re, va[j].im);
+        }
+#pragma unroll 1
+        for (int k = p - 1; k >= 1; --k) {
+            apply_sK<T>(u, wa, kc.az, kc.a1, kc.a6, kc.g2, kc.psi);
+            const T ikk = (T)r[k];
+#pragma unroll
+            for (int j = 0; j < 5; ++j) {
+                u[j].re = fma(ikk, wa[j].im, va[j].re); u[j].im = fma(-ikk, wa[j].re, va[j].im);
+            }
+        }
+#pragma unroll
+        for (int j = 0; j < 5; ++j) s.q[j][0] = cmul(ph, u[j]);
+    }
+    {
         cx<T> v[5], u[5];
 #pragma unroll
-        for (int j = 0; j < 5; ++j) v[j] = s.q[j][sg];
+        for (int j = 0; j < 5; ++j) v[j] = s.q[j][1];
         horner<T>(v, u, kc, r, p);
 #pragma unroll
-        for (int j = 0; j < 5; ++j) s.q[j][sg] = cmul(ph, u[j]);
+        for (int j = 0; j < 5; ++j) s.q[j][1] = cmul(ph, u[j]);
     }
 }
 
