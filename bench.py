@@ -65,6 +65,21 @@ def parse_args():
     return ap.parse_args()
 
 
+def load_traffic(workload, precision, order):
+    """{kernel: (dram bytes per launch, FP instr per site per launch)} from the committed ncu
+    capture (profiles/r1_traffic.csv), or {} when this workload was not captured."""
+    path = os.path.join(ROOT, "profiles", "r1_traffic.csv")
+    out = {}
+    if os.path.exists(path):
+        import csv
+        with open(path) as f:
+            for row in csv.DictReader(f):
+                if (row["workload"], row["precision"], row["order"]) == (workload, precision, order):
+                    out[row["kernel"]] = (float(row["dram_bytes_per_launch"]),
+                                          float(row["fp_thread_instr_per_site_per_launch"]))
+    return out
+
+
 def load_peaks():
     path = os.path.join(ROOT, "MEASURED_PEAKS.json")
     if os.path.exists(path):
@@ -406,12 +421,14 @@ def main():
         alu_peak = 148 * lanes * clk / 1e12                  # T instr/s at the clock seen under load
         alu_ach = units * fpi / (per_launch_ms * 1e-3) / 1e12
         hbm_ach = units * bps / (per_launch_ms * 1e-3) / 1e9
+        captured = load_traffic(args.workload, args.precision, args.order) if not args.lattice else {}
+        traffic = captured.get(dom, (None, None))[0]
         roof_hbm = {"bound": "hbm", "achieved": hbm_ach, "peak": hbm_peak, "unit": "GB/s",
-                    "frac": hbm_ach / hbm_peak, "traffic": None, "peak_kind": peak_kind,
+                    "frac": hbm_ach / hbm_peak, "traffic": traffic, "peak_kind": peak_kind,
                     "kernel": dom, "ms_per_launch": per_launch_ms,
                     "model": f"{bps:.0f} B per site-update x {units:.3g} site-updates per launch"}
         roof_alu = {"bound": "alu", "achieved": alu_ach, "peak": alu_peak, "unit": "Tinstr/s",
-                    "frac": alu_ach / alu_peak, "traffic": None, "kernel": dom,
+                    "frac": alu_ach / alu_peak, "traffic": traffic, "kernel": dom,
                     "ms_per_launch": per_launch_ms,
                     "model": f"{fpi:.0f} FP instr per site-update (degree {deg:.0f}) x {units:.3g} site-updates per launch; "
                              f"peak = 148 SMs x {lanes} lanes x {clk / 1e6:.0f} MHz (median clock under load)"}
