@@ -14,7 +14,7 @@
  *
  * State layout:  q[j][sigma][y][x]  complex,
  *   j = 0..4 <-> m_f = +2,+1,0,-1,-2 ; sigma = 0,1 <-> spinor component 1,2 ;
- *   x fastest; periodic in x (and y in 2D; ny = 1 in 1D).
+ *   x fastest; periodic in x (and y in 2D, z in 3D; ny = nz = 1 in 1D); 3D: q[j][sigma][z][y][x].
  *   Bosonic field psi_m = q_{m1} + q_{m2}.
  *
  * Readings of the paper where it is silent (R1..R9) are
@@ -47,9 +47,9 @@ static inline long wrapl(long i, long n) { i %= n; return i < 0 ? i + n : i; }
 size_t orc_sizeof_real(void) { return sizeof(real); }
 
 /* q1 = q2 = psi/2  [R6]  (psi: [5][ny][nx], q: [5][2][ny][nx]) */
-void orc_split_psi(const cplx *psi, cplx *q, long nx, long ny)
+void orc_split_psi(const cplx *psi, cplx *q, long nx, long ny, long nz)
 {
-    long n = nx * ny;
+    long n = nx * ny * nz;
     for (int j = 0; j < NM; ++j)
         for (long r = 0; r < n; ++r) {
             cplx h = psi[(size_t)j * n + r] / (real)2;
@@ -59,9 +59,9 @@ void orc_split_psi(const cplx *psi, cplx *q, long nx, long ny)
 }
 
 /* psi_m = q_m1 + q_m2 */
-void orc_psi_of_q(const cplx *q, cplx *psi, long nx, long ny)
+void orc_psi_of_q(const cplx *q, cplx *psi, long nx, long ny, long nz)
 {
-    long n = nx * ny;
+    long n = nx * ny * nz;
     for (int j = 0; j < NM; ++j)
         for (long r = 0; r < n; ++r)
             psi[(size_t)j * n + r] = q[((size_t)j * NS + 0) * n + r] + q[((size_t)j * NS + 1) * n + r];
@@ -72,11 +72,11 @@ void orc_psi_of_q(const cplx *q, cplx *psi, long nx, long ny)
  *   (q1, q2) -> (a q1 + b q2, b q1 + a q2),  a = (1-i)/2, b = (1+i)/2
  * the square-root-of-swap matrix, at every site and for every m.
  * ---------------------------------------------------------------------- */
-void orc_collide(cplx *q, long nx, long ny)
+void orc_collide(cplx *q, long nx, long ny, long nz)
 {
     const cplx a = ((real)1 - I) / (real)2;
     const cplx b = ((real)1 + I) / (real)2;
-    long n = nx * ny;
+    long n = nx * ny * nz;
     for (int j = 0; j < NM; ++j)
         for (long r = 0; r < n; ++r) {
             cplx q1 = q[((size_t)j * NS + 0) * n + r];
@@ -93,32 +93,34 @@ void orc_collide(cplx *q, long nx, long ny)
  * for all five m at once, periodic; the other spinor component is untouched.
  * d = 0 (x) or 1 (y); sigma = 0,1 <-> component 1,2.
  * ---------------------------------------------------------------------- */
-void orc_stream(cplx *q, long nx, long ny, int d, int sigma, int transpose)
+void orc_stream(cplx *q, long nx, long ny, long nz, int d, int sigma, int transpose)
 {
-    long n = nx * ny;
+    long n = nx * ny * nz;
     cplx *tmp = (cplx *)malloc(sizeof(cplx) * (size_t)n);
     long sh = transpose ? +1 : -1;          /* new(r) = old(r + sh e_d) */
     for (int j = 0; j < NM; ++j) {
         cplx *p = q + ((size_t)j * NS + (size_t)sigma) * n;
         memcpy(tmp, p, sizeof(cplx) * (size_t)n);
-        for (long y = 0; y < ny; ++y)
-            for (long x = 0; x < nx; ++x) {
-                long xs = (d == 0) ? wrapl(x + sh, nx) : x;
-                long ys = (d == 1) ? wrapl(y + sh, ny) : y;
-                p[y * nx + x] = tmp[ys * nx + xs];
-            }
+        for (long z = 0; z < nz; ++z)
+            for (long y = 0; y < ny; ++y)
+                for (long x = 0; x < nx; ++x) {
+                    long xs = (d == 0) ? wrapl(x + sh, nx) : x;
+                    long ys = (d == 1) ? wrapl(y + sh, ny) : y;
+                    long zs = (d == 2) ? wrapl(z + sh, nz) : z;
+                    p[(z * ny + y) * nx + x] = tmp[(zs * ny + ys) * nx + xs];
+                }
     }
     free(tmp);
 }
 
 /* Kinetic factor  I'_{d,sigma} = S C S^T C   (eq. 107),
  * rightmost operator applied first. */
-void orc_kinetic_factor(cplx *q, long nx, long ny, int d, int sigma)
+void orc_kinetic_factor(cplx *q, long nx, long ny, long nz, int d, int sigma)
 {
-    orc_collide(q, nx, ny);
-    orc_stream(q, nx, ny, d, sigma, 1);
-    orc_collide(q, nx, ny);
-    orc_stream(q, nx, ny, d, sigma, 0);
+    orc_collide(q, nx, ny, nz);
+    orc_stream(q, nx, ny, nz, d, sigma, 1);
+    orc_collide(q, nx, ny, nz);
+    orc_stream(q, nx, ny, nz, d, sigma, 0);
 }
 
 /* ------------------------------------------------------------------------
@@ -258,9 +260,9 @@ static void expm_apply(cplx K[NM][NM], real s, cplx v[NM])
  *   W = exp(-i s H_int[psi]),   q_{.,sigma} <- W q_{.,sigma}  for sigma = 1, 2,
  * evaluated as  exp(-i s c0 rho) * exp(-i s K)  (the scalar part commutes).
  * ---------------------------------------------------------------------- */
-void orc_interaction(cplx *q, long nx, long ny, real c0, real c1, real c2, real s)
+void orc_interaction(cplx *q, long nx, long ny, long nz, real c0, real c1, real c2, real s)
 {
-    long n = nx * ny;
+    long n = nx * ny * nz;
     for (long r = 0; r < n; ++r) {
         cplx psi[NM], K[NM][NM], v[NM];
         real rho;
@@ -282,18 +284,19 @@ void orc_interaction(cplx *q, long nx, long ny, real c0, real c1, real c2, real 
  *   order 1, interleaved eq. (112):  I'_{x1}U^{1/4} I'_{x1}U^{1/4} I'_{x2}U^{1/4} I'_{x2}U^{1/4}
  *   2D  [R7] ("n = 8"): the four y factors act before the four
  *   x factors, U (plain) or U^{1/8} (interleaved, before every factor).
+ *   3D  ("n = 12"): z factors, then y, then x; U^{1/12}.
  * ---------------------------------------------------------------------- */
-void orc_step(cplx *q, long nx, long ny, int ndim, real c0, real c1, real c2,
+void orc_step(cplx *q, long nx, long ny, long nz, int ndim, real c0, real c1, real c2,
               int order, long nsteps)
 {
     const int nfac = 4 * ndim;
     for (long t = 0; t < nsteps; ++t) {
-        if (order == 0) orc_interaction(q, nx, ny, c0, c1, c2, (real)1);
+        if (order == 0) orc_interaction(q, nx, ny, nz, c0, c1, c2, (real)1);
         for (int d = ndim - 1; d >= 0; --d)              /* y factors first, then x */
             for (int k = 0; k < 4; ++k) {
                 int sigma = (k < 2) ? 1 : 0;             /* component 2, 2, 1, 1 */
-                if (order == 1) orc_interaction(q, nx, ny, c0, c1, c2, (real)1 / (real)nfac);
-                orc_kinetic_factor(q, nx, ny, d, sigma);
+                if (order == 1) orc_interaction(q, nx, ny, nz, c0, c1, c2, (real)1 / (real)nfac);
+                orc_kinetic_factor(q, nx, ny, nz, d, sigma);
             }
     }
 }
@@ -314,17 +317,18 @@ void orc_step(cplx *q, long nx, long ny, int ndim, real c0, real c1, real c2,
  *   out[18,19] e_dt = i(<psi|psi> - <psi|psi_prev>)/<psi|psi>    eq. (85)
  *              (NaN if qprev == NULL), <a|b> = sum_{r,m} a_m^* b_m.
  * ---------------------------------------------------------------------- */
-void orc_observables(const cplx *q, const cplx *qprev, long nx, long ny, int ndim,
+void orc_observables(const cplx *q, const cplx *qprev, long nx, long ny, long nz, int ndim,
                      real c0, real c1, real c2, double *out)
 {
-    long n = nx * ny;
+    long n = nx * ny * nz;
     real nm[NM] = {0, 0, 0, 0, 0}, normq = 0, Fs[3] = {0, 0, 0}, a2 = 0;
     real ekin = 0, s_rho2 = 0, s_F2 = 0;
     cplx a00 = 0, ov = 0;
     const real rt5 = sqrt((real)5);
+    for (long zz = 0; zz < nz; ++zz)
     for (long y = 0; y < ny; ++y)
         for (long x = 0; x < nx; ++x) {
-            long r = y * nx + x;
+            long r = (zz * ny + y) * nx + x;
             cplx psi[NM], chi[NM], th;
             real rho, F[3];
             for (int j = 0; j < NM; ++j) {
@@ -344,7 +348,8 @@ void orc_observables(const cplx *q, const cplx *qprev, long nx, long ny, int ndi
             for (int d = 0; d < ndim; ++d) {
                 long xn = (d == 0) ? wrapl(x + 1, nx) : x;
                 long yn = (d == 1) ? wrapl(y + 1, ny) : y;
-                long rn = yn * nx + xn;
+                long zn = (d == 2) ? wrapl(zz + 1, nz) : zz;
+                long rn = (zn * ny + yn) * nx + xn;
                 for (int j = 0; j < NM; ++j) {
                     cplx pn = q[((size_t)j * NS + 0) * n + rn] + q[((size_t)j * NS + 1) * n + rn];
                     cplx df = pn - psi[j];
@@ -420,9 +425,9 @@ void orc_vorticity(const cplx *q, long nx, long ny, real *omega)
  *   epsilon = sum_lattice ( rho_ref(r) - rho(r) )^2 .
  * (the convergence study of Figs. 23-24.)
  * ---------------------------------------------------------------------- */
-void orc_density(const cplx *q, long nx, long ny, real *rho)
+void orc_density(const cplx *q, long nx, long ny, long nz, real *rho)
 {
-    long n = nx * ny;
+    long n = nx * ny * nz;
     for (long r = 0; r < n; ++r) {
         real s = 0;
         for (int j = 0; j < NM; ++j) {
@@ -433,11 +438,11 @@ void orc_density(const cplx *q, long nx, long ny, real *rho)
     }
 }
 
-double orc_density_l2_error(const cplx *q, const real *rho_ref, long nx, long ny)
+double orc_density_l2_error(const cplx *q, const real *rho_ref, long nx, long ny, long nz)
 {
-    long n = nx * ny;
+    long n = nx * ny * nz;
     real *rho = (real *)malloc(sizeof(real) * (size_t)n);
-    orc_density(q, nx, ny, rho);
+    orc_density(q, nx, ny, nz, rho);
     real e = 0;
     for (long r = 0; r < n; ++r) { real d = rho_ref[r] - rho[r]; e += d * d; }
     free(rho);

@@ -5,7 +5,8 @@ bench.py's cpu_baseline / --impl reference legs may import this module.  It neve
 imports the CUDA package and the CUDA package never imports it.
 
 `Oracle(precision="double" | "longdouble")` wraps one build of the C file;
-arrays are numpy complex128 (or clongdouble) in the layout q[5][2][Ny][Nx].
+arrays are numpy complex128 (or clongdouble) in the layout q[5][2][Ny][Nx]
+(1D, 2D) or q[5][2][Nz][Ny][Nx] (3D).
 """
 from __future__ import annotations
 
@@ -49,18 +50,18 @@ class Oracle:
         assert self.lib.orc_sizeof_real() == np.dtype(self.rtype).itemsize
         L, I, P, R = ctypes.c_long, ctypes.c_int, ctypes.c_void_p, self.creal
         sig = {
-            "orc_split_psi": [P, P, L, L],
-            "orc_psi_of_q": [P, P, L, L],
-            "orc_collide": [P, L, L],
-            "orc_stream": [P, L, L, I, I, I],
-            "orc_kinetic_factor": [P, L, L, I, I],
+            "orc_split_psi": [P, P, L, L, L],
+            "orc_psi_of_q": [P, P, L, L, L],
+            "orc_collide": [P, L, L, L],
+            "orc_stream": [P, L, L, L, I, I, I],
+            "orc_kinetic_factor": [P, L, L, L, I, I],
             "orc_spin_matrices": [P, P, P],
             "orc_site_hamiltonian": [P, R, R, R, P],
-            "orc_interaction": [P, L, L, R, R, R, R],
-            "orc_step": [P, L, L, I, R, R, R, I, L],
-            "orc_observables": [P, P, L, L, I, R, R, R, P],
+            "orc_interaction": [P, L, L, L, R, R, R, R],
+            "orc_step": [P, L, L, L, I, R, R, R, I, L],
+            "orc_observables": [P, P, L, L, L, I, R, R, R, P],
             "orc_vorticity": [P, L, L, P],
-            "orc_density": [P, L, L, P],
+            "orc_density": [P, L, L, L, P],
             "orc_winding": [P, L, L, P],
         }
         for name, args in sig.items():
@@ -68,7 +69,7 @@ class Oracle:
             fn.argtypes = args
             fn.restype = None
 
-        self.lib.orc_density_l2_error.argtypes = [P, P, L, L]
+        self.lib.orc_density_l2_error.argtypes = [P, P, L, L, L]
         self.lib.orc_density_l2_error.restype = ctypes.c_double
 
     # -- helpers ---------------------------------------------------------
@@ -84,40 +85,49 @@ class Oracle:
 
     @staticmethod
     def _dims(q):
-        assert q.ndim == 4 and q.shape[0] == 5 and q.shape[1] == 2, q.shape
+        """(nx, ny, nz) of a state q[5][2][Ny][Nx] (1D/2D) or q[5][2][Nz][Ny][Nx] (3D)."""
+        assert q.ndim in (4, 5) and q.shape[0] == 5 and q.shape[1] == 2, q.shape
+        if q.ndim == 4:
+            return q.shape[3], q.shape[2], 1
+        return q.shape[4], q.shape[3], q.shape[2]
+
+    @staticmethod
+    def _dims2(q):
+        assert q.ndim == 4, "2D-only operation"
         return q.shape[3], q.shape[2]
 
     # -- operators (each returns a new array) ------------------------------
     def split_psi(self, psi):
         psi = self._c(psi)
-        _, ny, nx = psi.shape
-        q = np.empty((5, 2, ny, nx), dtype=self.ctype)
-        self.lib.orc_split_psi(self._p(psi), self._p(q), nx, ny)
+        sp = psi.shape[1:]
+        nz, ny, nx = ((1,) + sp) if len(sp) == 2 else sp
+        q = np.empty((5, 2) + sp, dtype=self.ctype)
+        self.lib.orc_split_psi(self._p(psi), self._p(q), nx, ny, nz)
         return q
 
     def psi_of_q(self, q):
         q = self._c(q)
-        nx, ny = self._dims(q)
-        psi = np.empty((5, ny, nx), dtype=self.ctype)
-        self.lib.orc_psi_of_q(self._p(q), self._p(psi), nx, ny)
+        nx, ny, nz = self._dims(q)
+        psi = np.empty((5,) + q.shape[2:], dtype=self.ctype)
+        self.lib.orc_psi_of_q(self._p(q), self._p(psi), nx, ny, nz)
         return psi
 
     def collide(self, q):
         q = self._c(q).copy()
-        nx, ny = self._dims(q)
-        self.lib.orc_collide(self._p(q), nx, ny)
+        nx, ny, nz = self._dims(q)
+        self.lib.orc_collide(self._p(q), nx, ny, nz)
         return q
 
     def stream(self, q, d, sigma, transpose=False):
         q = self._c(q).copy()
-        nx, ny = self._dims(q)
-        self.lib.orc_stream(self._p(q), nx, ny, int(d), int(sigma), int(bool(transpose)))
+        nx, ny, nz = self._dims(q)
+        self.lib.orc_stream(self._p(q), nx, ny, nz, int(d), int(sigma), int(bool(transpose)))
         return q
 
     def kinetic_factor(self, q, d, sigma):
         q = self._c(q).copy()
-        nx, ny = self._dims(q)
-        self.lib.orc_kinetic_factor(self._p(q), nx, ny, int(d), int(sigma))
+        nx, ny, nz = self._dims(q)
+        self.lib.orc_kinetic_factor(self._p(q), nx, ny, nz, int(d), int(sigma))
         return q
 
     def spin_matrices(self):
@@ -135,37 +145,37 @@ class Oracle:
 
     def interaction(self, q, couplings, s):
         q = self._c(q).copy()
-        nx, ny = self._dims(q)
+        nx, ny, nz = self._dims(q)
         c0, c1, c2 = couplings
-        self.lib.orc_interaction(self._p(q), nx, ny, self.creal(c0), self.creal(c1),
+        self.lib.orc_interaction(self._p(q), nx, ny, nz, self.creal(c0), self.creal(c1),
                                  self.creal(c2), self.creal(s))
         return q
 
     def step(self, q, ndim, couplings, order, nsteps=1):
         """order: 0 = plain (eq. 108), 1 = interleaved (eq. 112)."""
         q = self._c(q).copy()
-        nx, ny = self._dims(q)
-        assert ndim in (1, 2) and (ndim == 2 or ny == 1)
+        nx, ny, nz = self._dims(q)
+        assert ndim in (1, 2, 3) and (ndim >= 2 or ny == 1) and (ndim == 3 or nz == 1)
         c0, c1, c2 = couplings
-        self.lib.orc_step(self._p(q), nx, ny, int(ndim), self.creal(c0), self.creal(c1),
+        self.lib.orc_step(self._p(q), nx, ny, nz, int(ndim), self.creal(c0), self.creal(c1),
                           self.creal(c2), int(order), int(nsteps))
         return q
 
     def observables(self, q, ndim, couplings, qprev=None):
         q = self._c(q)
-        nx, ny = self._dims(q)
+        nx, ny, nz = self._dims(q)
         out = np.empty(20, dtype=np.float64)
         c0, c1, c2 = couplings
         if qprev is not None:
             qprev = self._c(qprev, q.shape)
         self.lib.orc_observables(self._p(q), None if qprev is None else self._p(qprev),
-                                 nx, ny, int(ndim), self.creal(c0), self.creal(c1),
+                                 nx, ny, nz, int(ndim), self.creal(c0), self.creal(c1),
                                  self.creal(c2), self._p(out))
         return dict(zip(OBS_FIELDS, out.tolist()))
 
     def vorticity(self, q):
         q = self._c(q)
-        nx, ny = self._dims(q)
+        nx, ny = self._dims2(q)
         om = np.empty((5, ny, nx), dtype=self.rtype)
         self.lib.orc_vorticity(self._p(q), nx, ny, self._p(om))
         return om
@@ -173,23 +183,23 @@ class Oracle:
     def density(self, q):
         """rho(r) = sum_m |psi_m|^2, shape (Ny, Nx)."""
         q = self._c(q)
-        nx, ny = self._dims(q)
-        rho = np.empty((ny, nx), dtype=self.rtype)
-        self.lib.orc_density(self._p(q), nx, ny, self._p(rho))
+        nx, ny, nz = self._dims(q)
+        rho = np.empty(q.shape[2:], dtype=self.rtype)
+        self.lib.orc_density(self._p(q), nx, ny, nz, self._p(rho))
         return rho
 
     def density_l2_error(self, q, rho_ref):
         """eq. (115): sum_r (rho_ref - rho)^2."""
         q = self._c(q)
-        nx, ny = self._dims(q)
+        nx, ny, nz = self._dims(q)
         rho_ref = np.ascontiguousarray(rho_ref, dtype=self.rtype)
-        assert rho_ref.shape == (ny, nx)
-        return float(self.lib.orc_density_l2_error(self._p(q), self._p(rho_ref), nx, ny))
+        assert rho_ref.shape == q.shape[2:]
+        return float(self.lib.orc_density_l2_error(self._p(q), self._p(rho_ref), nx, ny, nz))
 
     def winding(self, q):
         """Plaquette winding numbers, int32 (5, Ny, Nx)."""
         q = self._c(q)
-        nx, ny = self._dims(q)
+        nx, ny = self._dims2(q)
         w = np.empty((5, ny, nx), dtype=np.int32)
         self.lib.orc_winding(self._p(q), nx, ny, self._p(w))
         return w

@@ -186,12 +186,13 @@ def random_field(dims, seed, amplitude=0.1):
 
 
 def random_spinor_state(dims, seed, amplitude=0.1):
-    """Seeded random full spinor state q of shape (5, 2, Ny, Nx) complex128
-    (both spinor components independent, i.e. with an antisymmetric part)."""
-    nx, ny = dims
+    """Seeded random full spinor state q of shape (5, 2, Ny, Nx) (dims = (Nx, Ny)) or
+    (5, 2, Nz, Ny, Nx) (dims = (Nx, Ny, Nz)) complex128, both spinor components
+    independent, i.e. with an antisymmetric part."""
+    shape = (5, 2) + tuple(reversed(tuple(dims)))
     rng = np.random.default_rng(seed)
-    re = rng.standard_normal((5, 2, ny, nx))
-    im = rng.standard_normal((5, 2, ny, nx))
+    re = rng.standard_normal(shape)
+    im = rng.standard_normal(shape)
     return amplitude * (re + 1j * im) / np.sqrt(2.0)
 
 
