@@ -17,12 +17,12 @@
  * stream; calls that return data to the host synchronise that stream.
  *
  * Data layout (both for the caller's transfers and inside the device buffers):
- *   q   : [5][2][Ny][Nx] complex   index ((j*2 + sigma)*Ny + y)*Nx + x
- *   psi : [5][Ny][Nx]    complex
- *   omega : [5][Ny][Nx]  real
+ *   q   : [5][2][Nz][Ny][Nx] complex   index (((j*2 + sigma)*Nz + z)*Ny + y)*Nx + x
+ *   psi : [5][Nz][Ny][Nx]    complex
+ *   omega : [5][Ny][Nx]      real (2D only)
  *   j = 0..4 <-> m_f = +2,+1,0,-1,-2;  sigma = 0,1 <-> spinor component 1,2;
- *   x fastest; Ny = 1 in 1D; complex = interleaved (re, im) of the context's real
- *   type (double for QLGA_F64, float for QLGA_F32); lattice periodic in x and y.
+ *   x fastest; Ny = Nz = 1 in 1D, Nz = 1 in 2D; complex = interleaved (re, im) of the
+ *   context's real type (double for QLGA_F64, float for QLGA_F32); periodic in x, y, z.
  */
 #ifndef QLGA_H
 #define QLGA_H
@@ -49,8 +49,9 @@ typedef enum { QLGA_F64 = 0, QLGA_F32 = 1 } qlga_prec;
 
 /* Operator ordering of one time step (rightmost operator acts first):
  *   QLGA_PLAIN        eq. (108):  I'_x1 I'_x1 I'_x2 I'_x2 [I'_y1 I'_y1 I'_y2 I'_y2] U
- *   QLGA_INTERLEAVED  eq. (112):  every I' preceded by U^{1/(4 ndim)}, "n = 8" in 2D
- *                                 (PAPER.md:1064).  The y factors act before the x factors (R7). */
+ *   QLGA_INTERLEAVED  eq. (112):  every I' preceded by U^{1/(4 ndim)}, "n = 8" in 2D and
+ *                                 "n = 12" in 3D.  Factors of z act first, then
+ *                                 y, then x (R7). */
 typedef enum { QLGA_PLAIN = 0, QLGA_INTERLEAVED = 1 } qlga_order;
 
 /* Tunables of qlga_set_option. */
@@ -88,30 +89,31 @@ typedef struct {
 
 /* Create a context (BASELINE.json north_star "qlga_init").
  *   out        HOST  receives the context.
- *   ndim       1 or 2.        dims  HOST  {Nx, Ny}; Ny must be 1 when ndim == 1; Nx, Ny >= 1.
+ *   ndim       1, 2 or 3.     dims  HOST  {Nx, Ny} (Ny must be 1 when ndim == 1) or, when
+ *              ndim == 3, {Nx, Ny, Nz}; all >= 1.
  *   c0,c1,c2   the paper's g0, g1, g2 of eq. (32)-(34).
  *   dev_buf_a, dev_buf_b   DEVICE, caller-owned, 16-byte aligned, each >= qlga_state_bytes().
- *   dev_buf_c  DEVICE or NULL.  Optional third buffer: in 2D a step is two passes
- *              (a -> b -> c), so the state of the previous step survives only with a
- *              third buffer; without it e_dt is NaN in 2D.  Unused in 1D.
+ *   dev_buf_c  DEVICE or NULL.  Optional third buffer: in 2D (3D) a step is two (three)
+ *              passes, so the state of the previous step survives only with a third
+ *              buffer; without it e_dt is NaN in 2D and 3D.  Unused in 1D.
  *   buf_bytes  size of each buffer.
  *   cuda_stream  the caller's cudaStream_t (NULL = legacy default stream).
  * Errors: QLGA_EINVAL (arguments), QLGA_ECUDA (no sm_100 device / CUDA failure), QLGA_ENOMEM. */
-qlga_status qlga_init(qlga_ctx** out, int ndim, const int64_t dims[2],
+qlga_status qlga_init(qlga_ctx** out, int ndim, const int64_t* dims,
                       double c0, double c1, double c2, qlga_order order, qlga_prec prec,
                       void* dev_buf_a, void* dev_buf_b, void* dev_buf_c, size_t buf_bytes,
                       void* cuda_stream);
 
-/* Bytes one state buffer needs: 10 * Nx * Ny * 2 * sizeof(real).  0 on bad arguments. */
-size_t qlga_state_bytes(int ndim, const int64_t dims[2], qlga_prec prec);
+/* Bytes one state buffer needs: 10 * Nx * Ny * Nz * 2 * sizeof(real).  0 on bad arguments. */
+size_t qlga_state_bytes(int ndim, const int64_t* dims, qlga_prec prec);
 
 /* Set a tunable (see qlga_option).  QLGA_EINVAL for unknown keys / bad values. */
 qlga_status qlga_set_option(qlga_ctx*, qlga_option key, int64_t value);
 
 /* Load the bosonic field: q_m1 = q_m2 = psi_m / 2 (reading R6).  psi: HOST or DEVICE
- * ([5][Ny][Nx] complex of the context's real type) per src_on_device.  Resets step to 0. */
+ * ([5][Nz][Ny][Nx] complex of the context's real type) per src_on_device.  Resets step to 0. */
 qlga_status qlga_set_state_psi(qlga_ctx*, const void* psi, int src_on_device);
-/* Load / read back the full spinor state q ([5][2][Ny][Nx] complex); also the checkpoint format. */
+/* Load / read back the full spinor state q ([5][2][Nz][Ny][Nx] complex); also the checkpoint format. */
 qlga_status qlga_set_state_q(qlga_ctx*, const void* q, int src_on_device);
 qlga_status qlga_get_state_q(qlga_ctx*, void* q, int dst_on_device);
 /* Read back psi_m = q_m1 + q_m2. */
@@ -129,7 +131,7 @@ qlga_status qlga_observables(qlga_ctx*, qlga_obs* host_out);
  * omega: HOST or DEVICE [5][Ny][Nx] real of the context's real type.  QLGA_EUNSUP in 1D. */
 qlga_status qlga_vorticity(qlga_ctx*, void* omega, int dst_on_device);
 
-/* Total density rho(r) = sum_m |psi_m(r)|^2 = psi psi^dagger; rho: HOST or DEVICE [Ny][Nx] real. */
+/* Total density rho(r) = sum_m |psi_m(r)|^2 = psi psi^dagger; rho: HOST or DEVICE [Nz][Ny][Nx] real. */
 qlga_status qlga_density(qlga_ctx*, void* rho, int dst_on_device);
 
 /* L2 error of eq. (115), PAPER.md:1074 (the paper's convergence measure, Figs. 23-24):

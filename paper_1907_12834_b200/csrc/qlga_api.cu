@@ -110,14 +110,24 @@ extern "C" qlga_status qlga_exp_polynomial(int tol_log2, int p, double* theta_ma
 
 extern "C" const char* qlga_version(void) { return "qlga-b200 0.1 (sm_100a)"; }
 
-extern "C" size_t qlga_state_bytes(int ndim, const int64_t dims[2], qlga_prec prec) {
-    if (!dims || (ndim != 1 && ndim != 2)) return 0;
-    if (dims[0] < 1 || dims[1] < 1 || (ndim == 1 && dims[1] != 1)) return 0;
-    if (prec != QLGA_F64 && prec != QLGA_F32) return 0;
-    return (size_t)10 * (size_t)dims[0] * (size_t)dims[1] * 2 * real_size(prec);
+// lattice extents from the caller's dims[]: {Nx, Ny} for ndim 1 and 2 (Ny = 1 in 1D),
+// {Nx, Ny, Nz} for ndim 3.  Returns false on bad arguments.
+static bool lattice_dims(int ndim, const int64_t* dims, int64_t& nx, int64_t& ny, int64_t& nz) {
+    if (!dims || ndim < 1 || ndim > 3) return false;
+    nx = dims[0]; ny = dims[1]; nz = (ndim == 3) ? dims[2] : 1;
+    if (nx < 1 || ny < 1 || nz < 1 || (ndim == 1 && ny != 1)) return false;
+    if ((double)nx * (double)ny * (double)nz > 1.0e12) return false;
+    return true;
 }
 
-extern "C" qlga_status qlga_init(qlga_ctx** out, int ndim, const int64_t dims[2],
+extern "C" size_t qlga_state_bytes(int ndim, const int64_t* dims, qlga_prec prec) {
+    int64_t nx, ny, nz;
+    if (!lattice_dims(ndim, dims, nx, ny, nz)) return 0;
+    if (prec != QLGA_F64 && prec != QLGA_F32) return 0;
+    return (size_t)10 * (size_t)nx * (size_t)ny * (size_t)nz * 2 * real_size(prec);
+}
+
+extern "C" qlga_status qlga_init(qlga_ctx** out, int ndim, const int64_t* dims,
                                  double c0, double c1, double c2, qlga_order order, qlga_prec prec,
                                  void* dev_buf_a, void* dev_buf_b, void* dev_buf_c, size_t buf_bytes,
                                  void* cuda_stream) {
@@ -135,8 +145,6 @@ extern "C" qlga_status qlga_init(qlga_ctx** out, int ndim, const int64_t dims[2]
         return fail(nullptr, QLGA_EINVAL, "qlga_init: device buffers must be 16-byte aligned");
     if (dev_buf_c && (dev_buf_c == dev_buf_a || dev_buf_c == dev_buf_b))
         return fail(nullptr, QLGA_EINVAL, "qlga_init: dev_buf_c aliases another buffer");
-    if (dims[0] * dims[1] > (int64_t)1 << 40)
-        return fail(nullptr, QLGA_EINVAL, "qlga_init: lattice too large");
 
     int dev = 0;
     cudaDeviceProp prop;
@@ -147,7 +155,8 @@ extern "C" qlga_status qlga_init(qlga_ctx** out, int ndim, const int64_t dims[2]
     qlga_ctx* c = new (std::nothrow) qlga_ctx;
     if (!c) return fail(nullptr, QLGA_ENOMEM, "qlga_init: out of host memory");
     memset(c, 0, sizeof(*c));
-    c->ndim = ndim; c->nx = dims[0]; c->ny = dims[1];
+    c->ndim = ndim;
+    lattice_dims(ndim, dims, c->nx, c->ny, c->nz);
     c->c[0] = c0; c->c[1] = c1; c->c[2] = c2;
     c->order = order; c->prec = prec;
     c->buf[0] = dev_buf_a; c->buf[1] = dev_buf_b; c->buf[2] = dev_buf_c;
@@ -253,7 +262,8 @@ extern "C" qlga_status qlga_profile_read(qlga_ctx* c, qlga_profile* out) {
 // ---------------------------------------------------------------------------
 // state transfers
 // ---------------------------------------------------------------------------
-static size_t state_bytes(const qlga_ctx* c) { return (size_t)10 * c->nx * c->ny * 2 * real_size(c->prec); }
+static size_t state_bytes(const qlga_ctx* c) { return (size_t)10 * c->nx * c->ny * c->nz * 2 * real_size(c->prec); }
+static int64_t nsites(const qlga_ctx* c) { return c->nx * c->ny * c->nz; }
 
 static qlga_status ensure_stage(qlga_ctx* c) {
     if (c->d_stage) return QLGA_OK;
@@ -287,7 +297,7 @@ extern "C" qlga_status qlga_get_state_q(qlga_ctx* c, void* q, int dst_on_device)
 
 extern "C" qlga_status qlga_set_state_psi(qlga_ctx* c, const void* psi, int src_on_device) {
     if (!c || !psi) return c ? fail(c, QLGA_EINVAL, "qlga_set_state_psi: NULL") : QLGA_EINVAL;
-    const int64_t n = c->nx * c->ny;
+    const int64_t n = nsites(c);
     Launch L{c->stream, &c->launches};
     if (src_on_device) {
         CU(c, launch_split_psi(L, c->prec, psi, c->buf[0], n, 0, n));
@@ -313,7 +323,7 @@ extern "C" qlga_status qlga_set_state_psi(qlga_ctx* c, const void* psi, int src_
 extern "C" qlga_status qlga_get_state_psi(qlga_ctx* c, void* psi, int dst_on_device) {
     if (!c || !psi) return c ? fail(c, QLGA_EINVAL, "qlga_get_state_psi: NULL") : QLGA_EINVAL;
     if (!c->have_state) return fail(c, QLGA_ESTATE, "qlga_get_state_psi: no state set");
-    const int64_t n = c->nx * c->ny;
+    const int64_t n = nsites(c);
     Launch L{c->stream, &c->launches};
     if (dst_on_device) {
         CU(c, launch_sum_psi(L, c->prec, c->buf[c->cur], psi, n, 0, n));
@@ -363,7 +373,7 @@ static qlga_status step_fused(qlga_ctx* c, int64_t nsteps) {
     const bool inter = c->order == QLGA_INTERLEAVED;
     const double s = inter ? 1.0 / (4.0 * c->ndim) : 1.0;
     PassParams P;
-    P.nx = c->nx; P.ny = c->ny;
+    P.nx = c->nx; P.ny = c->ny; P.nz = c->nz;
     fill_pass_consts(c, P, s);
     if (c->ndim == 1) {
         const int threads = c->threads_x ? c->threads_x : 128;
@@ -391,22 +401,31 @@ static qlga_status step_fused(qlga_ctx* c, int64_t nsteps) {
         }
         return QLGA_OK;
     }
+    // 2D: y pass then x pass; 3D: z, y, x (R7).  The passes ping-pong between buffers; with a
+    // third buffer the state before the step survives (for eq. 85), otherwise it is overwritten.
     for (int64_t t = 0; t < nsteps; ++t) {
-        const int mid = pick_other(c, c->cur, -1);                     // any buffer but cur
-        int dst = pick_other(c, c->cur, mid);                          // third buffer if present
-        const bool keep_prev = dst >= 0;
-        if (dst < 0) dst = c->cur;
-        P.ksteps = 1;
-        P.src = c->buf[c->cur]; P.dst = c->buf[mid];
-        P.umode = inter ? 2 : 1;                                       // U is the rightmost operator
-        prof_mark(c, 1);
-        CU(c, launch_pass(L, c->prec, 1, P, c->threads_y, c->tile_y));
-        P.src = c->buf[mid]; P.dst = c->buf[dst];
-        P.umode = inter ? 2 : 0;
-        prof_mark(c, 0);
-        CU(c, launch_pass(L, c->prec, 0, P, c->threads_x, 1));
-        c->prev = keep_prev ? c->cur : -1;
-        c->cur = dst;
+        const int start = c->cur;
+        const int third = pick_other(c, start, pick_other(c, start, -1));
+        int src = start;
+        for (int d = c->ndim - 1; d >= 0; --d) {
+            int dst;
+            if (third >= 0) {
+                // rotate through the two buffers that do not hold the step's initial state
+                const int a = pick_other(c, start, -1), b = third;
+                dst = (src == a) ? b : a;
+            } else {
+                dst = pick_other(c, src, -1);
+            }
+            P.ksteps = 1;
+            P.src = c->buf[src]; P.dst = c->buf[dst];
+            // U is the rightmost operator of the plain step: it rides on the first pass
+            P.umode = inter ? 2 : (d == c->ndim - 1 ? 1 : 0);
+            prof_mark(c, d == 0 ? 0 : 1);
+            CU(c, launch_pass(L, c->prec, d, P, d == 0 ? c->threads_x : c->threads_y, d == 0 ? 1 : c->tile_y));
+            src = dst;
+        }
+        c->prev = (third >= 0) ? start : -1;
+        c->cur = src;
         ++c->step;
     }
     return QLGA_OK;
@@ -419,13 +438,13 @@ static qlga_status step_per_operator(qlga_ctx* c, int64_t nsteps) {
     const double g[3] = {s * c->c[0], s * c->c[1], s * c->c[2] / 5.0};
     for (int64_t t = 0; t < nsteps; ++t) {
         prof_mark(c, 2);
-        if (!inter) CU(c, launch_interaction(L, c->prec, c->buf[c->cur], c->nx, c->ny, g, c->tab));
+        if (!inter) CU(c, launch_interaction(L, c->prec, c->buf[c->cur], nsites(c), g, c->tab));
         for (int d = c->ndim - 1; d >= 0; --d)
             for (int k = 0; k < 4; ++k) {
                 const int sigma = (k < 2) ? 1 : 0;                     // components 2, 2, 1, 1
-                if (inter) CU(c, launch_interaction(L, c->prec, c->buf[c->cur], c->nx, c->ny, g, c->tab));
+                if (inter) CU(c, launch_interaction(L, c->prec, c->buf[c->cur], nsites(c), g, c->tab));
                 const int dst = pick_other(c, c->cur, -1);
-                CU(c, launch_kinetic(L, c->prec, c->buf[c->cur], c->buf[dst], c->nx, c->ny, d, sigma));
+                CU(c, launch_kinetic(L, c->prec, c->buf[c->cur], c->buf[dst], c->nx, c->ny, c->nz, d, sigma));
                 c->cur = dst;
             }
         c->prev = -1;
@@ -452,10 +471,10 @@ extern "C" qlga_status qlga_observables(qlga_ctx* c, qlga_obs* out) {
     if (!c->have_state) return fail(c, QLGA_ESTATE, "qlga_observables: no state set");
     Launch L{c->stream, &c->launches};
     const void* prev = (c->prev >= 0) ? c->buf[c->prev] : nullptr;
-    int64_t n = c->nx * c->ny;
+    int64_t n = nsites(c);
     int blocks = c->obs_blocks;
     if ((int64_t)blocks * 256 > n) blocks = (int)((n + 255) / 256);
-    CU(c, launch_observables(L, c->prec, c->buf[c->cur], prev, c->nx, c->ny, c->ndim,
+    CU(c, launch_observables(L, c->prec, c->buf[c->cur], prev, c->nx, c->ny, c->nz, c->ndim,
                              c->d_partials, blocks, c->d_sums));
     double h[OBS_NACC];
     CU(c, cudaMemcpyAsync(h, c->d_sums, sizeof(h), cudaMemcpyDeviceToHost, c->stream));
@@ -517,7 +536,7 @@ extern "C" qlga_status qlga_density(qlga_ctx* c, void* rho, int dst_on_device) {
     if (!c || !rho) return c ? fail(c, QLGA_EINVAL, "qlga_density: NULL") : QLGA_EINVAL;
     if (!c->have_state) return fail(c, QLGA_ESTATE, "qlga_density: no state set");
     Launch L{c->stream, &c->launches};
-    const int64_t n = c->nx * c->ny;
+    const int64_t n = nsites(c);
     const size_t bytes = (size_t)n * real_size(c->prec);
     if (dst_on_device) {
         CU(c, launch_density(L, c->prec, c->buf[c->cur], rho, n));
@@ -537,7 +556,7 @@ extern "C" qlga_status qlga_density_l2_error(qlga_ctx* c, const void* rho_ref, i
     if (!c || !rho_ref || !host_eps) return c ? fail(c, QLGA_EINVAL, "qlga_density_l2_error: NULL") : QLGA_EINVAL;
     if (!c->have_state) return fail(c, QLGA_ESTATE, "qlga_density_l2_error: no state set");
     Launch L{c->stream, &c->launches};
-    const int64_t n = c->nx * c->ny;
+    const int64_t n = nsites(c);
     const size_t bytes = (size_t)n * real_size(c->prec);
     void* tmp = nullptr;
     const void* ref = rho_ref;

@@ -30,9 +30,9 @@ __device__ __forceinline__ void load_psi(const typename vec2<T>::type* q, int64_
 template <typename T>
 __global__ void __launch_bounds__(256) observables_kernel(const typename vec2<T>::type* q,
                                                           const typename vec2<T>::type* qprev,
-                                                          int64_t nx, int64_t ny, int ndim,
+                                                          int64_t nx, int64_t ny, int64_t nz, int ndim,
                                                           double* partials) {
-    const int64_t n = nx * ny;
+    const int64_t n = nx * ny * nz;
     double acc[OBS_NACC];
 #pragma unroll
     for (int k = 0; k < OBS_NACC; ++k) acc[k] = 0.0;
@@ -65,12 +65,13 @@ __global__ void __launch_bounds__(256) observables_kernel(const typename vec2<T>
         acc[A_A00R] += ar; acc[A_A00I] += ai; acc[A_A2] += ar * ar + ai * ai;
         acc[A_RHO2] += rho * rho;
         acc[A_F2] += Fx * Fx + Fy * Fy + Fz * Fz;
-        // kinetic: forward differences along x (and y)
-        const int64_t x = r % nx, y = r / nx;
+        // kinetic: forward differences along x (and y, z)
+        const int64_t x = r % nx, y = (r / nx) % ny, z = r / (nx * ny);
         for (int d = 0; d < ndim; ++d) {
             int64_t rn;
-            if (d == 0) rn = y * nx + (x == nx - 1 ? 0 : x + 1);
-            else rn = (y == ny - 1 ? 0 : y + 1) * nx + x;
+            if (d == 0) rn = r - x + (x == nx - 1 ? 0 : x + 1);
+            else if (d == 1) rn = r + ((y == ny - 1 ? 0 : y + 1) - y) * nx;
+            else rn = r + ((z == nz - 1 ? 0 : z + 1) - z) * nx * ny;
             double qr[5], qi[5];
             load_psi<T>(q, n, rn, qr, qi, nullptr);
 #pragma unroll
@@ -126,14 +127,14 @@ __global__ void __launch_bounds__(256) reduce_partials_kernel(const double* part
 }
 
 cudaError_t launch_observables(const Launch& L, qlga_prec prec, const void* q, const void* qprev,
-                               int64_t nx, int64_t ny, int ndim, double* partials, int nblocks,
+                               int64_t nx, int64_t ny, int64_t nz, int ndim, double* partials, int nblocks,
                                double* sums) {
     if (prec == QLGA_F64)
         observables_kernel<double><<<nblocks, 256, 0, L.stream>>>((const double2*)q, (const double2*)qprev,
-                                                                   nx, ny, ndim, partials);
+                                                                   nx, ny, nz, ndim, partials);
     else
         observables_kernel<float><<<nblocks, 256, 0, L.stream>>>((const float2*)q, (const float2*)qprev,
-                                                                  nx, ny, ndim, partials);
+                                                                  nx, ny, nz, ndim, partials);
     ++*L.counter;
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return e;

@@ -14,7 +14,7 @@ namespace qlga {
 struct PassParams {
     const void* src;
     void* dst;
-    int64_t nx, ny;
+    int64_t nx, ny, nz;    // lattice (ny = nz = 1 in 1D, nz = 1 in 2D)
     int ksteps;            // time steps fused in this launch (1 in 2D)
     int umode;             // 0: no U in this pass, 1: U before the first factor of each step,
                            // 2: U before every factor
@@ -28,7 +28,7 @@ struct Launch {
     int64_t* counter;      // incremented per kernel launched
 };
 
-// fused passes (qlga_step.cu); dir = 0 (x) or 1 (y).  `threads` / `cx` are tunables
+// fused passes (qlga_step.cu); dir = 0 (x), 1 (y) or 2 (z).  `threads` / `cx` are tunables
 // (0 = default).  Returns cudaGetLastError().
 cudaError_t launch_pass(const Launch& L, qlga_prec prec, int dir, const PassParams& P,
                         int threads, int cx);
@@ -36,15 +36,15 @@ cudaError_t launch_pass(const Launch& L, qlga_prec prec, int dir, const PassPara
 int max_ksteps(int threads);
 
 // one kernel per operator (reference path on the GPU)
-cudaError_t launch_interaction(const Launch& L, qlga_prec prec, void* q, int64_t nx, int64_t ny,
+cudaError_t launch_interaction(const Launch& L, qlga_prec prec, void* q, int64_t nsites,
                                const double g[3], const ExpTable& tab);
 cudaError_t launch_kinetic(const Launch& L, qlga_prec prec, const void* src, void* dst,
-                           int64_t nx, int64_t ny, int dir, int sigma);
+                           int64_t nx, int64_t ny, int64_t nz, int dir, int sigma);
 
 // diagnostics and state conversion (qlga_diag.cu)
 constexpr int OBS_NACC = 19;   // accumulators per block, see qlga_diag.cu
 cudaError_t launch_observables(const Launch& L, qlga_prec prec, const void* q, const void* qprev,
-                               int64_t nx, int64_t ny, int ndim, double* partials, int nblocks,
+                               int64_t nx, int64_t ny, int64_t nz, int ndim, double* partials, int nblocks,
                                double* sums);
 cudaError_t launch_vorticity(const Launch& L, qlga_prec prec, const void* q, void* omega,
                              int64_t nx, int64_t ny);
@@ -62,7 +62,7 @@ cudaError_t launch_sum_psi(const Launch& L, qlga_prec prec, const void* q, void*
 
 struct qlga_ctx {
     int ndim;
-    int64_t nx, ny;
+    int64_t nx, ny, nz;
     double c[3];
     qlga_order order;
     qlga_prec prec;

@@ -23,7 +23,11 @@ template <typename T>
 struct PassArgs {
     const typename vec2<T>::type* src;
     typename vec2<T>::type* dst;
-    int64_t nx, ny;
+    // geometry of the pass: sites along a line are `stride` elements apart and `len` many;
+    // `nx` columns (x, unit stride) and `n_outer` outer indices (`outer_stride` apart) give
+    // the lines.  x pass: len = nx, the lines are the ny*nz rows (outer_stride = nx).
+    // y pass: stride = nx, len = ny, outer = z.   z pass: stride = nx*ny, len = nz, outer = y.
+    int64_t nx, len, stride, n_outer, outer_stride, nsites;
     int ksteps, umode;
     UConst<T> uc[4];
     T out_scale;
@@ -92,29 +96,30 @@ __global__ void __launch_bounds__(NT, (NT >= 192 ? 2 : (NT >= 128 ? QLGA_MINB128
     const int c = t % CX, i = t / CX;
     const int H = 4 * P.ksteps;
     const int wout = TS - 2 * H;
-    const int64_t n = P.nx * P.ny;
+    const int64_t n = P.nsites;
 
-    int64_t x, y, spos, extent;
+    int64_t spos, idx;
+    const int64_t extent = P.len;
     bool col_ok = true;
     if (DIR == 0) {
-        const int64_t tiles = (P.nx + wout - 1) / wout;
+        const int64_t tiles = (P.len + wout - 1) / wout;
         const int64_t tile = blockIdx.x % tiles;
-        y = blockIdx.x / tiles;
+        const int64_t row = blockIdx.x / tiles;
         spos = tile * wout - H + i;
-        extent = P.nx;
-        x = pmod(spos, P.nx);
+        idx = row * P.outer_stride + pmod(spos, P.len);
     } else {
         const int64_t tiles_c = (P.nx + CX - 1) / CX;
+        const int64_t tiles_s = (P.len + wout - 1) / wout;
         const int64_t tc = blockIdx.x % tiles_c;
-        const int64_t ts = blockIdx.x / tiles_c;
-        x = tc * CX + c;
+        const int64_t rest = blockIdx.x / tiles_c;
+        const int64_t ts = rest % tiles_s;
+        const int64_t outer = rest / tiles_s;
+        int64_t x = tc * CX + c;
         col_ok = x < P.nx;
         if (!col_ok) x = P.nx - 1;
         spos = ts * wout - H + i;
-        extent = P.ny;
-        y = pmod(spos, P.ny);
+        idx = outer * P.outer_stride + pmod(spos, P.len) * P.stride + x;
     }
-    const int64_t idx = y * P.nx + x;
 
     // s.q[j][sigma]: sigma = 0,1 <-> spinor component 1,2 (the planes' own order)
     Site<T> s;
@@ -158,29 +163,32 @@ __global__ void __launch_bounds__(NT, (NT >= 192 ? 2 : (NT >= 128 ? QLGA_MINB128
 }
 
 template <typename T>
-static PassArgs<T> make_args(const PassParams& P) {
+static PassArgs<T> make_args(const PassParams& P, int dir) {
     PassArgs<T> A;
     A.src = (const typename vec2<T>::type*)P.src;
     A.dst = (typename vec2<T>::type*)P.dst;
-    A.nx = P.nx; A.ny = P.ny; A.ksteps = P.ksteps; A.umode = P.umode;
+    A.nx = P.nx; A.nsites = P.nx * P.ny * P.nz; A.ksteps = P.ksteps; A.umode = P.umode;
     for (int f = 0; f < 4; ++f) {
         A.uc[f].g0 = (T)P.g[f][0]; A.uc[f].g1 = (T)P.g[f][1]; A.uc[f].g2 = (T)P.g[f][2];
     }
     A.out_scale = (T)P.out_scale;
     A.tab = P.tab;
+    if (dir == 0)      { A.len = P.nx; A.stride = 1;           A.n_outer = P.ny * P.nz; A.outer_stride = P.nx; }
+    else if (dir == 1) { A.len = P.ny; A.stride = P.nx;        A.n_outer = P.nz;        A.outer_stride = P.nx * P.ny; }
+    else               { A.len = P.nz; A.stride = P.nx * P.ny; A.n_outer = P.ny;        A.outer_stride = P.nx; }
     return A;
 }
 
 template <typename T, int DIR, int CX, int NT>
-static cudaError_t run_pass(const Launch& L, const PassParams& P) {
+static cudaError_t run_pass(const Launch& L, const PassParams& P, int dir) {
     constexpr int TS = NT / CX;
     const int wout = TS - 8 * P.ksteps;
     if (wout <= 0) return cudaErrorInvalidValue;
+    PassArgs<T> A = make_args<T>(P, dir);
     int64_t blocks;
-    if (DIR == 0) blocks = ((P.nx + wout - 1) / wout) * P.ny;
-    else blocks = ((P.nx + CX - 1) / CX) * ((P.ny + wout - 1) / wout);
+    if (DIR == 0) blocks = ((A.len + wout - 1) / wout) * A.n_outer;
+    else blocks = ((A.nx + CX - 1) / CX) * ((A.len + wout - 1) / wout) * A.n_outer;
     if (blocks <= 0 || blocks > 2147483647LL) return cudaErrorInvalidValue;
-    PassArgs<T> A = make_args<T>(P);
     constexpr size_t smem = (size_t)4 * 5 * NT * sizeof(typename vec2<T>::type);   // sF[2], sB[2]
     static bool configured = false;            // per instantiation; more than 48 KB needs the opt-in
     if (!configured) {
@@ -201,11 +209,11 @@ static cudaError_t launch_pass_t(const Launch& L, int dir, const PassParams& P, 
     if (dir == 0) {
         if (threads == 0) threads = 128;
         switch (threads) {
-            case 64: return run_pass<T, 0, 1, 64>(L, P);
-            case 96: return run_pass<T, 0, 1, 96>(L, P);
-            case 128: return run_pass<T, 0, 1, 128>(L, P);
-            case 192: return run_pass<T, 0, 1, 192>(L, P);
-            case 256: return run_pass<T, 0, 1, 256>(L, P);
+            case 64: return run_pass<T, 0, 1, 64>(L, P, dir);
+            case 96: return run_pass<T, 0, 1, 96>(L, P, dir);
+            case 128: return run_pass<T, 0, 1, 128>(L, P, dir);
+            case 192: return run_pass<T, 0, 1, 192>(L, P, dir);
+            case 256: return run_pass<T, 0, 1, 256>(L, P, dir);
             default: return cudaErrorInvalidValue;
         }
     }
@@ -215,15 +223,15 @@ static cudaError_t launch_pass_t(const Launch& L, int dir, const PassParams& P, 
     if (cxw == 0) cxw = (sizeof(T) == 8) ? 1 : 4;
     if (threads == 0) threads = (cxw <= 2) ? 128 : 256;
     switch (cxw * 1000 + threads) {
-        case 1064: return run_pass<T, 1, 1, 64>(L, P);
-        case 1096: return run_pass<T, 1, 1, 96>(L, P);
-        case 1128: return run_pass<T, 1, 1, 128>(L, P);
-        case 1192: return run_pass<T, 1, 1, 192>(L, P);
-        case 2128: return run_pass<T, 1, 2, 128>(L, P);
-        case 2192: return run_pass<T, 1, 2, 192>(L, P);
-        case 2256: return run_pass<T, 1, 2, 256>(L, P);
-        case 4256: return run_pass<T, 1, 4, 256>(L, P);
-        case 8256: return run_pass<T, 1, 8, 256>(L, P);
+        case 1064: return run_pass<T, 1, 1, 64>(L, P, dir);
+        case 1096: return run_pass<T, 1, 1, 96>(L, P, dir);
+        case 1128: return run_pass<T, 1, 1, 128>(L, P, dir);
+        case 1192: return run_pass<T, 1, 1, 192>(L, P, dir);
+        case 2128: return run_pass<T, 1, 2, 128>(L, P, dir);
+        case 2192: return run_pass<T, 1, 2, 192>(L, P, dir);
+        case 2256: return run_pass<T, 1, 2, 256>(L, P, dir);
+        case 4256: return run_pass<T, 1, 4, 256>(L, P, dir);
+        case 8256: return run_pass<T, 1, 8, 256>(L, P, dir);
         default: return cudaErrorInvalidValue;
     }
 }
@@ -271,19 +279,22 @@ __global__ void __launch_bounds__(128) interaction_kernel(typename vec2<T>::type
 template <typename T>
 __global__ void __launch_bounds__(128) kinetic_kernel(const typename vec2<T>::type* src,
                                                       typename vec2<T>::type* dst,
-                                                      int64_t nx, int64_t ny, int dir, int sigma) {
+                                                      int64_t nx, int64_t ny, int64_t nz, int dir, int sigma) {
     using V = typename vec2<T>::type;
-    const int64_t n = nx * ny;
+    const int64_t n = nx * ny * nz;
     const int64_t r = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (r >= n) return;
-    const int64_t x = r % nx, y = r / nx;
+    const int64_t x = r % nx, y = (r / nx) % ny, z = r / (nx * ny);
     int64_t rm, rp;
     if (dir == 0) {
-        rm = y * nx + (x == 0 ? nx - 1 : x - 1);
-        rp = y * nx + (x == nx - 1 ? 0 : x + 1);
+        rm = r - x + (x == 0 ? nx - 1 : x - 1);
+        rp = r - x + (x == nx - 1 ? 0 : x + 1);
+    } else if (dir == 1) {
+        rm = r + ((y == 0 ? ny - 1 : y - 1) - y) * nx;
+        rp = r + ((y == ny - 1 ? 0 : y + 1) - y) * nx;
     } else {
-        rm = (y == 0 ? ny - 1 : y - 1) * nx + x;
-        rp = (y == ny - 1 ? 0 : y + 1) * nx + x;
+        rm = r + ((z == 0 ? nz - 1 : z - 1) - z) * nx * ny;
+        rp = r + ((z == nz - 1 ? 0 : z + 1) - z) * nx * ny;
     }
     const T half = (T)0.5;
     for (int j = 0; j < 5; ++j) {
@@ -301,9 +312,8 @@ __global__ void __launch_bounds__(128) kinetic_kernel(const typename vec2<T>::ty
     }
 }
 
-cudaError_t launch_interaction(const Launch& L, qlga_prec prec, void* q, int64_t nx, int64_t ny,
+cudaError_t launch_interaction(const Launch& L, qlga_prec prec, void* q, int64_t n,
                                const double g[3], const ExpTable& tab) {
-    const int64_t n = nx * ny;
     const unsigned blocks = (unsigned)((n + 127) / 128);
     if (prec == QLGA_F64) {
         UConst<double> uc{g[0], g[1], g[2]};
@@ -317,13 +327,13 @@ cudaError_t launch_interaction(const Launch& L, qlga_prec prec, void* q, int64_t
 }
 
 cudaError_t launch_kinetic(const Launch& L, qlga_prec prec, const void* src, void* dst,
-                           int64_t nx, int64_t ny, int dir, int sigma) {
-    const int64_t n = nx * ny;
+                           int64_t nx, int64_t ny, int64_t nz, int dir, int sigma) {
+    const int64_t n = nx * ny * nz;
     const unsigned blocks = (unsigned)((n + 127) / 128);
     if (prec == QLGA_F64)
-        kinetic_kernel<double><<<blocks, 128, 0, L.stream>>>((const double2*)src, (double2*)dst, nx, ny, dir, sigma);
+        kinetic_kernel<double><<<blocks, 128, 0, L.stream>>>((const double2*)src, (double2*)dst, nx, ny, nz, dir, sigma);
     else
-        kinetic_kernel<float><<<blocks, 128, 0, L.stream>>>((const float2*)src, (float2*)dst, nx, ny, dir, sigma);
+        kinetic_kernel<float><<<blocks, 128, 0, L.stream>>>((const float2*)src, (float2*)dst, nx, ny, nz, dir, sigma);
     ++*L.counter;
     return cudaGetLastError();
 }

@@ -108,13 +108,21 @@ def exp_polynomial(tol_log2, p):
     return th.value, b0.value, list(r)
 
 
+def _dims3(ndim, dims):
+    dims = tuple(int(v) for v in dims)
+    if int(ndim) == 3:
+        return (dims + (0, 0, 0))[:3]          # a missing extent is reported by the library (EINVAL)
+    return (dims[0], dims[1] if len(dims) > 1 else 1, 1)
+
+
 def state_bytes(ndim, dims, prec) -> int:
-    d = (ctypes.c_int64 * 2)(int(dims[0]), int(dims[1]))
+    d = (ctypes.c_int64 * 3)(*_dims3(ndim, dims))
     return int(_lib.qlga_state_bytes(int(ndim), d, int(prec)))
 
 
 class Qlga:
-    """One lattice on one GPU.  dims = (Nx, Ny) (Ny = 1 in 1D); couplings = (c0, c1, c2)
+    """One lattice on one GPU.  dims = (Nx, Ny) (Ny = 1 in 1D) or (Nx, Ny, Nz) in 3D; arrays
+    are q[5][2][Ny][Nx] / psi[5][Ny][Nx] (3D: [..][Nz][Ny][Nx]); couplings = (c0, c1, c2)
     = the paper's (g0, g1, g2); order "plain" (eq. 108) or "interleaved" (eq. 112);
     precision "f64" or "f32".  `keep_previous=True` allocates the third buffer that
     eq. (85)'s energy needs in 2D."""
@@ -126,22 +134,23 @@ class Qlga:
             raise RuntimeError("qlga needs a CUDA device (B200, sm_100a); there is no CPU fallback")
         self.torch = torch
         self.ndim = int(ndim)
-        self.nx, self.ny = int(dims[0]), int(dims[1])
+        self.nx, self.ny, self.nz = _dims3(ndim, dims)
+        self.lat = (self.ny, self.nx) if self.ndim < 3 else (self.nz, self.ny, self.nx)
         self.prec = QLGA_F64 if precision in ("f64", "fp64", "double") else QLGA_F32
         self.order = QLGA_INTERLEAVED if order in ("interleaved", 1) else QLGA_PLAIN
         self.device = torch.device(device)
         self.rdtype = torch.float64 if self.prec == QLGA_F64 else torch.float32
         self.np_cdtype = np.complex128 if self.prec == QLGA_F64 else np.complex64
         self.np_rdtype = np.float64 if self.prec == QLGA_F64 else np.float32
-        nbytes = state_bytes(self.ndim, (self.nx, self.ny), self.prec)
+        nbytes = state_bytes(self.ndim, (self.nx, self.ny, self.nz), self.prec)
         if nbytes == 0:
             raise QlgaError(QLGA_EINVAL, "bad ndim/dims")
         nreal = nbytes // (8 if self.prec == QLGA_F64 else 4)
         with torch.cuda.device(self.device):
-            nbuf = 3 if (keep_previous and self.ndim == 2) else 2
+            nbuf = 3 if (keep_previous and self.ndim >= 2) else 2
             self.bufs = [torch.empty(nreal, dtype=self.rdtype, device=self.device) for _ in range(nbuf)]
             self.stream = stream if stream is not None else torch.cuda.current_stream(self.device)
-            dims_c = (ctypes.c_int64 * 2)(self.nx, self.ny)
+            dims_c = (ctypes.c_int64 * 3)(self.nx, self.ny, self.nz)
             ctx = ctypes.c_void_p()
             c0, c1, c2 = (float(v) for v in couplings)
             st = _lib.qlga_init(ctypes.byref(ctx), self.ndim, dims_c, c0, c1, c2, self.order, self.prec,
@@ -183,27 +192,27 @@ class Qlga:
     def set_state_psi(self, psi):
         if isinstance(psi, np.ndarray):
             psi = np.ascontiguousarray(psi, dtype=self.np_cdtype)
-            assert psi.shape == (5, self.ny, self.nx), psi.shape
+            assert psi.shape == (5,) + self.lat, psi.shape
         p, dev = self._ptr(psi)
         self._check(_lib.qlga_set_state_psi(self.ctx, p, dev))
 
     def set_state_q(self, q):
         if isinstance(q, np.ndarray):
             q = np.ascontiguousarray(q, dtype=self.np_cdtype)
-            assert q.shape == (5, 2, self.ny, self.nx), q.shape
+            assert q.shape == (5, 2) + self.lat, q.shape
         p, dev = self._ptr(q)
         self._check(_lib.qlga_set_state_q(self.ctx, p, dev))
 
     def get_state_q(self, out=None):
         if out is None:
-            out = np.empty((5, 2, self.ny, self.nx), dtype=self.np_cdtype)
+            out = np.empty((5, 2) + self.lat, dtype=self.np_cdtype)
         p, dev = self._ptr(out)
         self._check(_lib.qlga_get_state_q(self.ctx, p, dev))
         return out
 
     def get_state_psi(self, out=None):
         if out is None:
-            out = np.empty((5, self.ny, self.nx), dtype=self.np_cdtype)
+            out = np.empty((5,) + self.lat, dtype=self.np_cdtype)
         p, dev = self._ptr(out)
         self._check(_lib.qlga_get_state_psi(self.ctx, p, dev))
         return out
@@ -230,7 +239,7 @@ class Qlga:
 
     def density(self, out=None):
         if out is None:
-            out = np.empty((self.ny, self.nx), dtype=self.np_rdtype)
+            out = np.empty(self.lat, dtype=self.np_rdtype)
         p, dev = self._ptr(out)
         self._check(_lib.qlga_density(self.ctx, p, dev))
         return out
@@ -239,7 +248,7 @@ class Qlga:
         """eq. (115): sum_r (rho_ref - rho)^2 against a reference density (numpy or torch)."""
         if isinstance(rho_ref, np.ndarray):
             rho_ref = np.ascontiguousarray(rho_ref, dtype=self.np_rdtype)
-            assert rho_ref.shape == (self.ny, self.nx)
+            assert rho_ref.shape == self.lat
         p, dev = self._ptr(rho_ref)
         eps = ctypes.c_double()
         self._check(_lib.qlga_density_l2_error(self.ctx, p, dev, ctypes.byref(eps)))

@@ -34,7 +34,9 @@ def test_state_bytes_and_argument_checks_without_gpu():
     assert qlga.state_bytes(2, (8192, 8192), qlga.QLGA_F64) == 10 * 8192 * 8192 * 16   # ~10.7 GB per buffer
     assert qlga.state_bytes(1, (1024, 1), qlga.QLGA_F32) == 10 * 1024 * 8
     assert qlga.state_bytes(1, (1024, 2), qlga.QLGA_F64) == 0
-    assert qlga.state_bytes(3, (8, 8), qlga.QLGA_F64) == 0
+    assert qlga.state_bytes(3, (8, 8), qlga.QLGA_F64) == 0            # 3D needs three extents
+    assert qlga.state_bytes(3, (8, 4, 2), qlga.QLGA_F64) == 10 * 64 * 16
+    assert qlga.state_bytes(4, (8, 8, 8), qlga.QLGA_F64) == 0
     assert qlga.state_bytes(2, (0, 8), qlga.QLGA_F64) == 0
 
 

@@ -25,8 +25,8 @@ def qlga():
 
 
 def run_gpu(qlga, q0, ndim, couplings, order, steps, precision="f64", options=(), keep_previous=False):
-    ny, nx = q0.shape[2], q0.shape[3]
-    sim = qlga.Qlga(ndim, (nx, ny), couplings, order=order, precision=precision, keep_previous=keep_previous)
+    dims = tuple(reversed(q0.shape[2:]))                   # (Nx, Ny) or (Nx, Ny, Nz)
+    sim = qlga.Qlga(ndim, dims, couplings, order=order, precision=precision, keep_previous=keep_previous)
     for k, v in options:
         sim.set_option(k, v)
     sim.set_state_q(q0)
@@ -415,3 +415,45 @@ def test_vortices_match_oracle_winding(qlga, oracle):
         sim.vortices()
     assert e.value.status == qlga.QLGA_EUNSUP
     sim.close()
+
+
+# ---------------------------------------------------------------------------
+# the 3D lattice (12 factors, U^(1/12))
+# ---------------------------------------------------------------------------
+@pytest.mark.parametrize("order", ["plain", "interleaved"])
+@pytest.mark.parametrize("dims", [(1, 1, 1), (5, 3, 2), (130, 5, 3), (9, 125, 4), (6, 7, 131), (40, 33, 21)])
+def test_3d_random_state_matches_oracle(qlga, oracle, order, dims):
+    c = (0.8, -0.25, 0.4)
+    q0 = inputs.random_spinor_state(dims, seed=3 + dims[0], amplitude=0.3)
+    ref = oracle.step(q0, 3, c, ORDERS[order], 2)
+    out = run_gpu(qlga, q0, 3, c, order, 2)
+    assert rel_l2(out, ref) < TOL64
+    a = run_gpu(qlga, q0, 3, c, order, 2, options=[(qlga.OPT_PATH, 1)])
+    assert rel_l2(a, ref) < TOL64
+
+
+def test_3d_fp32_observables_density_and_previous_state(qlga, oracle):
+    c = (1.0, 0.3, -0.1)
+    dims = (36, 20, 17)
+    q0 = inputs.random_spinor_state(dims, seed=8, amplitude=0.2)
+    q32 = q0.astype(np.complex64)
+    ref32 = oracle.step(q32.astype(np.complex128), 3, c, 1, 5)
+    assert rel_l2(run_gpu(qlga, q32, 3, c, "interleaved", 5, precision="f32"), ref32) < TOL32
+    for keep in (True, False):
+        sim = qlga.Qlga(3, dims, c, order="interleaved", keep_previous=keep)
+        sim.set_state_q(q0)
+        sim.step(3)
+        q3 = sim.get_state_q()
+        ob = sim.observables()
+        ref = oracle.observables(q3, 3, c, qprev=oracle.step(q0, 3, c, 1, 2))
+        for k, v in ref.items():
+            if k.startswith("e_dt"):
+                assert (abs(ob[k] - v) < 1e-10) if keep else np.isnan(ob[k])
+            else:
+                assert abs(ob[k] - v) <= 1e-11 * max(1.0, abs(v)), k
+        assert np.abs(sim.density() - oracle.density(q3)).max() < 1e-13
+        assert np.array_equal(sim.get_state_psi(), q3[:, 0] + q3[:, 1])
+        with pytest.raises(qlga.QlgaError) as e:
+            sim.vorticity()
+        assert e.value.status == qlga.QLGA_EUNSUP
+        sim.close()
