@@ -39,6 +39,7 @@ WORKLOADS = {
     "cfg3": dict(ndim=1, gen=lambda L: inputs.config3(L=L or (1 << 22)), L=1 << 22),
     "cfg4": dict(ndim=2, gen=lambda L: inputs.config4(L=L or 2048), L=2048),
     "cfg5": dict(ndim=2, gen=lambda L: inputs.config5(L=L or 8192), L=8192),
+    "cfg3d": dict(ndim=3, gen=lambda L: inputs.config3d(L=L or 256), L=256),   # SURVEY 8(f) row 3, not a BASELINE config
 }
 
 
@@ -187,8 +188,12 @@ def expected_degree(w, ndim, order, precision):
 # ---------------------------------------------------------------------------
 def oracle_sample(w, ndim, order, target_seconds):
     """A periodic crop of the workload's lattice sized for ~target_seconds of oracle time."""
-    nx, ny = w.dims
-    if ndim == 2:
+    nx, ny = w.dims[0], w.dims[1]
+    if ndim == 3:
+        edge = min(nx, 40)
+        o = nx // 2 - edge // 2
+        psi = w.psi[:, o:o + edge, o:o + edge, o:o + edge]
+    elif ndim == 2:
         edge = min(nx, 256)
         y0, x0 = ny // 2 - edge // 2, nx // 2 - edge // 2
         psi = w.psi[:, y0:y0 + edge, x0:x0 + edge]
@@ -204,7 +209,7 @@ def time_oracle(w, ndim, order, target_seconds):
     from oracle.qlga_oracle import Oracle     # test infrastructure: allowed here (cpu_baseline / reference arm)
     orc = Oracle("double")
     q, edge = oracle_sample(w, ndim, order, target_seconds)
-    sites = q.shape[2] * q.shape[3]
+    sites = int(np.prod(q.shape[2:]))
     o = 1 if order == "interleaved" else 0
     t0 = time.perf_counter()
     q = orc.step(q, ndim, w.couplings, o, 1)
@@ -214,7 +219,7 @@ def time_oracle(w, ndim, order, target_seconds):
     orc.step(q, ndim, w.couplings, o, nsteps)
     dt = time.perf_counter() - t0
     rate = sites * nsteps / dt
-    sample = (f"periodic {edge}x{edge} crop" if ndim == 2 else f"periodic {edge}-site crop") + \
+    sample = (f"periodic {'x'.join([str(edge)] * ndim)} crop" if ndim >= 2 else f"periodic {edge}-site crop") + \
              f" of the workload's input, {nsteps} time steps, {dt:.1f} s"
     return rate, sample, sites, nsteps
 
@@ -224,7 +229,7 @@ def run_reference(args, w, ndim, config):
     from oracle.qlga_oracle import Oracle
     orc = Oracle("double")
     q, edge = oracle_sample(w, ndim, args.order, 0)
-    sites = q.shape[2] * q.shape[3]
+    sites = int(np.prod(q.shape[2:]))
     o = 1 if args.order == "interleaved" else 0
     t0 = time.perf_counter()
     q = orc.step(q, ndim, w.couplings, o, 1)
@@ -238,7 +243,7 @@ def run_reference(args, w, ndim, config):
         q = orc.step(q, ndim, w.couplings, o, inner)
     dt = time.perf_counter() - t0
     val = sites * inner * args.steps / dt / 1e9
-    sample = (f"periodic {edge}x{edge} crop" if ndim == 2 else f"periodic {edge}-site crop") + \
+    sample = (f"periodic {'x'.join([str(edge)] * ndim)} crop" if ndim >= 2 else f"periodic {edge}-site crop") + \
              f" of the workload's input, {inner} time steps per bench step"
     line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus,
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": dt / args.steps * 1e3,
@@ -284,13 +289,16 @@ def main():
     if args.impl == "reference" and rank != 0:
         return                                              # rank 0 alone runs the oracle arm
     w = wl["gen"](args.lattice)
-    nx, ny = w.dims
-    sites = nx * ny
+    nx, ny = w.dims[0], w.dims[1]
+    sites = int(np.prod(w.dims))
+    lat = tuple(reversed(w.dims)) if ndim == 3 else (ny, nx)        # array shape of one plane
+    cfg_tag = (f"BASELINE.json configs[{int(args.workload[3]) - 1}]" if args.workload[3:].isdigit()
+               else "SURVEY.md 8(f) row 3, not a BASELINE.json config")
     inner = args.inner or max(1, min(1000, int(6.0e8 / sites)))   # ~0.5 s of GPU work per bench step
-    config = {"workload": f"{w.name} (BASELINE.json configs[{int(args.workload[3]) - 1}]): "
-                          f"{'2D' if ndim == 2 else '1D'} periodic {nx}x{ny}, {args.precision}, "
+    config = {"workload": f"{w.name} ({cfg_tag}): "
+                          f"{ndim}D periodic {'x'.join(str(v) for v in w.dims[:max(2, ndim)])}, {args.precision}, "
                           f"{args.order} ordering (eq. {'112' if args.order == 'interleaved' else '108'})",
-              "lattice": [nx, ny], "precision": args.precision, "order": args.order,
+              "lattice": list(w.dims), "precision": args.precision, "order": args.order,
               "couplings": list(w.couplings), "time_steps_per_bench_step": inner,
               "per_bench_step": f"{inner} time steps + 1 observables reduction" + (" + 1 vorticity map" if ndim == 2 else ""),
               "l2_policy": "state (%.1f GB per buffer) larger than the 126 MB L2" % (sites * 160 / 1e9 * (1 if args.precision == 'f64' else 0.5))
@@ -318,14 +326,14 @@ def main():
 
     cdt = torch.complex128 if args.precision == "f64" else torch.complex64
     # host input in pinned memory: q1 = q2 = psi/2 (reading R6)
-    q_host = torch.empty((5, 2, ny, nx), dtype=cdt, pin_memory=True)
+    q_host = torch.empty((5, 2) + lat, dtype=cdt, pin_memory=True)
     half = torch.from_numpy(w.psi / 2).to(cdt)
     q_host[:, 0] = half
     q_host[:, 1] = half
     del half
     out_host = torch.empty_like(q_host, pin_memory=True) if not args.no_e2e else None
 
-    sim = qlga.Qlga(ndim, (nx, ny), w.couplings, order=args.order, precision=args.precision, device=dev)
+    sim = qlga.Qlga(ndim, w.dims, w.couplings, order=args.order, precision=args.precision, device=dev)
     if args.tile_y:
         sim.set_option(qlga.OPT_TILE_Y, args.tile_y)
     if args.threads_x:
@@ -413,7 +421,8 @@ def main():
         dms, dn = kinds[dom]
         per_launch_ms = dms / dn
         # a pass launch advances every site by 1/ndim of a time step (times the fused steps in 1D)
-        units = sites * inner * args.steps / (ndim * dn)      # site-updates per launch
+        per_step = 1 if dom == "x_pass" else max(1, ndim - 1)  # the y_pass timer covers the y and z passes
+        units = sites * inner * args.steps * per_step / (ndim * dn)      # site-updates per launch
         deg = expected_degree(w, ndim, args.order, args.precision)
         fpi = fp_instr_per_site_update(ndim, args.order, deg)
         lanes = 64 if args.precision == "f64" else 128       # FP64 / FP32 FMA lanes per SM per clock

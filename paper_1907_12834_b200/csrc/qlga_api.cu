@@ -421,7 +421,11 @@ static qlga_status step_fused(qlga_ctx* c, int64_t nsteps) {
             // U is the rightmost operator of the plain step: it rides on the first pass
             P.umode = inter ? 2 : (d == c->ndim - 1 ? 1 : 0);
             prof_mark(c, d == 0 ? 0 : 1);
-            CU(c, launch_pass(L, c->prec, d, P, d == 0 ? c->threads_x : c->threads_y, d == 0 ? 1 : c->tile_y));
+            // strided passes: measured defaults -- 2D: one column per CTA; 3D (fp64): two columns,
+            // i.e. whole 32-byte sectors, which the page-crossing z lines need (+12 % at 512^3)
+            int cxw = c->tile_y, thr = c->threads_y;
+            if (d > 0 && cxw == 0 && c->ndim == 3 && c->prec == QLGA_F64) { cxw = 2; if (thr == 0) thr = 128; }
+            CU(c, launch_pass(L, c->prec, d, P, d == 0 ? c->threads_x : thr, d == 0 ? 1 : cxw));
             src = dst;
         }
         c->prev = (third >= 0) ? start : -1;

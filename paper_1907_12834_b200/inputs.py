@@ -170,6 +170,26 @@ def config5(L=8192, core=12.0, kick=0.03, sigma=1e-3, spacing=96.0, offset=256.0
     return Workload("cfg5_dipoles_2d", 2, (L, L), (c0, c1, c2), 5000, psi)
 
 
+def config3d(L=256, core=12.0, kick=0.03, sigma=1e-3, spacing=48.0, seed=None):
+    """3D workload for SURVEY.md section 8(f) row 3 (the paper quotes "a three dimensional cube of
+    512 sites" as capacity, and no 3D run): config 5's recipe extruded along z --
+    a straight Pade vortex-antivortex line pair in m_f=+1 kicked along y, uniform background in
+    the other channels, seeded phase noise.  psi: (5, L, L, L)."""
+    c0, c1, c2 = 1.0, 0.3, -0.1
+    a = 1.0 / core
+    rng = np.random.default_rng(seed_for(6) if seed is None else seed)
+    X, Y = _grid(L, L)
+    h = spacing / 2.0
+    D = (vortex_factor(X, Y, L / 2 + h, L / 2, a, +1) * vortex_factor(X, Y, L / 2 - h, L / 2, a, -1))
+    plane = a * D * np.exp(1j * kick * Y)
+    psi = np.empty((5, L, L, L), dtype=np.complex128)
+    psi[:] = a
+    psi[j_of_m(1)] = plane[None, :, :]
+    for j in range(5):
+        psi[j] *= np.exp(1j * sigma * rng.standard_normal((L, L, L)))
+    return Workload("cfg3d_vortex_lines", 3, (L, L, L), (c0, c1, c2), 1000, psi)
+
+
 CONFIGS = {1: config1, 2: config2, 3: config3, 4: config4, 5: config5}
 
 
