@@ -46,11 +46,13 @@ __device__ __forceinline__ int64_t pmod(int64_t a, int64_t n) {
 // ([j][thread]: conflict free), double buffered so that one barrier per factor
 // suffices.  (A warp-shuffle exchange was measured first: SHFL.32 issues at 6 cycles
 // per warp on sm_100a and a factor needs 40 of them.)
-template <typename T, int CX, int NT, int SIGMA>
+template <typename T, int CX, int NT, int SIGMA, bool HASU>
 __device__ __forceinline__ void factor(Site<T>& s, const PassArgs<T>& P, int f, int t, int& pb,
                                        typename vec2<T>::type (*sF)[5][NT], typename vec2<T>::type (*sB)[5][NT]) {
     using V = typename vec2<T>::type;
-    if (P.umode == 2 || (P.umode == 1 && f == 0)) interaction<T>(s, P.uc[f], P.tab);
+    if constexpr (HASU) {
+        if (P.umode == 2 || (P.umode == 1 && f == 0)) interaction<T>(s, P.uc[f], P.tab);
+    }
 
     cx<T> Fw[5], Bw[5], Fp[5], Bn[5];
     kin_messages<T>(s, SIGMA, Fw, Bw);
@@ -81,8 +83,13 @@ __device__ __forceinline__ void factor(Site<T>& s, const PassArgs<T>& P, int f, 
 #define QLGA_MINB128 3
 #endif
 
-template <typename T, int DIR, int CX, int NT>
-__global__ void __launch_bounds__(NT, (NT >= 192 ? 2 : (NT >= 128 ? QLGA_MINB128 : (NT >= 96 ? 4 : 6)))) pass_kernel(const __grid_constant__ PassArgs<T> P) {
+// HASU = false: a pass without any interaction (the plain ordering's later passes): the same
+// kernel minus the interaction code, a third of the registers, so more CTAs per SM keep the
+// HBM pipe full (this pass is memory-bound).
+template <typename T, int DIR, int CX, int NT, bool HASU>
+__global__ void __launch_bounds__(NT, (HASU ? (NT >= 192 ? 2 : (NT >= 128 ? QLGA_MINB128 : (NT >= 96 ? 4 : 6)))
+                                            : (NT >= 192 ? 2 : 4)))
+pass_kernel(const __grid_constant__ PassArgs<T> P) {
     using V = typename vec2<T>::type;
     constexpr int TS = NT / CX;              // sites per line handled by the CTA
     static_assert(NT % 32 == 0 && 32 % CX == 0 && CX < 32, "bad tile");
@@ -138,10 +145,10 @@ __global__ void __launch_bounds__(NT, (NT >= 192 ? 2 : (NT >= 128 ? QLGA_MINB128
         // one per streamed component, so that no register ever changes role
 #pragma unroll 1
         for (int f = 0; f < 2; ++f)
-            factor<T, CX, NT, 1>(s, P, f, t, pb, sF, sB);
+            factor<T, CX, NT, 1, HASU>(s, P, f, t, pb, sF, sB);
 #pragma unroll 1
         for (int f = 2; f < 4; ++f)
-            factor<T, CX, NT, 0>(s, P, f, t, pb, sF, sB);
+            factor<T, CX, NT, 0, HASU>(s, P, f, t, pb, sF, sB);
         // undo the four deferred halvings (exact)
 #pragma unroll
         for (int j = 0; j < 5; ++j) {
@@ -192,12 +199,16 @@ static cudaError_t run_pass(const Launch& L, const PassParams& P, int dir) {
     constexpr size_t smem = (size_t)4 * 5 * NT * sizeof(typename vec2<T>::type);   // sF[2], sB[2]
     static bool configured = false;            // per instantiation; more than 48 KB needs the opt-in
     if (!configured) {
-        cudaError_t e = cudaFuncSetAttribute(pass_kernel<T, DIR, CX, NT>,
+        cudaError_t e = cudaFuncSetAttribute(pass_kernel<T, DIR, CX, NT, true>,
                                              cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e == cudaSuccess)
+            e = cudaFuncSetAttribute(pass_kernel<T, DIR, CX, NT, false>,
+                                     cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;
         configured = true;
     }
-    pass_kernel<T, DIR, CX, NT><<<(unsigned)blocks, NT, smem, L.stream>>>(A);
+    if (P.umode != 0) pass_kernel<T, DIR, CX, NT, true><<<(unsigned)blocks, NT, smem, L.stream>>>(A);
+    else pass_kernel<T, DIR, CX, NT, false><<<(unsigned)blocks, NT, smem, L.stream>>>(A);
     ++*L.counter;
     return cudaGetLastError();
 }
