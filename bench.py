@@ -153,10 +153,12 @@ def bytes_per_site_update(precision):
 def fp_instr_per_site_update(ndim, order, degree):
     """FP instructions (FMA/ADD/MUL, one per lane) per site-update of the fused step,
     counted from qlga_math.cuh: one U of polynomial degree p
-    costs about 140 + 200 p, one kinetic factor 40, the final scaling 20 per pass."""
+    costs about 200 + 156 p (densities and spin 52, spin gauge 59, scalar phase 49, output 40;
+    per Horner stage and spinor vector 68 + 10), one kinetic factor 40, the final scaling 20
+    per pass."""
     n_fac = 4 * ndim
     n_u = n_fac if order == "interleaved" else 1
-    return n_u * (140.0 + 200.0 * degree) + n_fac * 40.0 + 20.0 * ndim
+    return n_u * (200.0 + 156.0 * degree) + n_fac * 40.0 + 20.0 * ndim
 
 
 def expected_degree(w, ndim, order, precision):

@@ -93,6 +93,18 @@ static void build_exp_table(ExpTable& tab, int tol_log2) {
     }
     const double top = tab.thr[QLGA_PMAX - 1];
     tab.theta_split = (float)(top < 0.5 ? top : 0.5);
+    // Taylor coefficients of the scalar phase (qlga_math.cuh, sincos_small)
+    long double f = 1.0L;                                  // running factorial
+    for (int k = 0; k < 7; ++k) {
+        f *= (long double)(2 * k + 1) * (long double)(2 * k + 2);          // (2k+2)!
+        const long double sg = (k % 2 == 0) ? -1.0L : 1.0L;
+        tab.sc.c[k] = (double)(sg / f);
+        tab.sc.cf[k] = (float)tab.sc.c[k];
+        if (k < 6) {
+            tab.sc.s[k] = (double)(sg / (f * (long double)(2 * k + 3)));    // (2k+3)!
+            tab.sc.sf[k] = (float)tab.sc.s[k];
+        }
+    }
 }
 
 // Introspection of the polynomial table (host only, no GPU): used by the CPU tests.

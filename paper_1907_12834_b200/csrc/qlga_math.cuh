@@ -40,26 +40,65 @@ template <typename T> __device__ __forceinline__ cx<T> cfma_conj(cx<T> a, cx<T> 
     return acc;
 }
 
+// acc - conj(a)*b
+template <typename T> __device__ __forceinline__ cx<T> cfnma_conj(cx<T> a, cx<T> b, cx<T> acc) {
+    acc.re = fma(-a.re, b.re, acc.re); acc.re = fma(-a.im, b.im, acc.re);
+    acc.im = fma(-a.re, b.im, acc.im); acc.im = fma(a.im, b.re, acc.im);
+    return acc;
+}
+// a * conj(b)
+template <typename T> __device__ __forceinline__ cx<T> cmul_conj(cx<T> a, cx<T> b) {
+    return mk<T>(fma(a.re, b.re, a.im * b.im), fma(a.im, b.re, -(a.re * b.im)));
+}
+
+// 1/sqrt(x) for x >= 1e-36: hardware seed (MUFU.RSQ64H / MUFU.RSQ) + Newton steps, no
+// special-case branches (the caller excludes zero and subnormal arguments)
+__device__ __forceinline__ double rsqrt_pos(double x) {
+    double y;
+    asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+    const double hx = 0.5 * x;
+#pragma unroll
+    for (int it = 0; it < 2; ++it) {                 // 2^-20 -> 2^-40 -> 2^-80
+        const double h = fma(-hx * y, y, 0.5);       // (1 - x y^2) / 2
+        y = fma(y, h, y);
+    }
+    return y;
+}
+__device__ __forceinline__ float rsqrt_pos(float x) {
+    float y = rsqrtf(x);
+    const float h = fmaf(-0.5f * x * y, y, 0.5f);
+    return fmaf(y, h, y);
+}
+
+// Taylor coefficients of the scalar-phase sin/cos, kept in the kernel-parameter constant bank
+// so that every DFMA/FFMA takes its coefficient as a constant operand (as immediates each
+// fp64 coefficient costs two register moves per use).
+//   cos x = 1 + z (c[0] + z (c[1] + ... + z c[6])),        c[k] = (-1)^(k+1) / (2k+2)!
+//   sin x = x + x z (s[0] + z (s[1] + ... + z s[5])),      s[k] = (-1)^(k+1) / (2k+3)!,  z = x^2
+struct SinCosTable {
+    double c[7], s[6];
+    float cf[7], sf[6];
+};
+__device__ __forceinline__ const double* sc_cos(const SinCosTable& t, double) { return t.c; }
+__device__ __forceinline__ const double* sc_sin(const SinCosTable& t, double) { return t.s; }
+__device__ __forceinline__ const float* sc_cos(const SinCosTable& t, float) { return t.cf; }
+__device__ __forceinline__ const float* sc_sin(const SinCosTable& t, float) { return t.sf; }
+
 // sin/cos of the scalar interaction phase for |x| <= 2^-4 (always the case at the
 // paper's scaled amplitudes): Taylor polynomials in x^2 to x^13 / x^14, remainder
 // < 2^-80, branch free so that the chain interleaves with the spin-density arithmetic.
 template <typename T>
-__device__ __forceinline__ void sincos_small(T x, T* s, T* c) {
+__device__ __forceinline__ void sincos_small(T x, const SinCosTable& t, T* s, T* c) {
     const T z = x * x;
-    T ps = fma(z, (T)(-1.0 / 156.0), (T)1);
-    T pc = fma(z, (T)(-1.0 / 182.0), (T)1);
-    ps = fma(z * (T)(-1.0 / 110.0), ps, (T)1);
-    pc = fma(z * (T)(-1.0 / 132.0), pc, (T)1);
-    ps = fma(z * (T)(-1.0 / 72.0), ps, (T)1);
-    pc = fma(z * (T)(-1.0 / 90.0), pc, (T)1);
-    ps = fma(z * (T)(-1.0 / 42.0), ps, (T)1);
-    pc = fma(z * (T)(-1.0 / 56.0), pc, (T)1);
-    ps = fma(z * (T)(-1.0 / 20.0), ps, (T)1);
-    pc = fma(z * (T)(-1.0 / 30.0), pc, (T)1);
-    ps = fma(z * (T)(-1.0 / 6.0), ps, (T)1);
-    pc = fma(z * (T)(-1.0 / 12.0), pc, (T)1);
-    *s = x * ps;
-    *c = fma(z * (T)-0.5, pc, (T)1);
+    const T* cc = sc_cos(t, x);
+    const T* cs = sc_sin(t, x);
+    T pc = cc[6], ps = cs[5];
+#pragma unroll
+    for (int k = 5; k >= 0; --k) pc = fma(z, pc, cc[k]);
+#pragma unroll
+    for (int k = 4; k >= 0; --k) ps = fma(z, ps, cs[k]);
+    *c = fma(z, pc, (T)1);
+    *s = fma(x * z, ps, x);
 }
 __device__ __forceinline__ void sincos_lib(double x, double* s, double* c) { sincos(x, s, c); }
 __device__ __forceinline__ void sincos_lib(float x, float* s, float* c) { sincosf(x, s, c); }
@@ -117,17 +156,25 @@ struct ExpTable {
     double b0[QLGA_PMAX];
     float thr[QLGA_PMAX];       // thr[p-1] = largest angle degree p serves within the tolerance
     float theta_split;          // angles above this are split into equal sub-angles
+    SinCosTable sc;
 };
 
-// w = (s K) u  with  s K = g1 F.f + g2 |chi><chi|,
-//   (F.f u)_m = m F_z u_m + (1/2) F_- alpha_{m-1} u_{m-1} + (1/2) F_+ alpha_m u_{m+1},
+// The site's own spin gauge.  With e = F_+/|F_+| and D = diag(e^-2, e^-1, 1, e, e^2) (rows
+// m = +2..-2), K' = D^-1 K D has REAL off-diagonal elements |g1 F_+| alpha_m / 2: a spin rotation
+// about z that turns F into the x-z plane.  P(K) v = D P(K') D^-1 v exactly, the rank-one part keeps
+// its form with psi' = D^-1 psi (time reversal commutes with rotations), so one application of
+// s K' costs 68 FP instructions instead of 88; the two diagonal rotations cost 16 per vector on
+// the way in and are folded into the scalar phase on the way out.
+//
+// w = (s K') u  with  s K' = g1 F'.f + g2 |chi'><chi'|,
+//   (F'.f u)_m = m F_z u_m + (1/2)|F_+| (alpha_{m-1} u_{m-1} + alpha_m u_{m+1}),
 //   alpha_1 = alpha_-2 = 2, alpha_0 = alpha_-1 = sqrt(6)   (f_+|m> = sqrt(6 - m(m+1))|m+1>),
-//   <chi|u> = sum_m (-1)^m psi_{-m} u_m,   chi_m = (-1)^m conj(psi_{-m}).
-// Inputs are pre-scaled: az = g1 F_z, a1 = g1 F_+ (coefficient 2/2), a6 = g1 (sqrt6/2) F_+.
+//   <chi'|u> = sum_m (-1)^m psi'_{-m} u_m,   chi'_m = (-1)^m conj(psi'_{-m}).
+// Inputs are pre-scaled: az = g1 F_z, az2 = 2 az, a1 = g1 |F_+|, a6 = (sqrt6/2) a1.
 template <typename T>
-__device__ __forceinline__ void apply_sK(const cx<T> u[5], cx<T> w[5], T az, cx<T> a1, cx<T> a6,
+__device__ __forceinline__ void apply_sK(const cx<T> u[5], cx<T> w[5], T az, T az2, T a1, T a6,
                                          T g2, const cx<T> psi[5]) {
-    // rank-one part: t = g2 <chi|u>
+    // rank-one part: t = g2 <chi'|u>
     cx<T> t = cmul(psi[4], u[0]);
     t = cfma(psi[2], u[2], t);
     t = cfma(psi[0], u[4], t);
@@ -135,26 +182,19 @@ __device__ __forceinline__ void apply_sK(const cx<T> u[5], cx<T> w[5], T az, cx<
     t2 = cfma(psi[1], u[3], t2);
     t = t - t2;
     t.re *= g2; t.im *= g2;
-    // spin part, rows m = +2..-2 (j = 0..4); raising uses conj(F_+) on u_{m-1} (j+1),
-    // lowering uses F_+ on u_{m+1} (j-1)
-    const T two = (T)2;
-    cx<T> r0 = mk<T>(two * az * u[0].re, two * az * u[0].im);
-    r0 = cfma_conj(a1, u[1], r0);
-    cx<T> r1 = mk<T>(az * u[1].re, az * u[1].im);
-    r1 = cfma(a1, u[0], r1);
-    r1 = cfma_conj(a6, u[2], r1);
-    cx<T> r2 = cmul(a6, u[1]);
-    r2 = cfma_conj(a6, u[3], r2);
-    cx<T> r3 = mk<T>(-az * u[3].re, -az * u[3].im);
-    r3 = cfma(a6, u[2], r3);
-    r3 = cfma_conj(a1, u[4], r3);
-    cx<T> r4 = mk<T>(-two * az * u[4].re, -two * az * u[4].im);
-    r4 = cfma(a1, u[3], r4);
-    // add t * chi_m,  chi_m = (-1)^m conj(psi_{-m})
+    // spin part, rows m = +2..-2 (j = 0..4), real symmetric tridiagonal
+    const cx<T> r0 = mk<T>(fma(a1, u[1].re, az2 * u[0].re), fma(a1, u[1].im, az2 * u[0].im));
+    const cx<T> r1 = mk<T>(fma(a6, u[2].re, fma(a1, u[0].re, az * u[1].re)),
+                           fma(a6, u[2].im, fma(a1, u[0].im, az * u[1].im)));
+    const cx<T> r2 = mk<T>(fma(a6, u[3].re, a6 * u[1].re), fma(a6, u[3].im, a6 * u[1].im));
+    const cx<T> r3 = mk<T>(fma(a1, u[4].re, fma(a6, u[2].re, -(az * u[3].re))),
+                           fma(a1, u[4].im, fma(a6, u[2].im, -(az * u[3].im))));
+    const cx<T> r4 = mk<T>(fma(a1, u[3].re, -(az2 * u[4].re)), fma(a1, u[3].im, -(az2 * u[4].im)));
+    // add t * chi'_m,  chi'_m = (-1)^m conj(psi'_{-m})
     w[0] = cfma_conj(psi[4], t, r0);
-    w[1] = r1 - cfma_conj(psi[3], t, mk<T>((T)0, (T)0));
+    w[1] = cfnma_conj(psi[3], t, r1);
     w[2] = cfma_conj(psi[2], t, r2);
-    w[3] = r3 - cfma_conj(psi[1], t, mk<T>((T)0, (T)0));
+    w[3] = cfnma_conj(psi[1], t, r3);
     w[4] = cfma_conj(psi[0], t, r4);
 }
 
@@ -172,52 +212,83 @@ __device__ __forceinline__ int count_below(const float* thr, float theta) {
     return c[0];
 }
 
-// Site-local coefficients of sK = g1 F.f + g2 |chi><chi| (pre-scaled, see apply_sK).
+// Site-local coefficients of sK' (pre-scaled, see apply_sK) in the site's spin gauge.
 template <typename T> struct KCoef {
-    T az, g2;
-    cx<T> a1, a6;
-    cx<T> psi[5];
+    T az, az2, a1, a6, g2;
+    cx<T> e, e2;                                   // gauge phase F_+/|F_+| and its square
+    cx<T> psi[5];                                  // psi' = D^-1 psi
     T rho;
     float theta;                                   // 2|g1||F| + |g2| rho, this lane
 };
 
+// Computes the coefficients from the site and rotates the site into the spin gauge in place:
+// s.q[j][sigma] <- D^-1_j s.q[j][sigma],  D^-1 = diag(e^2, e, 1, conj e, conj e^2).
 template <typename T>
-__device__ __forceinline__ void site_coefficients(const Site<T>& s, const UConst<T>& uc, KCoef<T>& kc) {
+__device__ __forceinline__ void site_coefficients(Site<T>& s, const UConst<T>& uc, KCoef<T>& kc) {
     T n[5];
+    cx<T> psi[5];
 #pragma unroll
     for (int j = 0; j < 5; ++j) {
-        kc.psi[j] = s.q[j][0] + s.q[j][1];
-        n[j] = fma(kc.psi[j].re, kc.psi[j].re, kc.psi[j].im * kc.psi[j].im);
+        psi[j] = s.q[j][0] + s.q[j][1];
+        n[j] = fma(psi[j].re, psi[j].re, psi[j].im * psi[j].im);
     }
     kc.rho = (n[0] + n[4]) + (n[1] + n[3]) + n[2];
     const T Fz = (T)2 * (n[0] - n[4]) + (n[1] - n[3]);
     // F_+ = sum_m alpha_m conj(psi_{m+1}) psi_m = 2(conj(psi_2) psi_1 + conj(psi_-1) psi_-2)
     //                                           + sqrt6 (conj(psi_1) psi_0 + conj(psi_0) psi_-1)
-    cx<T> fa = cfma_conj(kc.psi[0], kc.psi[1], mk<T>((T)0, (T)0));
-    fa = cfma_conj(kc.psi[3], kc.psi[4], fa);
-    cx<T> fb = cfma_conj(kc.psi[1], kc.psi[2], mk<T>((T)0, (T)0));
-    fb = cfma_conj(kc.psi[2], kc.psi[3], fb);
+    cx<T> fa = cfma_conj(psi[0], psi[1], mk<T>((T)0, (T)0));
+    fa = cfma_conj(psi[3], psi[4], fa);
+    cx<T> fb = cfma_conj(psi[1], psi[2], mk<T>((T)0, (T)0));
+    fb = cfma_conj(psi[2], psi[3], fb);
     const T rt6 = (T)2.4494897427831780981972840747059;
     const cx<T> Fp = mk<T>(fma(rt6, fb.re, (T)2 * fa.re), fma(rt6, fb.im, (T)2 * fa.im));
+    const T fp2 = fma(Fp.re, Fp.re, Fp.im * Fp.im);
     // angle bound theta = 2 |g1| |F| + |g2| rho (the exact spectral norms of the two parts);
     // |F| by the approximate reciprocal square root (2 ulp; the 2^-10 margin covers it)
-    const float f2 = fmaxf((float)(Fz * Fz + Fp.re * Fp.re + Fp.im * Fp.im), 1e-37f);
+    const float f2 = fmaxf((float)fma(Fz, Fz, fp2), 1e-37f);
     const float Fabs = f2 * __frsqrt_rn(f2);
     kc.theta = (2.0f * fabsf((float)uc.g1) * Fabs + fabsf((float)uc.g2) * (float)kc.rho) * 1.0009765625f;
     kc.g2 = uc.g2;
     kc.az = uc.g1 * Fz;
-    kc.a1 = mk<T>(uc.g1 * Fp.re, uc.g1 * Fp.im);
+    kc.az2 = kc.az + kc.az;
+    // gauge phase e = F_+/|F_+|; a transverse spin below 1e-18 is dropped (its term is below
+    // 1e-18 |g1| |u|, far under the truncation tolerance) and the gauge is the identity
+    const bool tiny = !(fp2 > (T)1e-36);
+    const T rinv = rsqrt_pos(tiny ? (T)1 : fp2);
+    kc.e = tiny ? mk<T>((T)1, (T)0) : mk<T>(Fp.re * rinv, Fp.im * rinv);
+    kc.e2 = mk<T>(fma(kc.e.re, kc.e.re, -(kc.e.im * kc.e.im)), (T)2 * kc.e.re * kc.e.im);
+    kc.a1 = tiny ? (T)0 : uc.g1 * (fp2 * rinv);
     const T rt6h = (T)1.2247448713915890490986420373529;          // sqrt(6)/2
-    kc.a6 = mk<T>(rt6h * kc.a1.re, rt6h * kc.a1.im);
+    kc.a6 = rt6h * kc.a1;
+#pragma unroll
+    for (int sg = 0; sg < 2; ++sg) {
+        s.q[0][sg] = cmul(kc.e2, s.q[0][sg]);
+        s.q[1][sg] = cmul(kc.e, s.q[1][sg]);
+        s.q[3][sg] = cmul_conj(s.q[3][sg], kc.e);
+        s.q[4][sg] = cmul_conj(s.q[4][sg], kc.e2);
+    }
+#pragma unroll
+    for (int j = 0; j < 5; ++j) kc.psi[j] = s.q[j][0] + s.q[j][1];
 }
 
-// u <- P_p(-i sK) v in Horner form u_{k-1} = v + r_k (-i sK) u_k, k = p..1, u_p = v
+// Leaves the gauge and applies the scalar phase: s.q[j][sigma] <- ph D_j u_j,
+// D = diag(conj e^2, conj e, 1, e, e^2).
+template <typename T>
+__device__ __forceinline__ void gauge_phases(const KCoef<T>& kc, cx<T> ph, cx<T> phj[5]) {
+    phj[0] = cmul_conj(ph, kc.e2);
+    phj[1] = cmul_conj(ph, kc.e);
+    phj[2] = ph;
+    phj[3] = cmul(ph, kc.e);
+    phj[4] = cmul(ph, kc.e2);
+}
+
+// u <- P_p(-i sK') v in Horner form u_{k-1} = v + r_k (-i sK') u_k, k = p..1, u_p = v
 // (stage p acts on v itself: no copy).  psi, hence K, is frozen (reading R4).
 template <typename T>
 __device__ __forceinline__ void horner(const cx<T> v[5], cx<T> u[5], const KCoef<T>& kc,
                                        const double* __restrict__ r, int p) {
     cx<T> w[5];
-    apply_sK<T>(v, w, kc.az, kc.a1, kc.a6, kc.g2, kc.psi);
+    apply_sK<T>(v, w, kc.az, kc.az2, kc.a1, kc.a6, kc.g2, kc.psi);
     {
         const T ik = (T)r[p];
 #pragma unroll
@@ -227,7 +298,7 @@ __device__ __forceinline__ void horner(const cx<T> v[5], cx<T> u[5], const KCoef
     }
 #pragma unroll 1
     for (int k = p - 1; k >= 1; --k) {
-        apply_sK<T>(u, w, kc.az, kc.a1, kc.a6, kc.g2, kc.psi);
+        apply_sK<T>(u, w, kc.az, kc.az2, kc.a1, kc.a6, kc.g2, kc.psi);
         const T ik = (T)r[k];
 #pragma unroll
         for (int j = 0; j < 5; ++j) {
@@ -238,22 +309,21 @@ __device__ __forceinline__ void horner(const cx<T> v[5], cx<T> u[5], const KCoef
 
 // General path (never taken at the paper's amplitudes): scalar phase by the library
 // sincos; angles above theta_split in nsub equal sub-angles (exact: K is frozen).
-// Out of line and by value so that the common path keeps its registers.
+// Takes the site already in its spin gauge.  Out of line and by value so that the
+// common path keeps its registers.
 template <typename T>
-__device__ __noinline__ Site<T> interaction_general(Site<T> s, UConst<T> uc, const ExpTable& tab, float theta) {
-    KCoef<T> kc;
-    site_coefficients<T>(s, uc, kc);
+__device__ __noinline__ Site<T> interaction_general(Site<T> s, KCoef<T> kc, T xph, const ExpTable& tab, float theta) {
     int nsub = 1;
     if (theta > tab.theta_split) nsub = (int)ceilf(theta / tab.theta_split);
     const T inv_nsub = (T)1 / (T)nsub;
-    kc.g2 *= inv_nsub; kc.az *= inv_nsub;
-    kc.a1.re *= inv_nsub; kc.a1.im *= inv_nsub; kc.a6.re *= inv_nsub; kc.a6.im *= inv_nsub;
+    kc.g2 *= inv_nsub; kc.az *= inv_nsub; kc.az2 *= inv_nsub; kc.a1 *= inv_nsub; kc.a6 *= inv_nsub;
     const int p = 1 + count_below(tab.thr, theta / (float)nsub * 1.0009765625f);
     T sn, cs;
-    sincos_lib(uc.g0 * kc.rho, &sn, &cs);
+    sincos_lib(xph, &sn, &cs);
     T b0n = (T)1;
     for (int rep = 0; rep < nsub; ++rep) b0n *= (T)tab.b0[p - 1];
-    const cx<T> ph = mk<T>(b0n * cs, -(b0n * sn));
+    cx<T> phj[5];
+    gauge_phases<T>(kc, mk<T>(b0n * cs, -(b0n * sn)), phj);
     for (int sg = 0; sg < 2; ++sg) {
         cx<T> v[5], u[5];
         for (int j = 0; j < 5; ++j) v[j] = s.q[j][sg];
@@ -261,7 +331,7 @@ __device__ __noinline__ Site<T> interaction_general(Site<T> s, UConst<T> uc, con
             horner<T>(v, u, kc, tab.r[p - 1], p);
             for (int j = 0; j < 5; ++j) v[j] = u[j];
         }
-        for (int j = 0; j < 5; ++j) s.q[j][sg] = cmul(ph, v[j]);
+        for (int j = 0; j < 5; ++j) s.q[j][sg] = cmul(phj[j], v[j]);
     }
     return s;
 }
@@ -272,27 +342,28 @@ __device__ __noinline__ Site<T> interaction_general(Site<T> s, UConst<T> uc, con
 template <typename T>
 __device__ __forceinline__ void interaction(Site<T>& s, const UConst<T>& uc, const ExpTable& tab) {
     KCoef<T> kc;
-    site_coefficients<T>(s, uc, kc);
+    site_coefficients<T>(s, uc, kc);               // s is in its spin gauge from here on
     // The first Horner stage of component 1 needs neither the degree nor the phase: it is
     // issued before the warp-wide reductions below so that their latency (rsqrt, REDUX,
-    // vote, the branch on their result) is covered by 88 independent FP64 instructions.
+    // vote, the branch on their result) is covered by independent FP64 instructions.
     cx<T> va[5], wa[5];
 #pragma unroll
     for (int j = 0; j < 5; ++j) va[j] = s.q[j][0];
-    apply_sK<T>(va, wa, kc.az, kc.a1, kc.a6, kc.g2, kc.psi);
+    apply_sK<T>(va, wa, kc.az, kc.az2, kc.a1, kc.a6, kc.g2, kc.psi);
     // warp-uniform angle (one polynomial degree per warp keeps the Horner loops convergent)
     const float theta = __uint_as_float(__reduce_max_sync(0xffffffffu, __float_as_uint(kc.theta)));
     const T xph = uc.g0 * kc.rho;                  // scalar phase exp(-i s c0 rho)
     const bool big_phase = !__all_sync(0xffffffffu, fabs(xph) <= (T)0.0625);
     if (big_phase || theta > tab.theta_split) {
-        s = interaction_general<T>(s, uc, tab, theta);
+        s = interaction_general<T>(s, kc, xph, tab, theta);
         return;
     }
     T sn, cs;
-    sincos_small<T>(xph, &sn, &cs);
+    sincos_small<T>(xph, tab.sc, &sn, &cs);
     const int p = 1 + count_below(tab.thr, theta);
     const T pb0 = (T)tab.b0[p - 1];                // constant term of the polynomial (1 - O(tol))
-    const cx<T> ph = mk<T>(pb0 * cs, -(pb0 * sn));
+    cx<T> phj[5];
+    gauge_phases<T>(kc, mk<T>(pb0 * cs, -(pb0 * sn)), phj);
     const double* r = tab.r[p - 1];
     {
         cx<T> u[5];
@@ -303,7 +374,7 @@ __device__ __forceinline__ void interaction(Site<T>& s, const UConst<T>& uc, con
         }
 #pragma unroll 1
         for (int k = p - 1; k >= 1; --k) {
-            apply_sK<T>(u, wa, kc.az, kc.a1, kc.a6, kc.g2, kc.psi);
+            apply_sK<T>(u, wa, kc.az, kc.az2, kc.a1, kc.a6, kc.g2, kc.psi);
             const T ikk = (T)r[k];
 #pragma unroll
             for (int j = 0; j < 5; ++j) {
@@ -311,7 +382,7 @@ __device__ __forceinline__ void interaction(Site<T>& s, const UConst<T>& uc, con
             }
         }
 #pragma unroll
-        for (int j = 0; j < 5; ++j) s.q[j][0] = cmul(ph, u[j]);
+        for (int j = 0; j < 5; ++j) s.q[j][0] = cmul(phj[j], u[j]);
     }
     {
         cx<T> v[5], u[5];
@@ -319,7 +390,7 @@ __device__ __forceinline__ void interaction(Site<T>& s, const UConst<T>& uc, con
         for (int j = 0; j < 5; ++j) v[j] = s.q[j][1];
         horner<T>(v, u, kc, r, p);
 #pragma unroll
-        for (int j = 0; j < 5; ++j) s.q[j][1] = cmul(ph, u[j]);
+        for (int j = 0; j < 5; ++j) s.q[j][1] = cmul(phj[j], u[j]);
     }
 }
 
