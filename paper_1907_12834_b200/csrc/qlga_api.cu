@@ -90,6 +90,8 @@ static void build_exp_table(ExpTable& tab, int tol_log2) {
         tab.b0[p - 1] = (double)b[0];
         for (int k = 0; k <= QLGA_PMAX; ++k) tab.r[p - 1][k] = 0.0;
         for (int k = 1; k <= p; ++k) tab.r[p - 1][k] = (double)(b[k] / b[k - 1]);
+        tab.b0f[p - 1] = (float)tab.b0[p - 1];
+        for (int k = 0; k <= QLGA_PMAX; ++k) tab.rf[p - 1][k] = (float)tab.r[p - 1][k];
     }
     const double top = tab.thr[QLGA_PMAX - 1];
     tab.theta_split = (float)(top < 0.5 ? top : 0.5);

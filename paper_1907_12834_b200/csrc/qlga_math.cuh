@@ -17,7 +17,7 @@ template <typename T> struct vec2;
 template <> struct vec2<double> { using type = double2; };
 template <> struct vec2<float>  { using type = float2; };
 
-template <typename T> struct cx {
+template <typename T> struct __align__(2 * sizeof(T)) cx {   // one 16-byte / 8-byte element, as in memory
     T re, im;
 };
 
@@ -49,6 +49,62 @@ template <typename T> __device__ __forceinline__ cx<T> cfnma_conj(cx<T> a, cx<T>
 // a * conj(b)
 template <typename T> __device__ __forceinline__ cx<T> cmul_conj(cx<T> a, cx<T> b) {
     return mk<T>(fma(a.re, b.re, a.im * b.im), fma(a.im, b.re, -(a.re * b.im)));
+}
+
+// real * complex, acc + real * complex
+template <typename T> __device__ __forceinline__ cx<T> rmul(T a, cx<T> u) { return mk<T>(a * u.re, a * u.im); }
+template <typename T> __device__ __forceinline__ cx<T> rfma(T a, cx<T> u, cx<T> acc) {
+    return mk<T>(fma(a, u.re, acc.re), fma(a, u.im, acc.im));
+}
+// a + i b,  a - i b,  v - i k w  (multiplication by +-i is a swap with one sign change)
+template <typename T> __device__ __forceinline__ cx<T> add_i(cx<T> a, cx<T> b) { return mk<T>(a.re - b.im, a.im + b.re); }
+template <typename T> __device__ __forceinline__ cx<T> sub_i(cx<T> a, cx<T> b) { return mk<T>(a.re + b.im, a.im - b.re); }
+template <typename T> __device__ __forceinline__ cx<T> axmi(T k, cx<T> w, cx<T> v) {
+    return mk<T>(fma(k, w.im, v.re), fma(-k, w.re, v.im));
+}
+
+// ---------------------------------------------------------------------------
+// fp32: packed arithmetic.  sm_100a has two-wide fp32 instructions (FFMA2, FADD2, FMUL2:
+// fma.rn.f32x2 ...) whose operands take a scalar broadcast, a half swap and per-half signs
+// as free modifiers, so a complex number held as one (re, im) register pair costs one
+// instruction per real-complex product or addition and two per complex-complex product:
+// half the issue slots of the scalar form.  Non-template overloads for cx<float>; the
+// fp64 path keeps the generic templates above (there is no packed fp64 arithmetic).
+// ---------------------------------------------------------------------------
+__device__ __forceinline__ float2 pk(cx<float> z) { return make_float2(z.re, z.im); }
+__device__ __forceinline__ float2 pk_i(cx<float> z) { return make_float2(-z.im, z.re); }     // i z
+__device__ __forceinline__ float2 pk_mi(cx<float> z) { return make_float2(z.im, -z.re); }    // -i z
+__device__ __forceinline__ float2 bc(float a) { return make_float2(a, a); }
+__device__ __forceinline__ cx<float> up(float2 v) { return mk<float>(v.x, v.y); }
+__device__ __forceinline__ cx<float> operator+(cx<float> a, cx<float> b) { return up(__fadd2_rn(pk(a), pk(b))); }
+__device__ __forceinline__ cx<float> operator-(cx<float> a, cx<float> b) {
+    return up(__fadd2_rn(pk(a), make_float2(-b.re, -b.im)));
+}
+// (the swap / sign modifiers exist on the first source operand of FFMA2 / FMUL2, the scalar
+// broadcast on the second: the complex value goes first, the broadcast coefficient second)
+__device__ __forceinline__ cx<float> cmul(cx<float> a, cx<float> b) {
+    return up(__ffma2_rn(pk_i(b), bc(a.im), __fmul2_rn(pk(b), bc(a.re))));
+}
+__device__ __forceinline__ cx<float> cfma(cx<float> a, cx<float> b, cx<float> acc) {
+    return up(__ffma2_rn(pk_i(b), bc(a.im), __ffma2_rn(pk(b), bc(a.re), pk(acc))));
+}
+__device__ __forceinline__ cx<float> cfma_conj(cx<float> a, cx<float> b, cx<float> acc) {
+    return up(__ffma2_rn(pk_mi(b), bc(a.im), __ffma2_rn(pk(b), bc(a.re), pk(acc))));
+}
+__device__ __forceinline__ cx<float> cfnma_conj(cx<float> a, cx<float> b, cx<float> acc) {
+    return up(__ffma2_rn(pk_i(b), bc(a.im), __ffma2_rn(pk(b), bc(-a.re), pk(acc))));
+}
+__device__ __forceinline__ cx<float> cmul_conj(cx<float> a, cx<float> b) {
+    return up(__ffma2_rn(pk_mi(a), bc(b.im), __fmul2_rn(pk(a), bc(b.re))));
+}
+__device__ __forceinline__ cx<float> rmul(float a, cx<float> u) { return up(__fmul2_rn(pk(u), bc(a))); }
+__device__ __forceinline__ cx<float> rfma(float a, cx<float> u, cx<float> acc) {
+    return up(__ffma2_rn(pk(u), bc(a), pk(acc)));
+}
+__device__ __forceinline__ cx<float> add_i(cx<float> a, cx<float> b) { return up(__fadd2_rn(pk(a), pk_i(b))); }
+__device__ __forceinline__ cx<float> sub_i(cx<float> a, cx<float> b) { return up(__fadd2_rn(pk(a), pk_mi(b))); }
+__device__ __forceinline__ cx<float> axmi(float k, cx<float> w, cx<float> v) {
+    return up(__ffma2_rn(pk_mi(w), bc(k), pk(v)));
 }
 
 // 1/sqrt(x) for x >= 1e-36: hardware seed (MUFU.RSQ64H / MUFU.RSQ) + Newton steps, no
@@ -121,8 +177,8 @@ __device__ __forceinline__ void kin_messages(const Site<T>& s, int sigma, cx<T> 
 #pragma unroll
     for (int j = 0; j < 5; ++j) {
         cx<T> a = s.q[j][sigma], b = s.q[j][1 - sigma];
-        Fw[j] = mk<T>(b.re - a.im, b.im + a.re);
-        Bw[j] = mk<T>(a.re - b.im, a.im + b.re);
+        Fw[j] = add_i(b, a);
+        Bw[j] = add_i(a, b);
     }
 }
 
@@ -131,8 +187,8 @@ __device__ __forceinline__ void kin_update(Site<T>& s, int sigma, const cx<T> Fw
                                            const cx<T> Fprev[5], const cx<T> Bnext[5]) {
 #pragma unroll
     for (int j = 0; j < 5; ++j) {
-        s.q[j][sigma]     = mk<T>(Fprev[j].re + Bw[j].im, Fprev[j].im - Bw[j].re);
-        s.q[j][1 - sigma] = mk<T>(Bnext[j].re + Fw[j].im, Bnext[j].im - Fw[j].re);
+        s.q[j][sigma]     = sub_i(Fprev[j], Bw[j]);
+        s.q[j][1 - sigma] = sub_i(Bnext[j], Fw[j]);
     }
 }
 
@@ -154,6 +210,8 @@ struct ExpTable {
     // Chebyshev-economised Taylor polynomial of exp(y) on |y| <= thr[p-1].
     double r[QLGA_PMAX][QLGA_PMAX + 1];
     double b0[QLGA_PMAX];
+    float rf[QLGA_PMAX][QLGA_PMAX + 1];   // the same rounded to fp32 (no conversions in the fp32 loops)
+    float b0f[QLGA_PMAX];
     float thr[QLGA_PMAX];       // thr[p-1] = largest angle degree p serves within the tolerance
     float theta_split;          // angles above this are split into equal sub-angles
     SinCosTable sc;
@@ -166,13 +224,37 @@ struct ExpTable {
 // s K' costs 68 FP instructions instead of 88; the two diagonal rotations cost 16 per vector on
 // the way in and are folded into the scalar phase on the way out.
 //
+__device__ __forceinline__ const double* exp_ratios(const ExpTable& t, int p, double) { return t.r[p - 1]; }
+__device__ __forceinline__ const float* exp_ratios(const ExpTable& t, int p, float) { return t.rf[p - 1]; }
+__device__ __forceinline__ double exp_b0(const ExpTable& t, int p, double) { return t.b0[p - 1]; }
+__device__ __forceinline__ float exp_b0(const ExpTable& t, int p, float) { return t.b0f[p - 1]; }
+
 // w = (s K') u  with  s K' = g1 F'.f + g2 |chi'><chi'|,
 //   (F'.f u)_m = m F_z u_m + (1/2)|F_+| (alpha_{m-1} u_{m-1} + alpha_m u_{m+1}),
 //   alpha_1 = alpha_-2 = 2, alpha_0 = alpha_-1 = sqrt(6)   (f_+|m> = sqrt(6 - m(m+1))|m+1>),
 //   <chi'|u> = sum_m (-1)^m psi'_{-m} u_m,   chi'_m = (-1)^m conj(psi'_{-m}).
 // Inputs are pre-scaled: az = g1 F_z, az2 = 2 az, a1 = g1 |F_+|, a6 = (sqrt6/2) a1.
-template <typename T>
-__device__ __forceinline__ void apply_sK(const cx<T> u[5], cx<T> w[5], T az, T az2, T a1, T a6,
+//
+// fp32 does not use the gauge: at its degree (3) the two rotations cost what the real
+// coefficients save, and they add two roundings per application (measured: 1.5-2x the
+// error against the oracle).  There a1 = g1 F_+ and a6 stay complex, the lowering
+// element acts as a u, the raising element as conj(a) u, and psi' = psi.
+template <typename T> struct SpinGauge { static constexpr bool on = sizeof(T) == 8; };
+template <typename T, bool G> struct OffDiag { using type = T; };
+template <typename T> struct OffDiag<T, false> { using type = cx<T>; };
+
+template <typename T> __device__ __forceinline__ cx<T> lower(T a, cx<T> u) { return rmul(a, u); }
+template <typename T> __device__ __forceinline__ cx<T> lower(cx<T> a, cx<T> u) { return cmul(a, u); }
+template <typename T> __device__ __forceinline__ cx<T> lower(T a, cx<T> u, cx<T> acc) { return rfma(a, u, acc); }
+template <typename T> __device__ __forceinline__ cx<T> lower(cx<T> a, cx<T> u, cx<T> acc) { return cfma(a, u, acc); }
+template <typename T> __device__ __forceinline__ cx<T> raise(T a, cx<T> u, cx<T> acc) { return rfma(a, u, acc); }
+template <typename T> __device__ __forceinline__ cx<T> raise(cx<T> a, cx<T> u, cx<T> acc) { return cfma_conj(a, u, acc); }
+
+template <typename T> __device__ __forceinline__ void scale_by(T& a, T k) { a *= k; }
+template <typename T> __device__ __forceinline__ void scale_by(cx<T>& a, T k) { a = rmul(k, a); }
+
+template <typename T, typename A>
+__device__ __forceinline__ void apply_sK(const cx<T> u[5], cx<T> w[5], T az, T az2, A a1, A a6,
                                          T g2, const cx<T> psi[5]) {
     // rank-one part: t = g2 <chi'|u>
     cx<T> t = cmul(psi[4], u[0]);
@@ -180,16 +262,13 @@ __device__ __forceinline__ void apply_sK(const cx<T> u[5], cx<T> w[5], T az, T a
     t = cfma(psi[0], u[4], t);
     cx<T> t2 = cmul(psi[3], u[1]);
     t2 = cfma(psi[1], u[3], t2);
-    t = t - t2;
-    t.re *= g2; t.im *= g2;
-    // spin part, rows m = +2..-2 (j = 0..4), real symmetric tridiagonal
-    const cx<T> r0 = mk<T>(fma(a1, u[1].re, az2 * u[0].re), fma(a1, u[1].im, az2 * u[0].im));
-    const cx<T> r1 = mk<T>(fma(a6, u[2].re, fma(a1, u[0].re, az * u[1].re)),
-                           fma(a6, u[2].im, fma(a1, u[0].im, az * u[1].im)));
-    const cx<T> r2 = mk<T>(fma(a6, u[3].re, a6 * u[1].re), fma(a6, u[3].im, a6 * u[1].im));
-    const cx<T> r3 = mk<T>(fma(a1, u[4].re, fma(a6, u[2].re, -(az * u[3].re))),
-                           fma(a1, u[4].im, fma(a6, u[2].im, -(az * u[3].im))));
-    const cx<T> r4 = mk<T>(fma(a1, u[3].re, -(az2 * u[4].re)), fma(a1, u[3].im, -(az2 * u[4].im)));
+    t = rmul(g2, t - t2);
+    // spin part, rows m = +2..-2 (j = 0..4), Hermitian tridiagonal (real symmetric in the gauge)
+    const cx<T> r0 = raise(a1, u[1], rmul(az2, u[0]));
+    const cx<T> r1 = raise(a6, u[2], lower(a1, u[0], rmul(az, u[1])));
+    const cx<T> r2 = raise(a6, u[3], lower(a6, u[1]));
+    const cx<T> r3 = raise(a1, u[4], lower(a6, u[2], rmul(-az, u[3])));
+    const cx<T> r4 = lower(a1, u[3], rmul(-az2, u[4]));
     // add t * chi'_m,  chi'_m = (-1)^m conj(psi'_{-m})
     w[0] = cfma_conj(psi[4], t, r0);
     w[1] = cfnma_conj(psi[3], t, r1);
@@ -214,7 +293,9 @@ __device__ __forceinline__ int count_below(const float* thr, float theta) {
 
 // Site-local coefficients of sK' (pre-scaled, see apply_sK) in the site's spin gauge.
 template <typename T> struct KCoef {
-    T az, az2, a1, a6, g2;
+    using A = typename OffDiag<T, SpinGauge<T>::on>::type;
+    T az, az2, g2;
+    A a1, a6;
     cx<T> e, e2;                                   // gauge phase F_+/|F_+| and its square
     cx<T> psi[5];                                  // psi' = D^-1 psi
     T rho;
@@ -251,59 +332,67 @@ __device__ __forceinline__ void site_coefficients(Site<T>& s, const UConst<T>& u
     kc.g2 = uc.g2;
     kc.az = uc.g1 * Fz;
     kc.az2 = kc.az + kc.az;
-    // gauge phase e = F_+/|F_+|; a transverse spin below 1e-18 is dropped (its term is below
-    // 1e-18 |g1| |u|, far under the truncation tolerance) and the gauge is the identity
-    const bool tiny = !(fp2 > (T)1e-36);
-    const T rinv = rsqrt_pos(tiny ? (T)1 : fp2);
-    kc.e = tiny ? mk<T>((T)1, (T)0) : mk<T>(Fp.re * rinv, Fp.im * rinv);
-    kc.e2 = mk<T>(fma(kc.e.re, kc.e.re, -(kc.e.im * kc.e.im)), (T)2 * kc.e.re * kc.e.im);
-    kc.a1 = tiny ? (T)0 : uc.g1 * (fp2 * rinv);
     const T rt6h = (T)1.2247448713915890490986420373529;          // sqrt(6)/2
-    kc.a6 = rt6h * kc.a1;
+    if constexpr (SpinGauge<T>::on) {
+        // gauge phase e = F_+/|F_+|; a transverse spin below 1e-18 is dropped (its term is below
+        // 1e-18 |g1| |u|, far under the truncation tolerance) and the gauge is the identity
+        const bool tiny = !(fp2 > (T)1e-36);
+        const T rinv = rsqrt_pos(tiny ? (T)1 : fp2);
+        kc.e = tiny ? mk<T>((T)1, (T)0) : mk<T>(Fp.re * rinv, Fp.im * rinv);
+        kc.e2 = mk<T>(fma(kc.e.re, kc.e.re, -(kc.e.im * kc.e.im)), (T)2 * kc.e.re * kc.e.im);
+        kc.a1 = tiny ? (T)0 : uc.g1 * (fp2 * rinv);
+        kc.a6 = rt6h * kc.a1;
 #pragma unroll
-    for (int sg = 0; sg < 2; ++sg) {
-        s.q[0][sg] = cmul(kc.e2, s.q[0][sg]);
-        s.q[1][sg] = cmul(kc.e, s.q[1][sg]);
-        s.q[3][sg] = cmul_conj(s.q[3][sg], kc.e);
-        s.q[4][sg] = cmul_conj(s.q[4][sg], kc.e2);
+        for (int sg = 0; sg < 2; ++sg) {
+            s.q[0][sg] = cmul(kc.e2, s.q[0][sg]);
+            s.q[1][sg] = cmul(kc.e, s.q[1][sg]);
+            s.q[3][sg] = cmul_conj(s.q[3][sg], kc.e);
+            s.q[4][sg] = cmul_conj(s.q[4][sg], kc.e2);
+        }
+#pragma unroll
+        for (int j = 0; j < 5; ++j) kc.psi[j] = s.q[j][0] + s.q[j][1];
+    } else {
+        kc.a1 = rmul(uc.g1, Fp);
+        kc.a6 = rmul(rt6h, kc.a1);
+#pragma unroll
+        for (int j = 0; j < 5; ++j) kc.psi[j] = psi[j];
     }
-#pragma unroll
-    for (int j = 0; j < 5; ++j) kc.psi[j] = s.q[j][0] + s.q[j][1];
 }
 
 // Leaves the gauge and applies the scalar phase: s.q[j][sigma] <- ph D_j u_j,
 // D = diag(conj e^2, conj e, 1, e, e^2).
 template <typename T>
 __device__ __forceinline__ void gauge_phases(const KCoef<T>& kc, cx<T> ph, cx<T> phj[5]) {
-    phj[0] = cmul_conj(ph, kc.e2);
-    phj[1] = cmul_conj(ph, kc.e);
-    phj[2] = ph;
-    phj[3] = cmul(ph, kc.e);
-    phj[4] = cmul(ph, kc.e2);
+    if constexpr (SpinGauge<T>::on) {
+        phj[0] = cmul_conj(ph, kc.e2);
+        phj[1] = cmul_conj(ph, kc.e);
+        phj[2] = ph;
+        phj[3] = cmul(ph, kc.e);
+        phj[4] = cmul(ph, kc.e2);
+    } else {
+#pragma unroll
+        for (int j = 0; j < 5; ++j) phj[j] = ph;
+    }
 }
 
 // u <- P_p(-i sK') v in Horner form u_{k-1} = v + r_k (-i sK') u_k, k = p..1, u_p = v
 // (stage p acts on v itself: no copy).  psi, hence K, is frozen (reading R4).
 template <typename T>
 __device__ __forceinline__ void horner(const cx<T> v[5], cx<T> u[5], const KCoef<T>& kc,
-                                       const double* __restrict__ r, int p) {
+                                       const T* __restrict__ r, int p) {
     cx<T> w[5];
-    apply_sK<T>(v, w, kc.az, kc.az2, kc.a1, kc.a6, kc.g2, kc.psi);
+    apply_sK(v, w, kc.az, kc.az2, kc.a1, kc.a6, kc.g2, kc.psi);
     {
-        const T ik = (T)r[p];
+        const T ik = r[p];
 #pragma unroll
-        for (int j = 0; j < 5; ++j) {
-            u[j].re = fma(ik, w[j].im, v[j].re); u[j].im = fma(-ik, w[j].re, v[j].im);
-        }
+        for (int j = 0; j < 5; ++j) u[j] = axmi(ik, w[j], v[j]);
     }
 #pragma unroll 1
     for (int k = p - 1; k >= 1; --k) {
-        apply_sK<T>(u, w, kc.az, kc.az2, kc.a1, kc.a6, kc.g2, kc.psi);
-        const T ik = (T)r[k];
+        apply_sK(u, w, kc.az, kc.az2, kc.a1, kc.a6, kc.g2, kc.psi);
+        const T ik = r[k];
 #pragma unroll
-        for (int j = 0; j < 5; ++j) {
-            u[j].re = fma(ik, w[j].im, v[j].re); u[j].im = fma(-ik, w[j].re, v[j].im);
-        }
+        for (int j = 0; j < 5; ++j) u[j] = axmi(ik, w[j], v[j]);
     }
 }
 
@@ -316,19 +405,20 @@ __device__ __noinline__ Site<T> interaction_general(Site<T> s, KCoef<T> kc, T xp
     int nsub = 1;
     if (theta > tab.theta_split) nsub = (int)ceilf(theta / tab.theta_split);
     const T inv_nsub = (T)1 / (T)nsub;
-    kc.g2 *= inv_nsub; kc.az *= inv_nsub; kc.az2 *= inv_nsub; kc.a1 *= inv_nsub; kc.a6 *= inv_nsub;
+    kc.g2 *= inv_nsub; kc.az *= inv_nsub; kc.az2 *= inv_nsub;
+    scale_by(kc.a1, inv_nsub); scale_by(kc.a6, inv_nsub);
     const int p = 1 + count_below(tab.thr, theta / (float)nsub * 1.0009765625f);
     T sn, cs;
     sincos_lib(xph, &sn, &cs);
     T b0n = (T)1;
-    for (int rep = 0; rep < nsub; ++rep) b0n *= (T)tab.b0[p - 1];
+    for (int rep = 0; rep < nsub; ++rep) b0n *= exp_b0(tab, p, (T)0);
     cx<T> phj[5];
     gauge_phases<T>(kc, mk<T>(b0n * cs, -(b0n * sn)), phj);
     for (int sg = 0; sg < 2; ++sg) {
         cx<T> v[5], u[5];
         for (int j = 0; j < 5; ++j) v[j] = s.q[j][sg];
         for (int rep = 0; rep < nsub; ++rep) {
-            horner<T>(v, u, kc, tab.r[p - 1], p);
+            horner<T>(v, u, kc, exp_ratios(tab, p, (T)0), p);
             for (int j = 0; j < 5; ++j) v[j] = u[j];
         }
         for (int j = 0; j < 5; ++j) s.q[j][sg] = cmul(phj[j], v[j]);
@@ -349,7 +439,7 @@ __device__ __forceinline__ void interaction(Site<T>& s, const UConst<T>& uc, con
     cx<T> va[5], wa[5];
 #pragma unroll
     for (int j = 0; j < 5; ++j) va[j] = s.q[j][0];
-    apply_sK<T>(va, wa, kc.az, kc.az2, kc.a1, kc.a6, kc.g2, kc.psi);
+    apply_sK(va, wa, kc.az, kc.az2, kc.a1, kc.a6, kc.g2, kc.psi);
     // warp-uniform angle (one polynomial degree per warp keeps the Horner loops convergent)
     const float theta = __uint_as_float(__reduce_max_sync(0xffffffffu, __float_as_uint(kc.theta)));
     const T xph = uc.g0 * kc.rho;                  // scalar phase exp(-i s c0 rho)
@@ -361,25 +451,21 @@ __device__ __forceinline__ void interaction(Site<T>& s, const UConst<T>& uc, con
     T sn, cs;
     sincos_small<T>(xph, tab.sc, &sn, &cs);
     const int p = 1 + count_below(tab.thr, theta);
-    const T pb0 = (T)tab.b0[p - 1];                // constant term of the polynomial (1 - O(tol))
+    const T pb0 = exp_b0(tab, p, (T)0);                // constant term of the polynomial (1 - O(tol))
     cx<T> phj[5];
     gauge_phases<T>(kc, mk<T>(pb0 * cs, -(pb0 * sn)), phj);
-    const double* r = tab.r[p - 1];
+    const T* r = exp_ratios(tab, p, (T)0);
     {
         cx<T> u[5];
-        const T ik = (T)r[p];
+        const T ik = r[p];
 #pragma unroll
-        for (int j = 0; j < 5; ++j) {
-            u[j].re = fma(ik, wa[j].im, va[j].re); u[j].im = fma(-ik, wa[j].re, va[j].im);
-        }
+        for (int j = 0; j < 5; ++j) u[j] = axmi(ik, wa[j], va[j]);
 #pragma unroll 1
         for (int k = p - 1; k >= 1; --k) {
-            apply_sK<T>(u, wa, kc.az, kc.az2, kc.a1, kc.a6, kc.g2, kc.psi);
-            const T ikk = (T)r[k];
+            apply_sK(u, wa, kc.az, kc.az2, kc.a1, kc.a6, kc.g2, kc.psi);
+            const T ikk = r[k];
 #pragma unroll
-            for (int j = 0; j < 5; ++j) {
-                u[j].re = fma(ikk, wa[j].im, va[j].re); u[j].im = fma(-ikk, wa[j].re, va[j].im);
-            }
+            for (int j = 0; j < 5; ++j) u[j] = axmi(ikk, wa[j], va[j]);
         }
 #pragma unroll
         for (int j = 0; j < 5; ++j) s.q[j][0] = cmul(phj[j], u[j]);
