@@ -148,6 +148,42 @@ qlga_status qlga_density_l2_error(qlga_ctx*, const void* rho_ref, int src_on_dev
  * *host_count (may exceed max_out).  Synchronises the stream.  QLGA_EUNSUP in 1D. */
 qlga_status qlga_vortices(qlga_ctx*, int32_t* host_out, int64_t max_out, int64_t* host_count);
 
+/* ---- Slab decomposition over several GPUs ---------------------
+ * The paper only states that its code "naturally scales with the number of GPUs"
+ * (PAPER.md:1092-1094).  Here the lattice is cut into slabs along its slowest axis (x in 1D,
+ * y in 2D, z in 3D), one slab per GPU / context.  A slab context is an ordinary context whose
+ * slowest axis holds `ghost` ghost layers, then the owned layers, then `ghost` ghost layers.
+ * A time step moves information by exactly 4 sites per direction (four kinetic factors of
+ * radius 1), so with ghost = 4 valid ghost layers before a step the owned layers are exact
+ * after it, whatever the periodic wrap of the extended slab puts into its ghost layers; the
+ * ghost layers are then refreshed from the neighbouring slabs' edge layers (one exchange of
+ * 2 x ghost x 160 B per site of a layer per step in fp64).  The library moves layers between
+ * the state and contiguous DEVICE buffers; the transport between GPUs (NCCL send/recv, peer
+ * copies) belongs to the caller.
+ *
+ * qlga_slab_configure: declare `ghost` (>= 0; 0 = not a slab) ghost layers on each side of the
+ *   slowest axis; needs extent >= 3 * ghost.  The lattice sums (qlga_observable_sums,
+ *   qlga_observables) then run over the owned layers only; the per-site maps (vorticity,
+ *   density, vortices, state read-back) still cover the whole extended slab.
+ * qlga_slab_edge_get: copy the `ghost` lowest (side 0) or highest (side 1) OWNED layers of all
+ *   10 planes to dev_out, DEVICE [10][ghost][layer sites] complex.  Asynchronous on the stream.
+ * qlga_slab_ghost_set: overwrite the low (side 0) or high (side 1) GHOST layers from dev_in
+ *   (same layout).  Asynchronous on the stream.
+ * Errors: QLGA_EINVAL (bad side / ghost, NULL), QLGA_ESTATE (no state, or not a slab). */
+qlga_status qlga_slab_configure(qlga_ctx*, int64_t ghost);
+qlga_status qlga_slab_edge_get(qlga_ctx*, int side, void* dev_out);
+qlga_status qlga_slab_ghost_set(qlga_ctx*, int side, const void* dev_in);
+
+/* The additive lattice sums behind qlga_observables, so that slabs can be added up before the
+ * derived quantities are formed: host_sums HOST [QLGA_NSUMS] =
+ *   n_m[5], sum|q|^2, F_x, F_y, F_z, Re A00, Im A00, sum|A00|^2, e_kin, sum rho^2, sum|F|^2,
+ *   Re<psi(t)|psi(t-tau)>, Im<psi(t)|psi(t-tau)>  (the last two are NaN without a previous state).
+ * Synchronises the stream.  qlga_observables_from_sums forms the qlga_obs record from such
+ * sums (of one context or added over slabs); it launches nothing. */
+#define QLGA_NSUMS 17
+qlga_status qlga_observable_sums(qlga_ctx*, double* host_sums);
+qlga_status qlga_observables_from_sums(const qlga_ctx*, const double* host_sums, qlga_obs* host_out);
+
 /* Kernel timing hooks (used by bench.py for the roofline of the dominant kernel).
  * While enabled, qlga_step records a CUDA event on the caller's stream before every
  * pass kernel and one after the last; qlga_profile_read synchronises the stream,

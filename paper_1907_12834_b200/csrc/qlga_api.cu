@@ -484,19 +484,31 @@ extern "C" qlga_status qlga_step(qlga_ctx* c, int64_t n) {
 // ---------------------------------------------------------------------------
 // diagnostics
 // ---------------------------------------------------------------------------
-extern "C" qlga_status qlga_observables(qlga_ctx* c, qlga_obs* out) {
-    if (!c || !out) return c ? fail(c, QLGA_EINVAL, "qlga_observables: NULL") : QLGA_EINVAL;
-    if (!c->have_state) return fail(c, QLGA_ESTATE, "qlga_observables: no state set");
+// extent of the slowest axis (the one a slab decomposition cuts) and sites per layer of it
+static int64_t slow_extent(const qlga_ctx* c) { return c->ndim == 1 ? c->nx : (c->ndim == 2 ? c->ny : c->nz); }
+static int64_t layer_sites(const qlga_ctx* c) { return nsites(c) / slow_extent(c); }
+
+extern "C" qlga_status qlga_observable_sums(qlga_ctx* c, double* host_sums) {
+    if (!c || !host_sums) return c ? fail(c, QLGA_EINVAL, "qlga_observable_sums: NULL") : QLGA_EINVAL;
+    if (!c->have_state) return fail(c, QLGA_ESTATE, "qlga_observable_sums: no state set");
     Launch L{c->stream, &c->launches};
     const void* prev = (c->prev >= 0) ? c->buf[c->prev] : nullptr;
-    int64_t n = nsites(c);
+    const int64_t r0 = c->ghost * layer_sites(c), r1 = nsites(c) - r0;      // owned layers
     int blocks = c->obs_blocks;
-    if ((int64_t)blocks * 256 > n) blocks = (int)((n + 255) / 256);
-    CU(c, launch_observables(L, c->prec, c->buf[c->cur], prev, c->nx, c->ny, c->nz, c->ndim,
+    if ((int64_t)blocks * 256 > r1 - r0) blocks = (int)((r1 - r0 + 255) / 256);
+    CU(c, launch_observables(L, c->prec, c->buf[c->cur], prev, c->nx, c->ny, c->nz, c->ndim, r0, r1,
                              c->d_partials, blocks, c->d_sums));
     double h[OBS_NACC];
     CU(c, cudaMemcpyAsync(h, c->d_sums, sizeof(h), cudaMemcpyDeviceToHost, c->stream));
     CU(c, cudaStreamSynchronize(c->stream));
+    for (int k = 0; k < 15; ++k) host_sums[k] = h[k];
+    host_sums[15] = prev ? h[15] : NAN;
+    host_sums[16] = prev ? h[16] : NAN;
+    return QLGA_OK;
+}
+
+extern "C" qlga_status qlga_observables_from_sums(const qlga_ctx* c, const double* h, qlga_obs* out) {
+    if (!c || !h || !out) return QLGA_EINVAL;
     double npsi = 0.0;
     for (int j = 0; j < 5; ++j) { out->n_m[j] = h[j]; npsi += h[j]; }
     out->norm_psi = npsi; out->norm_q = h[5];
@@ -507,14 +519,59 @@ extern "C" qlga_status qlga_observables(qlga_ctx* c, qlga_obs* out) {
     out->e_c1 = 0.5 * c->c[1] * h[14];
     out->e_c2 = 0.5 * c->c[2] * h[11];
     out->e_total = out->e_kin + out->e_c0 + out->e_c1 + out->e_c2;
-    if (prev) {   // i (N - O)/N with O = <psi|psi_prev>:  re = Im(O)/N, im = (N - Re(O))/N
-        out->e_dt_re = h[16] / npsi;
-        out->e_dt_im = (npsi - h[15]) / npsi;
-    } else {
-        out->e_dt_re = NAN; out->e_dt_im = NAN;
-    }
+    // eq. (85): i (N - O)/N with O = <psi|psi_prev>:  re = Im(O)/N, im = (N - Re(O))/N
+    out->e_dt_re = h[16] / npsi;                     // NaN without a previous state
+    out->e_dt_im = (npsi - h[15]) / npsi;
     out->step = c->step;
     return QLGA_OK;
+}
+
+extern "C" qlga_status qlga_observables(qlga_ctx* c, qlga_obs* out) {
+    if (!c || !out) return c ? fail(c, QLGA_EINVAL, "qlga_observables: NULL") : QLGA_EINVAL;
+    double h[QLGA_NSUMS];
+    const qlga_status st = qlga_observable_sums(c, h);
+    if (st != QLGA_OK) return st;
+    return qlga_observables_from_sums(c, h, out);
+}
+
+// ---- slab decomposition: ghost / edge layers of the slowest axis ------------------------------
+extern "C" qlga_status qlga_slab_configure(qlga_ctx* c, int64_t ghost) {
+    if (!c) return QLGA_EINVAL;
+    if (ghost < 0 || 3 * ghost > slow_extent(c))
+        return fail(c, QLGA_EINVAL, "qlga_slab_configure: need 0 <= 3 * ghost <= extent of the slowest axis");
+    c->ghost = ghost;
+    return QLGA_OK;
+}
+
+// copies `ghost` consecutive layers starting at layer `first` of all 10 planes between the
+// current state and a packed [10][ghost][layer] buffer: one strided copy (10 rows of
+// ghost * layer contiguous elements, pitch = one plane)
+static qlga_status slab_copy(qlga_ctx* c, const char* what, int64_t first, void* packed, bool to_packed) {
+    const size_t elem = 2 * real_size(c->prec);
+    const size_t width = (size_t)c->ghost * layer_sites(c) * elem;
+    const size_t pitch = (size_t)nsites(c) * elem;
+    char* st = (char*)c->buf[c->cur] + (size_t)first * layer_sites(c) * elem;
+    cudaError_t e = to_packed
+        ? cudaMemcpy2DAsync(packed, width, st, pitch, width, 10, cudaMemcpyDeviceToDevice, c->stream)
+        : cudaMemcpy2DAsync(st, pitch, packed, width, width, 10, cudaMemcpyDeviceToDevice, c->stream);
+    if (e != cudaSuccess) return cuda_fail(c, what, e);
+    return QLGA_OK;
+}
+
+extern "C" qlga_status qlga_slab_edge_get(qlga_ctx* c, int side, void* dev_out) {
+    if (!c || !dev_out || (side != 0 && side != 1))
+        return c ? fail(c, QLGA_EINVAL, "qlga_slab_edge_get: bad arguments") : QLGA_EINVAL;
+    if (!c->have_state || c->ghost <= 0) return fail(c, QLGA_ESTATE, "qlga_slab_edge_get: no state, or not a slab");
+    const int64_t first = side == 0 ? c->ghost : slow_extent(c) - 2 * c->ghost;
+    return slab_copy(c, "qlga_slab_edge_get", first, dev_out, true);
+}
+
+extern "C" qlga_status qlga_slab_ghost_set(qlga_ctx* c, int side, const void* dev_in) {
+    if (!c || !dev_in || (side != 0 && side != 1))
+        return c ? fail(c, QLGA_EINVAL, "qlga_slab_ghost_set: bad arguments") : QLGA_EINVAL;
+    if (!c->have_state || c->ghost <= 0) return fail(c, QLGA_ESTATE, "qlga_slab_ghost_set: no state, or not a slab");
+    const int64_t first = side == 0 ? 0 : slow_extent(c) - c->ghost;
+    return slab_copy(c, "qlga_slab_ghost_set", first, const_cast<void*>(dev_in), false);
 }
 
 extern "C" qlga_status qlga_vorticity(qlga_ctx* c, void* omega, int dst_on_device) {

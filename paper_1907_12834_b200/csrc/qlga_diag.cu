@@ -31,7 +31,8 @@ template <typename T>
 __global__ void __launch_bounds__(256) observables_kernel(const typename vec2<T>::type* q,
                                                           const typename vec2<T>::type* qprev,
                                                           int64_t nx, int64_t ny, int64_t nz, int ndim,
-                                                          double* partials) {
+                                                          int64_t r0, int64_t r1, double* partials) {
+    // sums over the sites r0 <= r < r1 (the owned layers of a slab, else the whole lattice)
     const int64_t n = nx * ny * nz;
     double acc[OBS_NACC];
 #pragma unroll
@@ -39,7 +40,7 @@ __global__ void __launch_bounds__(256) observables_kernel(const typename vec2<T>
     const double rt6 = 2.4494897427831780981972840747059;
     const double irt5 = 0.44721359549995793928183473374626;
 
-    for (int64_t r = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; r < n;
+    for (int64_t r = r0 + (int64_t)blockIdx.x * blockDim.x + threadIdx.x; r < r1;
          r += (int64_t)gridDim.x * blockDim.x) {
         double pr[5], pi[5], nq;
         load_psi<T>(q, n, r, pr, pi, &nq);
@@ -127,14 +128,14 @@ __global__ void __launch_bounds__(256) reduce_partials_kernel(const double* part
 }
 
 cudaError_t launch_observables(const Launch& L, qlga_prec prec, const void* q, const void* qprev,
-                               int64_t nx, int64_t ny, int64_t nz, int ndim, double* partials, int nblocks,
-                               double* sums) {
+                               int64_t nx, int64_t ny, int64_t nz, int ndim, int64_t r0, int64_t r1,
+                               double* partials, int nblocks, double* sums) {
     if (prec == QLGA_F64)
         observables_kernel<double><<<nblocks, 256, 0, L.stream>>>((const double2*)q, (const double2*)qprev,
-                                                                   nx, ny, nz, ndim, partials);
+                                                                   nx, ny, nz, ndim, r0, r1, partials);
     else
         observables_kernel<float><<<nblocks, 256, 0, L.stream>>>((const float2*)q, (const float2*)qprev,
-                                                                  nx, ny, nz, ndim, partials);
+                                                                  nx, ny, nz, ndim, r0, r1, partials);
     ++*L.counter;
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return e;

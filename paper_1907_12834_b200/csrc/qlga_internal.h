@@ -44,8 +44,8 @@ cudaError_t launch_kinetic(const Launch& L, qlga_prec prec, const void* src, voi
 // diagnostics and state conversion (qlga_diag.cu)
 constexpr int OBS_NACC = 19;   // accumulators per block, see qlga_diag.cu
 cudaError_t launch_observables(const Launch& L, qlga_prec prec, const void* q, const void* qprev,
-                               int64_t nx, int64_t ny, int64_t nz, int ndim, double* partials, int nblocks,
-                               double* sums);
+                               int64_t nx, int64_t ny, int64_t nz, int ndim, int64_t r0, int64_t r1,
+                               double* partials, int nblocks, double* sums);
 cudaError_t launch_vorticity(const Launch& L, qlga_prec prec, const void* q, void* omega,
                              int64_t nx, int64_t ny);
 cudaError_t launch_density(const Launch& L, qlga_prec prec, const void* q, void* rho, int64_t nsites);
@@ -72,6 +72,7 @@ struct qlga_ctx {
     int cur;               // index of the buffer holding the current state
     int prev;              // index of the buffer holding the previous step's state, or -1
     int have_state;
+    int64_t ghost;         // slab decomposition: ghost layers on each side of the slowest axis (0 = none)
     int64_t step;
     int64_t launches;
     // options

@@ -26,7 +26,10 @@ ABI_SYMBOLS = (
     "qlga_launch_count", "qlga_last_error", "qlga_destroy", "qlga_version",
     "qlga_profile_enable", "qlga_profile_read", "qlga_exp_polynomial",
     "qlga_density", "qlga_density_l2_error", "qlga_vortices",
+    "qlga_slab_configure", "qlga_slab_edge_get", "qlga_slab_ghost_set",
+    "qlga_observable_sums", "qlga_observables_from_sums",
 )
+NSUMS = 17
 
 
 class QlgaObs(ctypes.Structure):
@@ -84,6 +87,16 @@ def load_library():
     lib.qlga_density_l2_error.restype = I
     lib.qlga_vortices.argtypes = [P, P, I64, ctypes.POINTER(I64)]
     lib.qlga_vortices.restype = I
+    lib.qlga_slab_configure.argtypes = [P, I64]
+    lib.qlga_slab_configure.restype = I
+    lib.qlga_slab_edge_get.argtypes = [P, I, P]
+    lib.qlga_slab_edge_get.restype = I
+    lib.qlga_slab_ghost_set.argtypes = [P, I, P]
+    lib.qlga_slab_ghost_set.restype = I
+    lib.qlga_observable_sums.argtypes = [P, ctypes.POINTER(D)]
+    lib.qlga_observable_sums.restype = I
+    lib.qlga_observables_from_sums.argtypes = [P, ctypes.POINTER(D), ctypes.POINTER(QlgaObs)]
+    lib.qlga_observables_from_sums.restype = I
     lib.qlga_exp_polynomial.argtypes = [I, I, ctypes.POINTER(D), ctypes.POINTER(D), ctypes.POINTER(D)]
     lib.qlga_exp_polynomial.restype = I
     lib.qlga_version.argtypes = []
@@ -221,14 +234,42 @@ class Qlga:
     def step(self, n=1):
         self._check(_lib.qlga_step(self.ctx, int(n)))
 
-    def observables(self):
-        ob = QlgaObs()
-        self._check(_lib.qlga_observables(self.ctx, ctypes.byref(ob)))
+    @staticmethod
+    def _obs_dict(ob):
         return {"n_p2": ob.n_m[0], "n_p1": ob.n_m[1], "n_0": ob.n_m[2], "n_m1": ob.n_m[3], "n_m2": ob.n_m[4],
                 "norm_psi": ob.norm_psi, "norm_q": ob.norm_q, "F_x": ob.F[0], "F_y": ob.F[1], "F_z": ob.F[2],
                 "A00_re": ob.A00_re, "A00_im": ob.A00_im, "A00_abs2": ob.A00_abs2, "e_kin": ob.e_kin,
                 "e_c0": ob.e_c0, "e_c1": ob.e_c1, "e_c2": ob.e_c2, "e_total": ob.e_total,
                 "e_dt_re": ob.e_dt_re, "e_dt_im": ob.e_dt_im, "step": ob.step}
+
+    def observables(self):
+        ob = QlgaObs()
+        self._check(_lib.qlga_observables(self.ctx, ctypes.byref(ob)))
+        return self._obs_dict(ob)
+
+    def observable_sums(self):
+        """The NSUMS additive lattice sums behind observables() (owned layers of a slab)."""
+        h = (ctypes.c_double * NSUMS)()
+        self._check(_lib.qlga_observable_sums(self.ctx, h))
+        return np.array(h, dtype=np.float64)
+
+    def observables_from_sums(self, sums):
+        h = (ctypes.c_double * NSUMS)(*[float(v) for v in sums])
+        ob = QlgaObs()
+        self._check(_lib.qlga_observables_from_sums(self.ctx, h, ctypes.byref(ob)))
+        return self._obs_dict(ob)
+
+    # -- slab decomposition (include/qlga.h "Slab decomposition"; driver in slab.py) --------
+    def slab_configure(self, ghost):
+        self._check(_lib.qlga_slab_configure(self.ctx, int(ghost)))
+
+    def slab_edge_get(self, side, dev_out):
+        assert dev_out.is_cuda and dev_out.is_contiguous()
+        self._check(_lib.qlga_slab_edge_get(self.ctx, int(side), dev_out.data_ptr()))
+
+    def slab_ghost_set(self, side, dev_in):
+        assert dev_in.is_cuda and dev_in.is_contiguous()
+        self._check(_lib.qlga_slab_ghost_set(self.ctx, int(side), dev_in.data_ptr()))
 
     def vorticity(self, out=None):
         if out is None:
