@@ -63,6 +63,10 @@ def parse_args():
     ap.add_argument("--threads-y", type=int, default=0)
     ap.add_argument("--steps-per-launch", type=int, default=0, help="QLGA_OPT_STEPS_PER_LAUNCH (1D)")
     ap.add_argument("--tol-log2", type=int, default=0, help="QLGA_OPT_EXP_TOL_LOG2 override (experiments only)")
+    ap.add_argument("--slab", action="store_true",
+                    help="one lattice cut into slabs along its slowest axis, one slab per GPU, 4-layer halo exchange "
+                         "per step (paper_1907_12834_b200/slab.py); weak scaling: every rank owns the workload's lattice "
+                         "of a lattice N times as long.  Default is independent replicas (DESIGN.md section 11)")
     return ap.parse_args()
 
 
@@ -305,7 +309,10 @@ def main():
               "per_bench_step": f"{inner} time steps + 1 observables reduction" + (" + 1 vorticity map" if ndim == 2 else ""),
               "l2_policy": "state (%.1f GB per buffer) larger than the 126 MB L2" % (sites * 160 / 1e9 * (1 if args.precision == 'f64' else 0.5))
                            if sites * 80 > 126e6 else "state fits in L2 (latency-bound workload; no HBM claim)",
-              "parallelism": f"replicas x{args.gpus} (one lattice per GPU, no data-path collective)"}
+              "parallelism": (f"slabs x{args.gpus} of one lattice {args.gpus} times as long along its slowest axis, "
+                              "ring exchange of 4 ghost layers per side per time step (NCCL P2P; device copy at N=1)"
+                              if args.slab else
+                              f"replicas x{args.gpus} (one lattice per GPU, no data-path collective)")}
     if args.impl == "reference":
         run_reference(args, w, ndim, config)
         return
@@ -335,7 +342,21 @@ def main():
     del half
     out_host = torch.empty_like(q_host, pin_memory=True) if not args.no_e2e else None
 
-    sim = qlga.Qlga(ndim, w.dims, w.couplings, order=args.order, precision=args.precision, device=dev)
+    ss = None
+    if args.slab:
+        # every rank owns the workload's lattice; the global lattice is that tile repeated along the slab
+        # axis (continuous: the tile is periodic), so the extended slab is the tile plus its own wrap
+        from paper_1907_12834_b200 import slab
+        args.no_e2e = True
+        gdims = tuple(w.dims[:ndim - 1]) + (w.dims[ndim - 1] * world,)
+        ss = slab.SlabQlga(ndim, gdims, w.couplings, order=args.order, precision=args.precision,
+                           rank=rank, world=world, device=dev)
+        sim = ss.sim
+        n_own = w.dims[ndim - 1]
+        ext = (np.arange(-slab.GHOST, n_own + slab.GHOST)) % n_own
+        q_ext = np.ascontiguousarray(np.take(q_host.numpy(), ext, axis=-ndim))
+    else:
+        sim = qlga.Qlga(ndim, w.dims, w.couplings, order=args.order, precision=args.precision, device=dev)
     if args.tile_y:
         sim.set_option(qlga.OPT_TILE_Y, args.tile_y)
     if args.threads_x:
@@ -346,20 +367,24 @@ def main():
         sim.set_option(qlga.OPT_STEPS_PER_LAUNCH, args.steps_per_launch)
     if args.tol_log2:
         sim.set_option(qlga.OPT_EXP_TOL_LOG2, args.tol_log2)
-    omega_dev = (torch.empty((5, ny, nx), dtype=torch.float64 if args.precision == "f64" else torch.float32,
+    omega_dev = (torch.empty((5, sim.ny, nx), dtype=torch.float64 if args.precision == "f64" else torch.float32,
                              device=dev) if ndim == 2 else None)
     state_bytes = q_host.numel() * q_host.element_size()
 
     def hot_path_step():
-        sim.step(inner)
-        obs = sim.observables()
+        if ss is not None:
+            ss.step(inner)                   # inner x (library step on the extended slab + halo exchange)
+            obs = ss.observables()           # owned-layer sums, all-reduced over the slabs
+        else:
+            sim.step(inner)
+            obs = sim.observables()
         if omega_dev is not None:
             sim.vorticity(omega_dev)
         return obs
 
     # ---- device-resident measurement -------------------------------------------------
-    sim.set_state_q(q_host.numpy())
-    obs0 = sim.observables()
+    sim.set_state_q(q_ext if ss is not None else q_host.numpy())
+    obs0 = ss.observables() if ss is not None else sim.observables()
     for _ in range(max(3, args.warmup)):
         hot_path_step()
     sim.profile_enable(True)
@@ -487,6 +512,11 @@ def main():
             "pass_kernel_share_of_step": pass_ms / ms if ms > 0 else None,
             "norm_q_drift": obs["norm_q"] / obs0["norm_q"] - 1.0,
             "sim_step": obs["step"]}
+    if ss is not None:
+        halo = 2 * ss.edge_lo.numel() * ss.edge_lo.element_size()
+        line["slab"] = {"ghost_layers": 4, "owned_layers": int(w.dims[ndim - 1]),
+                        "halo_bytes_sent_per_rank_per_time_step": halo,
+                        "transport": "torch.distributed P2P (NCCL)" if world > 1 else "device copy (one slab, its own wrap)"}
     print(json.dumps(line))
 
 
