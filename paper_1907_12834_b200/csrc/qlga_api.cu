@@ -435,10 +435,16 @@ static qlga_status step_fused(qlga_ctx* c, int64_t nsteps) {
             // U is the rightmost operator of the plain step: it rides on the first pass
             P.umode = inter ? 2 : (d == c->ndim - 1 ? 1 : 0);
             prof_mark(c, d == 0 ? 0 : 1);
-            // strided passes: measured defaults -- 2D: one column per CTA; 3D (fp64): two columns,
-            // i.e. whole 32-byte sectors, which the page-crossing z lines need (+12 % at 512^3)
+            // strided passes, measured defaults.  Interleaved (FP-pipe bound): the kernel's own (fp64 one
+            // column x 128 rows, fp32 two x 64); 3D fp64: two columns, i.e. whole 32-byte sectors, which the
+            // page-crossing z lines need (+12 % at 512^3).  Plain ordering (one U per step or none: the
+            // memory phases count): whole sectors again -- fp64 two columns x 64 rows (8192^2: 8.8 ms
+            // against 12.2 for one column), fp32 four x 64 (5.4 against 5.9 ms)
             int cxw = c->tile_y, thr = c->threads_y;
-            if (d > 0 && cxw == 0 && c->ndim == 3 && c->prec == QLGA_F64) { cxw = 2; if (thr == 0) thr = 128; }
+            if (d > 0 && cxw == 0) {
+                if (!inter) { cxw = c->prec == QLGA_F64 ? 2 : 4; if (thr == 0) thr = c->prec == QLGA_F64 ? 128 : 256; }
+                else if (c->ndim == 3 && c->prec == QLGA_F64) { cxw = 2; if (thr == 0) thr = 128; }
+            }
             CU(c, launch_pass(L, c->prec, d, P, d == 0 ? c->threads_x : thr, d == 0 ? 1 : cxw));
             src = dst;
         }

@@ -457,3 +457,23 @@ def test_3d_fp32_observables_density_and_previous_state(qlga, oracle):
             sim.vorticity()
         assert e.value.status == qlga.QLGA_EUNSUP
         sim.close()
+
+
+def test_dispersion_relation_of_kicked_solitons_fig5(qlga, oracle):
+    # SURVEY.md 8(f) row 4 / Fig. 5: energies of kicked solitons measured with
+    # eq. (85) on the CUDA path follow E = p^2 - k^2 (eq. 74) and E = p^2 + 2 k^2,
+    # and agree with the oracle's eq. (85) on the same input.
+    from paper_1907_12834_b200 import dispersion
+    L, k = 1024, 1.0 / 16
+    for kind, row, c in (("bright", 3, (-1.0, -0.5, 0.2)), ("dark", 5, (1.0, 0.3, -0.1))):
+        es = []
+        for n in (0, 4, 8):
+            p = 2 * np.pi * n / L
+            e = dispersion.measured_energy(kind, row, c, L, k, n, steps=21)
+            es.append(e)
+            assert abs(e - dispersion.predicted_energy(kind, k, p)) < 0.02 * (p * p + k * k), (kind, n)
+            q0 = oracle.split_psi(dispersion.kicked_soliton(kind, row, c, L, k, n))
+            qa = oracle.step(q0, 1, c, 1, 20)
+            qb = oracle.step(qa, 1, c, 1, 1)
+            assert e == pytest.approx(oracle.observables(qb, 1, c, qprev=qa)["e_dt_re"], rel=1e-9, abs=1e-14)
+        assert es[0] < es[1] < es[2]                       # parabolic in p
