@@ -84,13 +84,25 @@ __device__ __forceinline__ void factor(Site<T>& s, const PassArgs<T>& P, int f, 
 #ifndef QLGA_MINB128
 #define QLGA_MINB128 3
 #endif
+// fp32 is latency bound at 4 CTAs per SM (ncu: FMA pipe 62 %, issue 67 % busy): a few spilled
+// words buy 5 (strided passes) / 6 (x pass) CTAs per SM: 8192^2 interleaved 3.90 -> 4.2 GSUP/s
+#ifndef QLGA_MINB128_F32
+#define QLGA_MINB128_F32 5
+#endif
+#ifndef QLGA_MINB_NOU
+#define QLGA_MINB_NOU 4
+#endif
+#ifndef QLGA_MINB128_F32X
+#define QLGA_MINB128_F32X 6
+#endif
 
 // HASU = false: a pass without any interaction (the plain ordering's later passes): the same
 // kernel minus the interaction code, a third of the registers, so more CTAs per SM keep the
 // HBM pipe full (this pass is memory-bound).
 template <typename T, int DIR, int CX, int NT, bool HASU>
-__global__ void __launch_bounds__(NT, (HASU ? (NT >= 192 ? 2 : (NT >= 128 ? QLGA_MINB128 : (NT >= 96 ? 4 : 6)))
-                                            : (NT >= 192 ? 2 : 4)))
+__global__ void __launch_bounds__(NT, (HASU ? (NT >= 192 ? 2 : (NT >= 128 ? (sizeof(T) == 8 ? QLGA_MINB128 : (DIR == 0 ? QLGA_MINB128_F32X : QLGA_MINB128_F32))
+                                                                         : (NT >= 96 ? 4 : 6)))
+                                            : (NT >= 192 ? 2 : QLGA_MINB_NOU)))
 pass_kernel(const __grid_constant__ PassArgs<T> P) {
     using V = typename vec2<T>::type;
     constexpr int TS = NT / CX;              // sites per line handled by the CTA
