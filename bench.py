@@ -80,8 +80,8 @@ def load_traffic(workload, precision, order):
         with open(path) as f:
             for row in csv.DictReader(f):
                 if (row["workload"], row["precision"], row["order"]) == (workload, precision, order):
-                    out[row["kernel"]] = (float(row["dram_bytes_per_launch"]),
-                                          float(row["fp_thread_instr_per_site_per_launch"]))
+                    fpi = row["fp_thread_instr_per_site_per_launch"]
+                    out[row["kernel"]] = (float(row["dram_bytes_per_launch"]), float(fpi) if fpi else None)
     return out
 
 
