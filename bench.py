@@ -154,15 +154,17 @@ def bytes_per_site_update(precision):
     return 320.0 if precision == "f64" else 160.0
 
 
-def fp_instr_per_site_update(ndim, order, degree):
+def fp_instr_per_site_update(ndim, order, degree, precision="f64"):
     """FP instructions (FMA/ADD/MUL, one per lane) per site-update of the fused step,
-    counted from qlga_math.cuh: one U of polynomial degree p
-    costs about 200 + 156 p (densities and spin 52, spin gauge 59, scalar phase 49, output 40;
-    per Horner stage and spinor vector 68 + 10), one kinetic factor 40, the final scaling 20
-    per pass."""
+    counted from qlga_math.cuh: one U of polynomial degree p costs
+    180 + 156 p in fp64 (densities and spin 52, spin gauge 59, scalar phase 29, output 40; per
+    Horner stage and spinor vector 68 + 10) and 120 + 196 p in fp32 (no gauge: 88 + 10 per stage),
+    one kinetic factor 40, the final scaling 20 per pass.  ncu at config 5 (fp64): 7860 per
+    site-update without the halo recompute; this model gives 7800 at the mean degree 4.85."""
     n_fac = 4 * ndim
     n_u = n_fac if order == "interleaved" else 1
-    return n_u * (200.0 + 156.0 * degree) + n_fac * 40.0 + 20.0 * ndim
+    per_u = (180.0 + 156.0 * degree) if precision == "f64" else (120.0 + 196.0 * degree)
+    return n_u * per_u + n_fac * 40.0 + 20.0 * ndim
 
 
 def expected_degree(w, ndim, order, precision):
@@ -186,7 +188,7 @@ def expected_degree(w, ndim, order, precision):
     deg = np.ones_like(theta)
     for p in range(1, 12):
         deg += theta * 1.001 > qlga.exp_polynomial(tol_log2, p)[0]
-    return float(np.percentile(deg, 90))
+    return float(np.mean(deg))
 
 
 # ---------------------------------------------------------------------------
@@ -473,7 +475,7 @@ def main():
         per_step = 1 if dom == "x_pass" else max(1, ndim - 1)  # the y_pass timer covers the y and z passes
         units = sites * inner * args.steps * per_step / (ndim * dn)      # site-updates per launch
         deg = expected_degree(w, ndim, args.order, args.precision)
-        fpi = fp_instr_per_site_update(ndim, args.order, deg)
+        fpi = fp_instr_per_site_update(ndim, args.order, deg, args.precision)
         lanes = 64 if args.precision == "f64" else 128       # FP64 / FP32 FMA lanes per SM per clock
         clk = (clocks.get("sm_mhz") or sm_max) * 1e6
         alu_peak = 148 * lanes * clk / 1e12                  # T instr/s at the clock seen under load
@@ -488,7 +490,7 @@ def main():
         roof_alu = {"bound": "alu", "achieved": alu_ach, "peak": alu_peak, "unit": "Tinstr/s",
                     "frac": alu_ach / alu_peak, "traffic": traffic, "kernel": dom,
                     "ms_per_launch": per_launch_ms,
-                    "model": f"{fpi:.0f} FP instr per site-update (degree {deg:.0f}) x {units:.3g} site-updates per launch; "
+                    "model": f"{fpi:.0f} FP instr per site-update (mean degree {deg:.2f}) x {units:.3g} site-updates per launch; "
                              f"peak = 148 SMs x {lanes} lanes x {clk / 1e6:.0f} MHz (median clock under load)"}
         # the binding roofline is the one with the larger fraction
         roof = roof_alu if roof_alu["frac"] > roof_hbm["frac"] else roof_hbm

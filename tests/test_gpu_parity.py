@@ -477,3 +477,26 @@ def test_dispersion_relation_of_kicked_solitons_fig5(qlga, oracle):
             qb = oracle.step(qa, 1, c, 1, 1)
             assert e == pytest.approx(oracle.observables(qb, 1, c, qprev=qa)["e_dt_re"], rel=1e-9, abs=1e-14)
         assert es[0] < es[1] < es[2]                       # parabolic in p
+
+
+def test_spin_gauge_degenerate_transverse_spin(qlga, oracle):
+    # The fp64 kernels evaluate U in the gauge e = F_+/|F_+| (R12b).  Cases where the
+    # transverse spin vanishes or is too small to normalise: single-channel and (m, -m) states
+    # (F_+ = 0 exactly), amplitudes whose |F_+|^2 falls below the 1e-36 cut-off, and a state that
+    # mixes sites of both kinds inside one warp.
+    c = (1.0, 0.3, -0.1)
+    L = 96
+    rng = np.random.default_rng(77)
+    base = inputs.random_spinor_state((L, 1), seed=31, amplitude=0.1)
+    only2 = np.zeros_like(base); only2[0] = base[0]                       # m = +2 only
+    pair = np.zeros_like(base); pair[0] = base[0]; pair[4] = base[4]      # m = +2 and -2: F_+ = 0, A00 != 0
+    tiny = base * 1e-10                                                   # |F_+|^2 ~ 1e-42 < 1e-36
+    mixed = base.copy(); mixed[1:4, :, :, ::2] = 0.0                      # every other site has F_+ = 0
+    for name, q0 in (("only2", only2), ("pair", pair), ("tiny", tiny), ("mixed", mixed)):
+        for order in ("plain", "interleaved"):
+            ref = oracle.step(q0, 1, c, ORDERS[order], 6)
+            assert rel_l2(run_gpu(qlga, q0, 1, c, order, 6), ref) < TOL64, (name, order)
+    q2 = inputs.random_spinor_state((24, 20), seed=32, amplitude=0.1)
+    q2[1:4, :, ::3, :] = 0.0
+    ref = oracle.step(q2, 2, c, 1, 4)
+    assert rel_l2(run_gpu(qlga, q2, 2, c, "interleaved", 4), ref) < TOL64
