@@ -199,6 +199,10 @@ qlga_status qlga_profile_read(qlga_ctx*, qlga_profile* host_out);
  * the Chebyshev-economised Taylor polynomial of degree p, valid for ||s K|| <= *theta_max within
  * 2^tol_log2.  p = 1..12.  Exposed so that the table can be tested on the CPU. */
 qlga_status qlga_exp_polynomial(int tol_log2, int p, double* theta_max, double* b0, double* r);
+/* The degree the kernels pick for a (warp-uniform) angle theta <= min(theta_max of degree 12, 1/2): a table
+ * lookup on the exponent and the top four mantissa bits of theta as a float, whose entry serves the upper
+ * edge of its bucket -- never below "smallest p with theta <= theta_max(p)", at most one above (host only). */
+qlga_status qlga_exp_degree(int tol_log2, double theta, int* p);
 
 /* Number of kernels this context has launched so far (for bench.py's gpu_launches). */
 int64_t qlga_launch_count(const qlga_ctx*);

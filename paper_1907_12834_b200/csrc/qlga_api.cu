@@ -95,6 +95,15 @@ static void build_exp_table(ExpTable& tab, int tol_log2) {
     }
     const double top = tab.thr[QLGA_PMAX - 1];
     tab.theta_split = (float)(top < 0.5 ? top : 0.5);
+    // degree lookup table: bucket k holds the angles whose float bits >> 19 equal QLGA_LUT_BASE + k
+    for (int k = 0; k < QLGA_LUT_N; ++k) {
+        const uint32_t next = (uint32_t)(QLGA_LUT_BASE + k + 1) << 19;      // first float of the next bucket
+        float upper;
+        memcpy(&upper, &next, sizeof(upper));
+        int p = 1;
+        for (int j = 0; j < QLGA_PMAX; ++j) p += (upper > tab.thr[j]) ? 1 : 0;
+        tab.plut[k] = (unsigned char)(p > QLGA_PMAX ? QLGA_PMAX : p);        // theta <= theta_split <= thr[PMAX-1]
+    }
     // Taylor coefficients of the scalar phase (qlga_math.cuh, sincos_small)
     long double f = 1.0L;                                  // running factorial
     for (int k = 0; k < 7; ++k) {
@@ -119,6 +128,21 @@ extern "C" qlga_status qlga_exp_polynomial(int tol_log2, int p, double* theta_ma
     *theta_max = tab.thr[p - 1];
     *b0 = tab.b0[p - 1];
     for (int k = 0; k <= p; ++k) r[k] = tab.r[p - 1][k];
+    return QLGA_OK;
+}
+
+// The degree the kernels' lookup table gives for a warp-uniform angle theta (host only).
+extern "C" qlga_status qlga_exp_degree(int tol_log2, double theta, int* p) {
+    if (tol_log2 > -8 || tol_log2 < -100 || !p || !(theta >= 0.0)) return QLGA_EINVAL;
+    static ExpTable tab;
+    build_exp_table(tab, tol_log2);
+    if (theta > tab.theta_split) return QLGA_EINVAL;          // the kernels split such angles first
+    const float th = (float)theta;
+    uint32_t bits;
+    memcpy(&bits, &th, sizeof(bits));
+    int k = (int)(bits >> 19) - QLGA_LUT_BASE;
+    k = k < 0 ? 0 : (k > QLGA_LUT_N - 1 ? QLGA_LUT_N - 1 : k);
+    *p = tab.plut[k];
     return QLGA_OK;
 }
 

@@ -199,6 +199,8 @@ __device__ __forceinline__ void kin_update(Site<T>& s, int sigma, const cx<T> Fw
 // thr[p-1] = largest angle for which a degree-p polynomial meets the tolerance.
 // ---------------------------------------------------------------------------
 constexpr int QLGA_PMAX = 12;
+constexpr int QLGA_LUT_BASE = 83 * 16;      // theta = 2^-44: below it degree 1 serves every tolerance in use
+constexpr int QLGA_LUT_N = 44 * 16;         // up to theta = 1 (theta_split <= 1/2 ends the table's use)
 
 template <typename T> struct UConst {
     T g0, g1, g2;
@@ -215,6 +217,10 @@ struct ExpTable {
     float thr[QLGA_PMAX];       // thr[p-1] = largest angle degree p serves within the tolerance
     float theta_split;          // angles above this are split into equal sub-angles
     SinCosTable sc;
+    // degree by table lookup: index = (bits of theta >> 19) - QLGA_LUT_BASE, i.e. the exponent and the
+    // top four mantissa bits (buckets 4-6 % wide); the entry is the degree that serves the bucket's
+    // upper edge, so the choice is never below the rule "smallest p with theta <= thr[p-1]"
+    unsigned char plut[QLGA_LUT_N];
 };
 
 // The site's own spin gauge.  With e = F_+/|F_+| and D = diag(e^-2, e^-1, 1, e, e^2) (rows
@@ -289,6 +295,14 @@ __device__ __forceinline__ int count_below(const float* thr, float theta) {
 #pragma unroll
         for (int k = 0; k + w < QLGA_PMAX - 1; k += 2 * w) c[k] += c[k + w];
     return c[0];
+}
+
+// degree for a warp-uniform angle theta <= theta_split: five instructions instead of the 45 of the
+// compare tree (which the out-of-line general path still uses)
+__device__ __forceinline__ int lut_degree(const ExpTable& t, float theta) {
+    int k = (int)(__float_as_uint(theta) >> 19) - QLGA_LUT_BASE;
+    k = max(0, min(k, QLGA_LUT_N - 1));
+    return t.plut[k];
 }
 
 // Site-local coefficients of sK' (pre-scaled, see apply_sK) in the site's spin gauge.
@@ -450,7 +464,7 @@ __device__ __forceinline__ void interaction(Site<T>& s, const UConst<T>& uc, con
     }
     T sn, cs;
     sincos_small<T>(xph, tab.sc, &sn, &cs);
-    const int p = 1 + count_below(tab.thr, theta);
+    const int p = lut_degree(tab, theta);
     const T pb0 = exp_b0(tab, p, (T)0);                // constant term of the polynomial (1 - O(tol))
     cx<T> phj[5];
     gauge_phases<T>(kc, mk<T>(pb0 * cs, -(pb0 * sn)), phj);

@@ -27,7 +27,7 @@ ABI_SYMBOLS = (
     "qlga_profile_enable", "qlga_profile_read", "qlga_exp_polynomial",
     "qlga_density", "qlga_density_l2_error", "qlga_vortices",
     "qlga_slab_configure", "qlga_slab_edge_get", "qlga_slab_ghost_set",
-    "qlga_observable_sums", "qlga_observables_from_sums",
+    "qlga_observable_sums", "qlga_observables_from_sums", "qlga_exp_degree",
 )
 NSUMS = 17
 
@@ -99,6 +99,8 @@ def load_library():
     lib.qlga_observables_from_sums.restype = I
     lib.qlga_exp_polynomial.argtypes = [I, I, ctypes.POINTER(D), ctypes.POINTER(D), ctypes.POINTER(D)]
     lib.qlga_exp_polynomial.restype = I
+    lib.qlga_exp_degree.argtypes = [I, D, ctypes.POINTER(I)]
+    lib.qlga_exp_degree.restype = I
     lib.qlga_version.argtypes = []
     lib.qlga_version.restype = ctypes.c_char_p
     return lib
@@ -119,6 +121,15 @@ def exp_polynomial(tol_log2, p):
     if st != QLGA_OK:
         raise QlgaError(st, "qlga_exp_polynomial: bad arguments")
     return th.value, b0.value, list(r)
+
+
+def exp_degree(tol_log2, theta):
+    """Degree the kernels' lookup table picks for the angle theta (host only)."""
+    p = ctypes.c_int()
+    st = _lib.qlga_exp_degree(int(tol_log2), float(theta), ctypes.byref(p))
+    if st != QLGA_OK:
+        raise QlgaError(st, "qlga_exp_degree: bad arguments")
+    return p.value
 
 
 def _dims3(ndim, dims):

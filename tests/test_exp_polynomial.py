@@ -56,3 +56,25 @@ def test_bad_arguments():
     for args in ((-56, 0), (-56, 13), (-4, 3), (-200, 3)):
         with pytest.raises(qlga.QlgaError):
             qlga.exp_polynomial(*args)
+
+
+def test_degree_lookup_table_is_never_below_the_threshold_rule():
+    # the kernels pick the degree by a table lookup on the float bits of theta (qlga_exp_degree):
+    # never below "smallest p with theta <= theta_max(p)", at most one above, equal away from bucket edges
+    import numpy as np
+    from paper_1907_12834_b200 import qlga
+    rng = np.random.default_rng(5)
+    for tol in (-56, -27):
+        thr = [qlga.exp_polynomial(tol, p)[0] for p in range(1, 13)]
+        top = min(thr[-1], 0.5)
+        thetas = np.concatenate([10.0 ** rng.uniform(-15, np.log10(top), 4000),
+                                 np.array(thr[:-1]) * (1 - 1e-6), np.array(thr[:-1]) * (1 + 1e-6), [0.0, 1e-30, top]])
+        above = 0
+        for th in thetas:
+            if th > top:
+                continue
+            rule = 1 + sum(np.float32(th) > np.float32(t) for t in thr)
+            got = qlga.exp_degree(tol, float(th))
+            assert rule <= got <= min(rule + 1, 12), (tol, th, rule, got)
+            above += got > rule
+        assert above < 0.05 * len(thetas)          # buckets are 4-6 % wide: few angles pay an extra stage
