@@ -10,6 +10,7 @@
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
+#include <math.h>
 
 namespace qlga {
 
@@ -120,8 +121,13 @@ __device__ __forceinline__ double rsqrt_pos(double x) {
     }
     return y;
 }
+__device__ __forceinline__ float rsqrt_approx(float x) {       // MUFU.RSQ, 2 ulp, no special cases
+    float y;
+    asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+}
 __device__ __forceinline__ float rsqrt_pos(float x) {
-    float y = rsqrtf(x);
+    float y = rsqrt_approx(x);
     const float h = fmaf(-0.5f * x * y, y, 0.5f);
     return fmaf(y, h, y);
 }
@@ -204,7 +210,17 @@ constexpr int QLGA_LUT_N = 44 * 16;         // up to theta = 1 (theta_split <= 1
 
 template <typename T> struct UConst {
     T g0, g1, g2;
+    float tg1, tg2;             // 2|g1| and |g2| as floats, for the angle bound (no conversions per site)
 };
+template <typename T> inline UConst<T> make_uconst(double g0, double g1, double g2) {
+    UConst<T> u;
+    u.g0 = (T)g0; u.g1 = (T)g1; u.g2 = (T)g2;
+    // rounded up: the bound must not fall below the true angle
+    u.tg1 = nextafterf((float)(2.0 * fabs(g1)), INFINITY);
+    u.tg2 = nextafterf((float)fabs(g2), INFINITY);
+    return u;
+}
+
 
 struct ExpTable {
     // Horner ratios of the degree-p polynomial P_p(y) = b0 (1 + r1 y (1 + r2 y (... (1 + rp y)))),
@@ -341,8 +357,8 @@ __device__ __forceinline__ void site_coefficients(Site<T>& s, const UConst<T>& u
     // angle bound theta = 2 |g1| |F| + |g2| rho (the exact spectral norms of the two parts);
     // |F| by the approximate reciprocal square root (2 ulp; the 2^-10 margin covers it)
     const float f2 = fmaxf((float)fma(Fz, Fz, fp2), 1e-37f);
-    const float Fabs = f2 * __frsqrt_rn(f2);
-    kc.theta = (2.0f * fabsf((float)uc.g1) * Fabs + fabsf((float)uc.g2) * (float)kc.rho) * 1.0009765625f;
+    const float Fabs = f2 * rsqrt_approx(f2);
+    kc.theta = (uc.tg1 * Fabs + uc.tg2 * (float)kc.rho) * 1.0009765625f;
     kc.g2 = uc.g2;
     kc.az = uc.g1 * Fz;
     kc.az2 = kc.az + kc.az;

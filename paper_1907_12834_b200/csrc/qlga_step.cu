@@ -85,7 +85,8 @@ __device__ __forceinline__ void factor(Site<T>& s, const PassArgs<T>& P, int f, 
 #define QLGA_MINB128 3
 #endif
 // fp32 is latency bound at 4 CTAs per SM (ncu: FMA pipe 62 %, issue 67 % busy): a few spilled
-// words buy 5 (strided passes) / 6 (x pass) CTAs per SM: 8192^2 interleaved 3.90 -> 4.2 GSUP/s
+// words buy 5 CTAs per SM (96 registers): 8192^2 interleaved 3.90 -> 4.3 GSUP/s.  (6 CTAs, 80
+// registers, was faster for the x pass while it spilled 24 bytes and slower once it spilled 172.)
 #ifndef QLGA_MINB128_F32
 #define QLGA_MINB128_F32 5
 #endif
@@ -93,7 +94,7 @@ __device__ __forceinline__ void factor(Site<T>& s, const PassArgs<T>& P, int f, 
 #define QLGA_MINB_NOU 4
 #endif
 #ifndef QLGA_MINB128_F32X
-#define QLGA_MINB128_F32X 6
+#define QLGA_MINB128_F32X 5
 #endif
 
 // HASU = false: a pass without any interaction (the plain ordering's later passes): the same
@@ -189,9 +190,7 @@ static PassArgs<T> make_args(const PassParams& P, int dir) {
     A.src = (const typename vec2<T>::type*)P.src;
     A.dst = (typename vec2<T>::type*)P.dst;
     A.nx = P.nx; A.nsites = P.nx * P.ny * P.nz; A.ksteps = P.ksteps; A.umode = P.umode;
-    for (int f = 0; f < 4; ++f) {
-        A.uc[f].g0 = (T)P.g[f][0]; A.uc[f].g1 = (T)P.g[f][1]; A.uc[f].g2 = (T)P.g[f][2];
-    }
+    for (int f = 0; f < 4; ++f) A.uc[f] = make_uconst<T>(P.g[f][0], P.g[f][1], P.g[f][2]);
     A.out_scale = (T)P.out_scale;
     A.tab = P.tab;
     if (dir == 0)      { A.len = P.nx; A.stride = 1;           A.n_outer = P.ny * P.nz; A.outer_stride = P.nx; }
@@ -342,10 +341,10 @@ cudaError_t launch_interaction(const Launch& L, qlga_prec prec, void* q, int64_t
                                const double g[3], const ExpTable& tab) {
     const unsigned blocks = (unsigned)((n + 127) / 128);
     if (prec == QLGA_F64) {
-        UConst<double> uc{g[0], g[1], g[2]};
+        UConst<double> uc = make_uconst<double>(g[0], g[1], g[2]);
         interaction_kernel<double><<<blocks, 128, 0, L.stream>>>((double2*)q, n, uc, tab);
     } else {
-        UConst<float> uc{(float)g[0], (float)g[1], (float)g[2]};
+        UConst<float> uc = make_uconst<float>(g[0], g[1], g[2]);
         interaction_kernel<float><<<blocks, 128, 0, L.stream>>>((float2*)q, n, uc, tab);
     }
     ++*L.counter;
