@@ -260,7 +260,10 @@ static void expm_apply(cplx K[NM][NM], real s, cplx v[NM])
  *   W = exp(-i s H_int[psi]),   q_{.,sigma} <- W q_{.,sigma}  for sigma = 1, 2,
  * evaluated as  exp(-i s c0 rho) * exp(-i s K)  (the scalar part commutes).
  * ---------------------------------------------------------------------- */
-void orc_interaction(cplx *q, long nx, long ny, long nz, real c0, real c1, real c2, real s)
+/* With a chemical potential (section II.C: "a chemical potential term of the
+ * form mu psi_m"; eq. (75), E = mu + p^2 - k^2): H_int + mu 1, i.e. one more scalar
+ * phase exp(-i s mu).  mu = 0 is the paper's own simulations (bit-identical to the form without). */
+void orc_interaction_mu(cplx *q, long nx, long ny, long nz, real c0, real c1, real c2, real mu, real s)
 {
     long n = nx * ny * nz;
     for (long r = 0; r < n; ++r) {
@@ -269,13 +272,18 @@ void orc_interaction(cplx *q, long nx, long ny, long nz, real c0, real c1, real 
         for (int j = 0; j < NM; ++j)
             psi[j] = q[((size_t)j * NS + 0) * n + r] + q[((size_t)j * NS + 1) * n + r];
         site_K(psi, c1, c2, K, &rho);
-        cplx phase = exp(-I * (s * c0 * rho));
+        cplx phase = exp(-I * (s * c0 * rho + s * mu));
         for (int sg = 0; sg < NS; ++sg) {
             for (int j = 0; j < NM; ++j) v[j] = q[((size_t)j * NS + sg) * n + r];
             expm_apply(K, s, v);
             for (int j = 0; j < NM; ++j) q[((size_t)j * NS + sg) * n + r] = phase * v[j];
         }
     }
+}
+
+void orc_interaction(cplx *q, long nx, long ny, long nz, real c0, real c1, real c2, real s)
+{
+    orc_interaction_mu(q, nx, ny, nz, c0, c1, c2, (real)0, s);
 }
 
 /* ------------------------------------------------------------------------
@@ -286,19 +294,25 @@ void orc_interaction(cplx *q, long nx, long ny, long nz, real c0, real c1, real 
  *   x factors, U (plain) or U^{1/8} (interleaved, before every factor).
  *   3D  ("n = 12"): z factors, then y, then x; U^{1/12}.
  * ---------------------------------------------------------------------- */
-void orc_step(cplx *q, long nx, long ny, long nz, int ndim, real c0, real c1, real c2,
-              int order, long nsteps)
+void orc_step_mu(cplx *q, long nx, long ny, long nz, int ndim, real c0, real c1, real c2, real mu,
+                 int order, long nsteps)
 {
     const int nfac = 4 * ndim;
     for (long t = 0; t < nsteps; ++t) {
-        if (order == 0) orc_interaction(q, nx, ny, nz, c0, c1, c2, (real)1);
+        if (order == 0) orc_interaction_mu(q, nx, ny, nz, c0, c1, c2, mu, (real)1);
         for (int d = ndim - 1; d >= 0; --d)              /* y factors first, then x */
             for (int k = 0; k < 4; ++k) {
                 int sigma = (k < 2) ? 1 : 0;             /* component 2, 2, 1, 1 */
-                if (order == 1) orc_interaction(q, nx, ny, nz, c0, c1, c2, (real)1 / (real)nfac);
+                if (order == 1) orc_interaction_mu(q, nx, ny, nz, c0, c1, c2, mu, (real)1 / (real)nfac);
                 orc_kinetic_factor(q, nx, ny, nz, d, sigma);
             }
     }
+}
+
+void orc_step(cplx *q, long nx, long ny, long nz, int ndim, real c0, real c1, real c2,
+              int order, long nsteps)
+{
+    orc_step_mu(q, nx, ny, nz, ndim, c0, c1, c2, (real)0, order, nsteps);
 }
 
 /* ------------------------------------------------------------------------

@@ -58,7 +58,9 @@ class Oracle:
             "orc_spin_matrices": [P, P, P],
             "orc_site_hamiltonian": [P, R, R, R, P],
             "orc_interaction": [P, L, L, L, R, R, R, R],
+            "orc_interaction_mu": [P, L, L, L, R, R, R, R, R],
             "orc_step": [P, L, L, L, I, R, R, R, I, L],
+            "orc_step_mu": [P, L, L, L, I, R, R, R, R, I, L],
             "orc_observables": [P, P, L, L, L, I, R, R, R, P],
             "orc_vorticity": [P, L, L, P],
             "orc_density": [P, L, L, L, P],
@@ -143,22 +145,31 @@ class Oracle:
                                       self.creal(c2), self._p(H))
         return H
 
-    def interaction(self, q, couplings, s):
+    def interaction(self, q, couplings, s, mu=None):
+        """mu: chemical potential (eq. 75); None = the form without it."""
         q = self._c(q).copy()
         nx, ny, nz = self._dims(q)
         c0, c1, c2 = couplings
-        self.lib.orc_interaction(self._p(q), nx, ny, nz, self.creal(c0), self.creal(c1),
-                                 self.creal(c2), self.creal(s))
+        if mu is None:
+            self.lib.orc_interaction(self._p(q), nx, ny, nz, self.creal(c0), self.creal(c1),
+                                     self.creal(c2), self.creal(s))
+        else:
+            self.lib.orc_interaction_mu(self._p(q), nx, ny, nz, self.creal(c0), self.creal(c1),
+                                        self.creal(c2), self.creal(mu), self.creal(s))
         return q
 
-    def step(self, q, ndim, couplings, order, nsteps=1):
-        """order: 0 = plain (eq. 108), 1 = interleaved (eq. 112)."""
+    def step(self, q, ndim, couplings, order, nsteps=1, mu=None):
+        """order: 0 = plain (eq. 108), 1 = interleaved (eq. 112); mu: chemical potential or None."""
         q = self._c(q).copy()
         nx, ny, nz = self._dims(q)
         assert ndim in (1, 2, 3) and (ndim >= 2 or ny == 1) and (ndim == 3 or nz == 1)
         c0, c1, c2 = couplings
-        self.lib.orc_step(self._p(q), nx, ny, nz, int(ndim), self.creal(c0), self.creal(c1),
-                          self.creal(c2), int(order), int(nsteps))
+        if mu is None:
+            self.lib.orc_step(self._p(q), nx, ny, nz, int(ndim), self.creal(c0), self.creal(c1),
+                              self.creal(c2), int(order), int(nsteps))
+        else:
+            self.lib.orc_step_mu(self._p(q), nx, ny, nz, int(ndim), self.creal(c0), self.creal(c1),
+                                 self.creal(c2), self.creal(mu), int(order), int(nsteps))
         return q
 
     def observables(self, q, ndim, couplings, qprev=None):

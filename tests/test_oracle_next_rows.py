@@ -79,3 +79,47 @@ def test_winding_total_is_zero_and_plane_wave_has_none(oracle):
     circ = (wrap(np.roll(S, -1, 1) - S) + wrap(np.roll(np.roll(S, -1, 1), -1, 0) - np.roll(S, -1, 1))
             + wrap(np.roll(S, -1, 0) - np.roll(np.roll(S, -1, 1), -1, 0)) + wrap(S - np.roll(S, -1, 0)))
     assert np.array_equal(w[1], np.rint(circ / (2 * np.pi)).astype(np.int32))
+
+
+# ---- chemical potential (section II.C; eq. 75) ----
+def test_chemical_potential_is_a_global_phase_and_zero_is_the_plain_form(oracle):
+    import numpy as np
+    from paper_1907_12834_b200 import inputs
+    from conftest import rel_l2
+    c, mu = (1.0, 0.3, -0.1), 0.0375
+    for ndim, dims in ((1, (24, 1)), (2, (10, 8))):
+        q0 = inputs.random_spinor_state(dims, seed=8, amplitude=0.1)
+        for order in (0, 1):
+            ref = oracle.step(q0, ndim, c, order, 5)
+            assert np.array_equal(oracle.step(q0, ndim, c, order, 5, mu=0.0), ref)      # bit for bit
+            got = oracle.step(q0, ndim, c, order, 5, mu=mu)
+            assert rel_l2(got, np.exp(-1j * mu * 5) * ref) < 1e-14
+    one = oracle.interaction(q0, c, 0.25, mu=mu)
+    assert rel_l2(one, np.exp(-1j * mu * 0.25) * oracle.interaction(q0, c, 0.25)) < 1e-15
+
+
+def test_dispersion_with_chemical_potential_eq75(oracle):
+    # eq. (75): E = mu + p^2 - k^2 (bright): E = mu + p^2 + 2 k^2 (dark), by eq. (85)
+    import numpy as np
+    from paper_1907_12834_b200 import dispersion
+    L, k, n, mu = 512, 1.0 / 16, 4, 0.011
+    p = 2 * np.pi * n / L
+    for kind, row, c in (("bright", 3, (-1.0, -0.5, 0.2)), ("dark", 5, (1.0, 0.3, -0.1))):
+        q0 = oracle.split_psi(dispersion.kicked_soliton(kind, row, c, L, k, n))
+        qa = oracle.step(q0, 1, c, 1, 10, mu=mu)
+        qb = oracle.step(qa, 1, c, 1, 1, mu=mu)
+        e = oracle.observables(qb, 1, c, qprev=qa)["e_dt_re"]
+        want = mu + dispersion.predicted_energy(kind, k, p)
+        assert abs(e - want) < 0.02 * (p * p + k * k), (kind, e, want)
+        e0 = oracle.observables(oracle.step(qa, 1, c, 1, 1), 1, c, qprev=qa)["e_dt_re"]
+        assert abs((e - e0) - mu) < 1e-3 * mu          # the shift is mu (sin mu at this size)
+
+
+def test_uniform_table1_state_with_chemical_potential(oracle):
+    import numpy as np
+    from conftest import table1_coeffs
+    c, E, mu, n = (1.0, 0.3, -0.1), 0.002, 0.004, 25
+    cm = table1_coeffs(13, E, c)
+    psi = np.zeros((5, 1, 8), complex); psi[:, 0, :] = cm[:, None]
+    out = oracle.psi_of_q(oracle.step(oracle.split_psi(psi), 1, c, 1, n, mu=mu))
+    assert np.abs(out - np.exp(-1j * (E + mu) * n) * psi).max() < 1e-14
