@@ -119,6 +119,12 @@ qlga_status qlga_get_state_q(qlga_ctx*, void* q, int dst_on_device);
 /* Read back psi_m = q_m1 + q_m2. */
 qlga_status qlga_get_state_psi(qlga_ctx*, void* psi, int dst_on_device);
 
+/* Chemical potential term mu psi_m of the equation of motion (section II.C;
+ * dispersion relations eq. 75): H_int + mu 1, one more scalar phase
+ * exp(-i s mu) in every U^(s).  Default 0 (the paper's own simulations).  Takes effect from the next
+ * qlga_step.  QLGA_EINVAL for a non-finite value. */
+qlga_status qlga_set_chemical_potential(qlga_ctx*, double mu);
+
 /* Advance n >= 0 time steps of eq. (108)/(112).  Asynchronous on the stream. */
 qlga_status qlga_step(qlga_ctx*, int64_t n);
 

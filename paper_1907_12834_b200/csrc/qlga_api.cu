@@ -396,6 +396,7 @@ static void fill_pass_consts(const qlga_ctx* c, PassParams& P, double s) {
         P.g[f][1] = sc * c->c[1];
         P.g[f][2] = sc * c->c[2] / 5.0;
     }
+    P.smu = s * c->mu;
     P.out_scale = 0.0625;
     P.tab = c->tab;
 }
@@ -486,11 +487,11 @@ static qlga_status step_per_operator(qlga_ctx* c, int64_t nsteps) {
     const double g[3] = {s * c->c[0], s * c->c[1], s * c->c[2] / 5.0};
     for (int64_t t = 0; t < nsteps; ++t) {
         prof_mark(c, 2);
-        if (!inter) CU(c, launch_interaction(L, c->prec, c->buf[c->cur], nsites(c), g, c->tab));
+        if (!inter) CU(c, launch_interaction(L, c->prec, c->buf[c->cur], nsites(c), g, s * c->mu, c->tab));
         for (int d = c->ndim - 1; d >= 0; --d)
             for (int k = 0; k < 4; ++k) {
                 const int sigma = (k < 2) ? 1 : 0;                     // components 2, 2, 1, 1
-                if (inter) CU(c, launch_interaction(L, c->prec, c->buf[c->cur], nsites(c), g, c->tab));
+                if (inter) CU(c, launch_interaction(L, c->prec, c->buf[c->cur], nsites(c), g, s * c->mu, c->tab));
                 const int dst = pick_other(c, c->cur, -1);
                 CU(c, launch_kinetic(L, c->prec, c->buf[c->cur], c->buf[dst], c->nx, c->ny, c->nz, d, sigma));
                 c->cur = dst;
@@ -498,6 +499,13 @@ static qlga_status step_per_operator(qlga_ctx* c, int64_t nsteps) {
         c->prev = -1;
         ++c->step;
     }
+    return QLGA_OK;
+}
+
+extern "C" qlga_status qlga_set_chemical_potential(qlga_ctx* c, double mu) {
+    if (!c) return QLGA_EINVAL;
+    if (!(mu == mu) || mu - mu != 0.0) return fail(c, QLGA_EINVAL, "qlga_set_chemical_potential: not a finite value");
+    c->mu = mu;
     return QLGA_OK;
 }
 

@@ -19,6 +19,7 @@ struct PassParams {
     int umode;             // 0: no U in this pass, 1: U before the first factor of each step,
                            // 2: U before every factor
     double g[4][3];        // per factor: (s c0, s c1, s c2/5) * 4^-e  (e = deferred halvings so far)
+    double smu;            // s * mu, the chemical-potential phase of one U (not scaled: it multiplies no density)
     double out_scale;      // 2^-4, applied after the 4 factors of a step
     ExpTable tab;
 };
@@ -37,7 +38,7 @@ int max_ksteps(int threads);
 
 // one kernel per operator (reference path on the GPU)
 cudaError_t launch_interaction(const Launch& L, qlga_prec prec, void* q, int64_t nsites,
-                               const double g[3], const ExpTable& tab);
+                               const double g[3], double smu, const ExpTable& tab);
 cudaError_t launch_kinetic(const Launch& L, qlga_prec prec, const void* src, void* dst,
                            int64_t nx, int64_t ny, int64_t nz, int dir, int sigma);
 
@@ -64,6 +65,7 @@ struct qlga_ctx {
     int ndim;
     int64_t nx, ny, nz;
     double c[3];
+    double mu;             // chemical potential (0 unless qlga_set_chemical_potential)
     qlga_order order;
     qlga_prec prec;
     void* buf[3];

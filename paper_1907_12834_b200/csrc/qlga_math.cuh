@@ -210,11 +210,12 @@ constexpr int QLGA_LUT_N = 44 * 16;         // up to theta = 1 (theta_split <= 1
 
 template <typename T> struct UConst {
     T g0, g1, g2;
+    T smu;                      // s mu: chemical-potential phase of this application
     float tg1, tg2;             // 2|g1| and |g2| as floats, for the angle bound (no conversions per site)
 };
-template <typename T> inline UConst<T> make_uconst(double g0, double g1, double g2) {
+template <typename T> inline UConst<T> make_uconst(double g0, double g1, double g2, double smu) {
     UConst<T> u;
-    u.g0 = (T)g0; u.g1 = (T)g1; u.g2 = (T)g2;
+    u.g0 = (T)g0; u.g1 = (T)g1; u.g2 = (T)g2; u.smu = (T)smu;
     // rounded up: the bound must not fall below the true angle
     u.tg1 = nextafterf((float)(2.0 * fabs(g1)), INFINITY);
     u.tg2 = nextafterf((float)fabs(g2), INFINITY);
@@ -472,7 +473,7 @@ __device__ __forceinline__ void interaction(Site<T>& s, const UConst<T>& uc, con
     apply_sK(va, wa, kc.az, kc.az2, kc.a1, kc.a6, kc.g2, kc.psi);
     // warp-uniform angle (one polynomial degree per warp keeps the Horner loops convergent)
     const float theta = __uint_as_float(__reduce_max_sync(0xffffffffu, __float_as_uint(kc.theta)));
-    const T xph = uc.g0 * kc.rho;                  // scalar phase exp(-i s c0 rho)
+    const T xph = fma(uc.g0, kc.rho, uc.smu);      // scalar phase exp(-i s (c0 rho + mu))
     const bool big_phase = !__all_sync(0xffffffffu, fabs(xph) <= (T)0.0625);
     if (big_phase || theta > tab.theta_split) {
         s = interaction_general<T>(s, kc, xph, tab, theta);

@@ -190,7 +190,7 @@ static PassArgs<T> make_args(const PassParams& P, int dir) {
     A.src = (const typename vec2<T>::type*)P.src;
     A.dst = (typename vec2<T>::type*)P.dst;
     A.nx = P.nx; A.nsites = P.nx * P.ny * P.nz; A.ksteps = P.ksteps; A.umode = P.umode;
-    for (int f = 0; f < 4; ++f) A.uc[f] = make_uconst<T>(P.g[f][0], P.g[f][1], P.g[f][2]);
+    for (int f = 0; f < 4; ++f) A.uc[f] = make_uconst<T>(P.g[f][0], P.g[f][1], P.g[f][2], P.smu);
     A.out_scale = (T)P.out_scale;
     A.tab = P.tab;
     if (dir == 0)      { A.len = P.nx; A.stride = 1;           A.n_outer = P.ny * P.nz; A.outer_stride = P.nx; }
@@ -338,13 +338,13 @@ __global__ void __launch_bounds__(128) kinetic_kernel(const typename vec2<T>::ty
 }
 
 cudaError_t launch_interaction(const Launch& L, qlga_prec prec, void* q, int64_t n,
-                               const double g[3], const ExpTable& tab) {
+                               const double g[3], double smu, const ExpTable& tab) {
     const unsigned blocks = (unsigned)((n + 127) / 128);
     if (prec == QLGA_F64) {
-        UConst<double> uc = make_uconst<double>(g[0], g[1], g[2]);
+        UConst<double> uc = make_uconst<double>(g[0], g[1], g[2], smu);
         interaction_kernel<double><<<blocks, 128, 0, L.stream>>>((double2*)q, n, uc, tab);
     } else {
-        UConst<float> uc = make_uconst<float>(g[0], g[1], g[2]);
+        UConst<float> uc = make_uconst<float>(g[0], g[1], g[2], smu);
         interaction_kernel<float><<<blocks, 128, 0, L.stream>>>((float2*)q, n, uc, tab);
     }
     ++*L.counter;

@@ -27,7 +27,7 @@ ABI_SYMBOLS = (
     "qlga_profile_enable", "qlga_profile_read", "qlga_exp_polynomial",
     "qlga_density", "qlga_density_l2_error", "qlga_vortices",
     "qlga_slab_configure", "qlga_slab_edge_get", "qlga_slab_ghost_set",
-    "qlga_observable_sums", "qlga_observables_from_sums", "qlga_exp_degree",
+    "qlga_observable_sums", "qlga_observables_from_sums", "qlga_exp_degree", "qlga_set_chemical_potential",
 )
 NSUMS = 17
 
@@ -67,6 +67,8 @@ def load_library():
         fn = getattr(lib, name)
         fn.argtypes = [P, P, I]
         fn.restype = I
+    lib.qlga_set_chemical_potential.argtypes = [P, D]
+    lib.qlga_set_chemical_potential.restype = I
     lib.qlga_step.argtypes = [P, I64]
     lib.qlga_step.restype = I
     lib.qlga_observables.argtypes = [P, ctypes.POINTER(QlgaObs)]
@@ -242,6 +244,10 @@ class Qlga:
         return out
 
     # -- evolution and diagnostics -----------------------------------------
+    def set_chemical_potential(self, mu):
+        """mu psi_m term of the equation of motion (eq. 75); default 0."""
+        self._check(_lib.qlga_set_chemical_potential(self.ctx, float(mu)))
+
     def step(self, n=1):
         self._check(_lib.qlga_step(self.ctx, int(n)))
 

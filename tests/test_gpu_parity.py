@@ -500,3 +500,45 @@ def test_spin_gauge_degenerate_transverse_spin(qlga, oracle):
     q2[1:4, :, ::3, :] = 0.0
     ref = oracle.step(q2, 2, c, 1, 4)
     assert rel_l2(run_gpu(qlga, q2, 2, c, "interleaved", 4), ref) < TOL64
+
+
+def test_chemical_potential(qlga, oracle):
+    # mu psi_m term (eq. 75): parity with the oracle's orc_step_mu, both orderings,
+    # 1D with temporal blocking, 2D, fp32, the per-operator path, a phase beyond the fast path's range,
+    # and the dispersion relation E = mu + p^2 - k^2 measured with eq. (85).
+    c, mu = (1.0, 0.3, -0.1), 0.0375
+    def run(q0, ndim, order, steps, precision="f64", options=(), mu_=mu):
+        dims = tuple(reversed(q0.shape[2:]))
+        sim = qlga.Qlga(ndim, dims, c, order=order, precision=precision)
+        for k, v in options:
+            sim.set_option(k, v)
+        sim.set_chemical_potential(mu_)
+        sim.set_state_q(q0)
+        sim.step(steps)
+        out = sim.get_state_q().astype(np.complex128)
+        sim.close()
+        return out
+    q1 = inputs.random_spinor_state((300, 1), seed=41, amplitude=0.05)
+    q2 = inputs.random_spinor_state((40, 33), seed=42, amplitude=0.05)
+    for order in ("plain", "interleaved"):
+        assert rel_l2(run(q1, 1, order, 9), oracle.step(q1, 1, c, ORDERS[order], 9, mu=mu)) < TOL64
+        assert rel_l2(run(q2, 2, order, 5), oracle.step(q2, 2, c, ORDERS[order], 5, mu=mu)) < TOL64
+        assert rel_l2(run(q2, 2, order, 3, options=((qlga.OPT_PATH, 1),)),
+                      oracle.step(q2, 2, c, ORDERS[order], 3, mu=mu)) < TOL64
+    q32 = q2.astype(np.complex64)
+    assert rel_l2(run(q32, 2, "interleaved", 5, precision="f32"),
+                  oracle.step(q32.astype(np.complex128), 2, c, 1, 5, mu=mu)) < TOL32
+    assert rel_l2(run(q1, 1, "plain", 3, mu_=2.5), oracle.step(q1, 1, c, 0, 3, mu=2.5)) < TOL64   # general path
+    assert rel_l2(run(q1, 1, "plain", 3, mu_=0.0), oracle.step(q1, 1, c, 0, 3)) < TOL64
+    from paper_1907_12834_b200 import dispersion
+    cb, L, k, n = (-1.0, -0.5, 0.2), 1024, 1.0 / 16, 4
+    sim = qlga.Qlga(1, (L, 1), cb)
+    sim.set_chemical_potential(0.011)
+    sim.set_state_psi(dispersion.kicked_soliton("bright", 3, cb, L, k, n))
+    sim.step(21)
+    p = 2 * np.pi * n / L
+    assert abs(sim.observables()["e_dt_re"] - (0.011 + p * p - k * k)) < 0.02 * (p * p + k * k)
+    with pytest.raises(qlga.QlgaError) as e:
+        sim.set_chemical_potential(float("nan"))
+    assert e.value.status == qlga.QLGA_EINVAL
+    sim.close()
