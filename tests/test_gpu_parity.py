@@ -197,10 +197,11 @@ def test_long_run_error_growth(qlga, oracle):
 # full-size lattices in the launch configuration bench.py times: windowed parity
 # (the domain of dependence of a site is exactly 4 sites per step per direction)
 # ---------------------------------------------------------------------------
-def _windowed_parity(qlga, oracle, ndim, dims, couplings, q_dev_in, steps, windows, P, precision, tol):
+def _windowed_parity(qlga, oracle, ndim, dims, couplings, q_dev_in, steps, windows, P, precision, tol,
+                     order="interleaved"):
     import torch
     nx, ny = dims
-    sim = qlga.Qlga(ndim, dims, couplings, order="interleaved", precision=precision)
+    sim = qlga.Qlga(ndim, dims, couplings, order=order, precision=precision)
     sim.set_state_q(q_dev_in)
     sim.step(steps)
     cdt = torch.complex128 if precision == "f64" else torch.complex64
@@ -214,7 +215,7 @@ def _windowed_parity(qlga, oracle, ndim, dims, couplings, q_dev_in, steps, windo
         xi = torch.as_tensor(xs, device="cuda"); yi = torch.as_tensor(ys, device="cuda")
         patch_in = q_dev_in[:, :, yi][:, :, :, xi].cpu().numpy().astype(np.complex128)
         patch_out = out_dev[:, :, yi][:, :, :, xi].cpu().numpy().astype(np.complex128)
-        ref = oracle.step(patch_in, ndim, couplings, 1, steps)          # periodic patch: only the centre is valid
+        ref = oracle.step(patch_in, ndim, couplings, ORDERS[order], steps)   # periodic patch: only the centre is valid
         if ndim == 2:
             a, b = patch_out[:, :, h:h + P, h:h + P], ref[:, :, h:h + P, h:h + P]
         else:
@@ -233,9 +234,27 @@ def test_config5_full_size_windowed(qlga, oracle):
     del psi
     windows = [(0, 0), (L // 2 + 40, L // 2 - 260), (L - 20, L - 20), (1234, 4321)]   # wrap corners, a vortex core, bulk
     _windowed_parity(qlga, oracle, 2, (L, L), w.couplings, q_dev, 2, windows, 24, "f64", TOL64)
+    _windowed_parity(qlga, oracle, 2, (L, L), w.couplings, q_dev, 2, windows[:3], 24, "f64", TOL64, order="plain")
     q32 = q_dev.to(torch.complex64)
     del q_dev
     _windowed_parity(qlga, oracle, 2, (L, L), w.couplings, q32, 2, windows, 24, "f32", TOL32)
+    _windowed_parity(qlga, oracle, 2, (L, L), w.couplings, q32, 2, windows[:3], 24, "f32", TOL32, order="plain")
+
+
+def test_config4_and_config2_full_size_windowed(qlga, oracle):
+    import torch
+    L = 2048
+    w = inputs.config4(L=L)
+    q_dev = torch.from_numpy(_q_of(w)).cuda()
+    windows = [(0, 0), (L // 4 - 12, L // 4 - 12), (L - 20, L // 2)]            # wrap corner, a vortex core, wrap edge
+    for order in ("interleaved", "plain"):
+        _windowed_parity(qlga, oracle, 2, (L, L), w.couplings, q_dev, 3, windows, 24, "f64", TOL64, order=order)
+    L = 65536                                                                  # temporal blocking: 4 steps per launch
+    w = inputs.config2(L=L)
+    q_dev = torch.from_numpy(_q_of(w)).cuda()
+    windows = [(0, 0), (L // 4 - 60, 0), (3 * L // 4 - 60, 0), (L - 40, 0)]
+    for order in ("interleaved", "plain"):
+        _windowed_parity(qlga, oracle, 1, (L, 1), w.couplings, q_dev, 9, windows, 120, "f64", TOL64, order=order)
 
 
 def test_config3_full_size_windowed(qlga, oracle):
