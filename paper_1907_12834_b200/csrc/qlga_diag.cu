@@ -152,9 +152,44 @@ cudaError_t launch_observables(const Launch& L, qlga_prec prec, const void* q, c
 // The arithmetic is done in fp64 for both storage types.
 // ---------------------------------------------------------------------------
 __device__ __forceinline__ double arg_prod_conj(double ar, double ai, double br, double bi) {
-    // arg(a * conj(b))
-    const double re = ar * br + ai * bi, im = ai * br - ar * bi;
+    // arg(a * conj(b)); products rounded one by one (no FMA contraction): the sign of an exactly
+    // cancelling imaginary part decides between +pi and -pi
+    const double re = __dadd_rn(__dmul_rn(ar, br), __dmul_rn(ai, bi));
+    const double im = __dsub_rn(__dmul_rn(ai, br), __dmul_rn(ar, bi));
     return (re == 0.0 && im == 0.0) ? 0.0 : atan2(im, re);
+}
+
+// Winding number of the closed loop z0 -> z1 -> z2 -> z3 -> z0 whose edges are the wrapped phase
+// differences arg(z_{k+1} conj z_k) in (-pi, pi]: their sum is 2 pi w exactly, so w needs no atan2.
+// Each vertex is assigned the quadrant it lies in (half-open, so that the four sectors tile the plane
+// without the origin); an edge changes the quadrant count by 0, +-1 (neighbouring quadrants: the short
+// arc) or +-2 (opposite quadrants: the sign of Im(z_{k+1} conj z_k) gives the sense of rotation), and
+// w = (sum of the changes) / 4.  Returns false in the cases where a wrapped difference is not defined
+// by the geometry alone -- a vertex that is exactly zero (arg(0) := 0 breaks the loop) or two opposite
+// vertices exactly antiparallel (arg = +-pi by the sign of a zero) -- which take the atan2 path.
+__device__ __forceinline__ int quadrant(double re, double im) {
+    return (re > 0.0 && im >= 0.0) ? 0 : ((re <= 0.0 && im > 0.0) ? 1 : ((re < 0.0 && im <= 0.0) ? 2 : 3));
+}
+__device__ __forceinline__ bool loop_winding(const double zr[4], const double zi[4], int* w) {
+    int q[4];
+    bool ok = true;
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+        ok = ok && !(zr[k] == 0.0 && zi[k] == 0.0);
+        q[k] = quadrant(zr[k], zi[k]);
+    }
+    int sum = 0;
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+        const int t = (k + 1) & 3;
+        const int dq = (q[t] - q[k]) & 3;
+        // Im(z_t conj z_k), products rounded one by one so that exactly antiparallel vertices give exactly 0
+        const double im = __dsub_rn(__dmul_rn(zi[t], zr[k]), __dmul_rn(zr[t], zi[k]));
+        ok = ok && !(dq == 2 && im == 0.0);
+        sum += (dq == 0) ? 0 : ((dq == 1) ? 1 : ((dq == 3) ? -1 : (im > 0.0 ? 2 : -2)));
+    }
+    *w = sum / 4;
+    return ok;
 }
 
 template <typename T>
@@ -176,6 +211,15 @@ __global__ void __launch_bounds__(128) vorticity_kernel(const typename vec2<T>::
         a = p1[ipm]; b = p2[ipm]; const double pmr = (double)a.x + (double)b.x, pmi = (double)a.y + (double)b.y;
         a = p1[imp]; b = p2[imp]; const double mpr = (double)a.x + (double)b.x, mpi = (double)a.y + (double)b.y;
         a = p1[imm]; b = p2[imm]; const double mmr = (double)a.x + (double)b.x, mmi = (double)a.y + (double)b.y;
+        // The four terms are the wrapped phase differences around the closed loop
+        // (x+1,y-1) -> (x+1,y+1) -> (x-1,y+1) -> (x-1,y-1) -> (x+1,y-1): omega = (pi/2) x its winding number.
+        const double zr[4] = {pmr, ppr, mpr, mmr}, zi[4] = {pmi, ppi, mpi, mmi};
+        int w;
+        if (loop_winding(zr, zi, &w)) {
+            omega[(int64_t)j * n + r] = (T)(1.5707963267948966192313216916398 * (double)w);
+            continue;
+        }
+        // degenerate site (a zero or an exactly antiparallel pair among the four): the definition term by term
         // v_y(x+1,y), v_y(x-1,y), v_x(x,y+1), v_x(x,y-1)   (each is half the wrapped phase difference)
         const double vy_p = 0.5 * arg_prod_conj(ppr, ppi, pmr, pmi);
         const double vy_m = 0.5 * arg_prod_conj(mpr, mpi, mmr, mmi);
@@ -310,9 +354,13 @@ __global__ void __launch_bounds__(128) vortices_kernel(const typename vec2<T>::t
         u = p1[ib]; v = p2[ib]; const double br = (double)u.x + (double)v.x, bi = (double)u.y + (double)v.y;
         u = p1[ic]; v = p2[ic]; const double cr = (double)u.x + (double)v.x, ci = (double)u.y + (double)v.y;
         u = p1[id]; v = p2[id]; const double dr = (double)u.x + (double)v.x, di = (double)u.y + (double)v.y;
-        const double circ = arg_prod_conj(br, bi, ar, ai) + arg_prod_conj(cr, ci, br, bi)
-                          + arg_prod_conj(dr, di, cr, ci) + arg_prod_conj(ar, ai, dr, di);
-        const int w = (int)rint(circ * 0.15915494309189533576888376337251);      // 1/(2 pi)
+        const double zr[4] = {ar, br, cr, dr}, zi[4] = {ai, bi, ci, di};
+        int w;
+        if (!loop_winding(zr, zi, &w)) {          // degenerate plaquette: the definition term by term
+            const double circ = arg_prod_conj(br, bi, ar, ai) + arg_prod_conj(cr, ci, br, bi)
+                              + arg_prod_conj(dr, di, cr, ci) + arg_prod_conj(ar, ai, dr, di);
+            w = (int)rint(circ * 0.15915494309189533576888376337251);            // 1/(2 pi)
+        }
         if (w != 0) {
             const unsigned long long slot = atomicAdd(counter, 1ULL);
             if ((long long)slot < max_out) {

@@ -561,3 +561,34 @@ def test_chemical_potential(qlga, oracle):
         sim.set_chemical_potential(float("nan"))
     assert e.value.status == qlga.QLGA_EINVAL
     sim.close()
+
+
+def test_vorticity_and_vortices_degenerate_phases(qlga, oracle):
+    # The vorticity / vortex kernels count quadrant changes around the loop instead of calling atan2, and
+    # fall back to the term-by-term definition when a vertex is exactly zero or two vertices are exactly
+    # antiparallel.  Fields built to sit on those cases: real-valued (every phase 0 or pi), values on the
+    # axes, exact zeros sprinkled in, and 8th roots of unity (neighbours exactly antiparallel or orthogonal).
+    c = (1.0, 0.3, -0.1)
+    nx, ny = 37, 29
+    rng = np.random.default_rng(91)
+    real = rng.standard_normal((5, ny, nx)) + 0j
+    axes = np.where(rng.random((5, ny, nx)) < 0.5, 1.0, 1j) * rng.standard_normal((5, ny, nx))
+    unit = np.array([1, 1 + 1j, 1j, -1 + 1j, -1, -1 - 1j, -1j, 1 - 1j])          # exact directions, 45 degrees apart
+    roots = unit[rng.integers(0, 8, (5, ny, nx))] * 2.0 ** rng.integers(-3, 3, (5, ny, nx))
+    zeros = inputs.random_field((nx, ny), seed=92)
+    zeros[rng.random((5, ny, nx)) < 0.15] = 0.0
+    generic = inputs.random_field((nx, ny), seed=93)
+    for name, psi in (("real", real), ("axes", axes), ("roots", roots), ("zeros", zeros), ("generic", generic)):
+        q = np.repeat(psi[:, None] / 2, 2, axis=1)
+        for precision in ("f64", "f32"):
+            sim = qlga.Qlga(2, (nx, ny), c, precision=precision)
+            sim.set_state_q(q.astype(sim.np_cdtype))
+            state = sim.get_state_q().astype(np.complex128)
+            om = sim.vorticity().astype(np.float64)
+            rec, count = sim.vortices()
+            sim.close()
+            tol = 1e-10 if precision == "f64" else 2e-6
+            assert np.abs(om - oracle.vorticity(state)).max() < tol, (name, precision)
+            wind = oracle.winding(state)
+            want = sorted((int(j), int(x), int(y), int(wind[j, y, x])) for j, y, x in np.argwhere(wind != 0))
+            assert count == len(want) and sorted(tuple(int(v) for v in r) for r in rec) == want, (name, precision)
