@@ -61,8 +61,11 @@ typedef enum {
     QLGA_OPT_EXP_TOL_LOG2 = 2,/* truncation target of the interaction exponential, log2 (default -56 / -27) */
     QLGA_OPT_THREADS_X = 3,   /* CTA size of the x pass: 128, 192 or 256; 0 = auto               */
     QLGA_OPT_TILE_Y = 4,      /* y pass: columns per CTA (1,2,4,8); 0 = auto                     */
-    QLGA_OPT_THREADS_Y = 5    /* CTA size of the y pass: 128, 192 or 256 (valid pairs with TILE_Y: 1x128, 1x192,
+    QLGA_OPT_THREADS_Y = 5,   /* CTA size of the y pass: 128, 192 or 256 (valid pairs with TILE_Y: 1x128, 1x192,
                                  2x128, 2x192, 2x256, 4x256, 8x256); 0 = auto */
+    QLGA_OPT_FUSE_PLAIN_U = 6 /* plain ordering in 2D/3D, several steps per qlga_step call: 1 (default) = the U of
+                                 step t+1 is applied at the end of step t's x pass (same operator product, no halo
+                                 recompute of U, and it fills the memory-bound pass); 0 = always on the first pass */
 } qlga_option;
 
 /* Lattice sums returned by qlga_observables (always double).

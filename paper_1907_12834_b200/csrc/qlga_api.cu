@@ -201,7 +201,7 @@ extern "C" qlga_status qlga_init(qlga_ctx** out, int ndim, const int64_t* dims,
     c->buf_bytes = buf_bytes;
     c->stream = (cudaStream_t)cuda_stream;
     c->cur = 0; c->prev = -1; c->have_state = 0; c->step = 0; c->launches = 0;
-    c->path = 0; c->steps_per_launch = 0; c->threads_x = 0; c->tile_y = 0;
+    c->path = 0; c->steps_per_launch = 0; c->threads_x = 0; c->tile_y = 0; c->fuse_plain_u = 1;
     c->tol_log2 = (prec == QLGA_F64) ? -56 : -27;
     build_exp_table(c->tab, c->tol_log2);
     c->obs_blocks = prop.multiProcessorCount * 8;
@@ -254,6 +254,9 @@ extern "C" qlga_status qlga_set_option(qlga_ctx* c, qlga_option key, int64_t v) 
         case QLGA_OPT_TILE_Y:
             if (v != 0 && v != 1 && v != 2 && v != 4 && v != 8) return fail(c, QLGA_EINVAL, "QLGA_OPT_TILE_Y: 0,1,2,4,8");
             c->tile_y = (int)v; return QLGA_OK;
+        case QLGA_OPT_FUSE_PLAIN_U:
+            if (v != 0 && v != 1) return fail(c, QLGA_EINVAL, "QLGA_OPT_FUSE_PLAIN_U: 0 or 1");
+            c->fuse_plain_u = (int)v; return QLGA_OK;
     }
     return fail(c, QLGA_EINVAL, "qlga_set_option: unknown key");
 }
@@ -397,6 +400,8 @@ static void fill_pass_consts(const qlga_ctx* c, PassParams& P, double s) {
         P.g[f][2] = sc * c->c[2] / 5.0;
     }
     P.smu = s * c->mu;
+    P.utail = 0;
+    P.gt[0] = s * c->c[0]; P.gt[1] = s * c->c[1]; P.gt[2] = s * c->c[2] / 5.0;
     P.out_scale = 0.0625;
     P.tab = c->tab;
 }
@@ -442,10 +447,17 @@ static qlga_status step_fused(qlga_ctx* c, int64_t nsteps) {
     }
     // 2D: y pass then x pass; 3D: z, y, x (R7).  The passes ping-pong between buffers; with a
     // third buffer the state before the step survives (for eq. 85), otherwise it is overwritten.
+    // Plain ordering: inside one call the U of step t+1 rides on the end of step t's x pass (see
+    // pass_kernel); the first step of a call applies its own U on its first pass, the last step leaves the
+    // state without a trailing U.  With a third buffer the state before the last step must be a true state
+    // of the time series (eq. 85), so the last-but-one step does not carry the last step's U either.
+    bool u_done = false;                                   // the coming step's U has already been applied
+    const bool keeps_prev = pick_other(c, c->cur, pick_other(c, c->cur, -1)) >= 0;
     for (int64_t t = 0; t < nsteps; ++t) {
         const int start = c->cur;
         const int third = pick_other(c, start, pick_other(c, start, -1));
         int src = start;
+        const bool tail = !inter && c->fuse_plain_u && (t + 1 < nsteps) && !(keeps_prev && t + 2 == nsteps);
         for (int d = c->ndim - 1; d >= 0; --d) {
             int dst;
             if (third >= 0) {
@@ -458,21 +470,27 @@ static qlga_status step_fused(qlga_ctx* c, int64_t nsteps) {
             P.ksteps = 1;
             P.src = c->buf[src]; P.dst = c->buf[dst];
             // U is the rightmost operator of the plain step: it rides on the first pass
-            P.umode = inter ? 2 : (d == c->ndim - 1 ? 1 : 0);
+            P.umode = inter ? 2 : ((d == c->ndim - 1 && !u_done) ? 1 : 0);
+            P.utail = (d == 0 && tail) ? 1 : 0;
             prof_mark(c, d == 0 ? 0 : 1);
             // strided passes, measured defaults.  Interleaved (FP-pipe bound): the kernel's own (fp64 one
             // column x 128 rows, fp32 two x 64); 3D fp64: two columns, i.e. whole 32-byte sectors, which the
-            // page-crossing z lines need (+12 % at 512^3).  Plain ordering (one U per step or none: the
-            // memory phases count): whole sectors again -- fp64 two columns x 64 rows (8192^2: 8.8 ms
-            // against 12.2 for one column), fp32 four x 64 (5.4 against 5.9 ms)
+            // page-crossing z lines need (+12 % at 512^3).  Plain ordering: the memory phases count.  A pass
+            // that carries the step's U: fp64 two columns x 64 rows (8192^2: 8.8 ms against 12.2 for one
+            // column), fp32 four x 64; a U-free pass (pure streaming): fp64 four x 64 (6.2 ms against 8.7 for
+            // two columns), fp32 eight x 32 (3.2 against 5.3 ms)
             int cxw = c->tile_y, thr = c->threads_y;
             if (d > 0 && cxw == 0) {
-                if (!inter) { cxw = c->prec == QLGA_F64 ? 2 : 4; if (thr == 0) thr = c->prec == QLGA_F64 ? 128 : 256; }
-                else if (c->ndim == 3 && c->prec == QLGA_F64) { cxw = 2; if (thr == 0) thr = 128; }
+                if (!inter) {
+                    const bool f64 = c->prec == QLGA_F64;
+                    cxw = (P.umode != 0) ? (f64 ? 2 : 4) : (f64 ? 4 : 8);
+                    if (thr == 0) thr = (P.umode != 0 && f64) ? 128 : 256;
+                } else if (c->ndim == 3 && c->prec == QLGA_F64) { cxw = 2; if (thr == 0) thr = 128; }
             }
             CU(c, launch_pass(L, c->prec, d, P, d == 0 ? c->threads_x : thr, d == 0 ? 1 : cxw));
             src = dst;
         }
+        u_done = tail;
         c->prev = (third >= 0) ? start : -1;
         c->cur = src;
         ++c->step;

@@ -20,6 +20,8 @@ struct PassParams {
                            // 2: U before every factor
     double g[4][3];        // per factor: (s c0, s c1, s c2/5) * 4^-e  (e = deferred halvings so far)
     double smu;            // s * mu, the chemical-potential phase of one U (not scaled: it multiplies no density)
+    int utail;             // plain ordering: apply the NEXT step's U (constants gt) after this pass's last factor
+    double gt[3];          // (c0, c1, c2/5): the full-angle U on the unscaled state
     double out_scale;      // 2^-4, applied after the 4 factors of a step
     ExpTable tab;
 };
@@ -80,6 +82,7 @@ struct qlga_ctx {
     // options
     int path;              // 0 fused, 1 per-operator
     int steps_per_launch;  // 1D temporal blocking, 0 = auto
+    int fuse_plain_u;      // plain ordering, 2D/3D: the next step's U rides on the x pass (default on)
     int tol_log2;
     int threads_x;
     int tile_y;

@@ -28,8 +28,9 @@ struct PassArgs {
     // the lines.  x pass: len = nx, the lines are the ny*nz rows (outer_stride = nx).
     // y pass: stride = nx, len = ny, outer = z.   z pass: stride = nx*ny, len = nz, outer = y.
     int64_t nx, len, stride, n_outer, outer_stride, nsites;
-    int ksteps, umode;
+    int ksteps, umode, utail;
     UConst<T> uc[4];
+    UConst<T> uct;              // trailing U of the plain ordering (see pass_kernel)
     T out_scale;
     ExpTable tab;
 };
@@ -171,6 +172,13 @@ pass_kernel(const __grid_constant__ PassArgs<T> P) {
             s.q[j][1] = rmul(P.out_scale, s.q[j][1]);
         }
     }
+    // Plain ordering, several steps per call: the next step's U (the rightmost operator of eq. 108) is
+    // applied here, at the end of the last pass of this step, where the state is final and in registers
+    // and the pass is otherwise memory-bound -- instead of at the start of the next step's first pass,
+    // where the halo threads would recompute it.  Site-local, so the product of operators is the same.
+    if constexpr (HASU) {
+        if (P.utail) interaction<T>(s, P.uct, P.tab);
+    }
 
     if (i >= H && i < TS - H && spos < extent && col_ok) {
 #pragma unroll
@@ -189,7 +197,8 @@ static PassArgs<T> make_args(const PassParams& P, int dir) {
     PassArgs<T> A;
     A.src = (const typename vec2<T>::type*)P.src;
     A.dst = (typename vec2<T>::type*)P.dst;
-    A.nx = P.nx; A.nsites = P.nx * P.ny * P.nz; A.ksteps = P.ksteps; A.umode = P.umode;
+    A.nx = P.nx; A.nsites = P.nx * P.ny * P.nz; A.ksteps = P.ksteps; A.umode = P.umode; A.utail = P.utail;
+    A.uct = make_uconst<T>(P.gt[0], P.gt[1], P.gt[2], P.smu);
     for (int f = 0; f < 4; ++f) A.uc[f] = make_uconst<T>(P.g[f][0], P.g[f][1], P.g[f][2], P.smu);
     A.out_scale = (T)P.out_scale;
     A.tab = P.tab;
@@ -220,7 +229,7 @@ static cudaError_t run_pass(const Launch& L, const PassParams& P, int dir) {
         if (e != cudaSuccess) return e;
         configured = true;
     }
-    if (P.umode != 0) pass_kernel<T, DIR, CX, NT, true><<<(unsigned)blocks, NT, smem, L.stream>>>(A);
+    if (P.umode != 0 || P.utail) pass_kernel<T, DIR, CX, NT, true><<<(unsigned)blocks, NT, smem, L.stream>>>(A);
     else pass_kernel<T, DIR, CX, NT, false><<<(unsigned)blocks, NT, smem, L.stream>>>(A);
     ++*L.counter;
     return cudaGetLastError();

@@ -18,7 +18,7 @@ _LIB_PATH = os.path.join(_HERE, "libqlga.so")
 QLGA_OK, QLGA_EINVAL, QLGA_ENOMEM, QLGA_ECUDA, QLGA_ESTATE, QLGA_EUNSUP = range(6)
 QLGA_F64, QLGA_F32 = 0, 1
 QLGA_PLAIN, QLGA_INTERLEAVED = 0, 1
-OPT_PATH, OPT_STEPS_PER_LAUNCH, OPT_EXP_TOL_LOG2, OPT_THREADS_X, OPT_TILE_Y, OPT_THREADS_Y = range(6)
+OPT_PATH, OPT_STEPS_PER_LAUNCH, OPT_EXP_TOL_LOG2, OPT_THREADS_X, OPT_TILE_Y, OPT_THREADS_Y, OPT_FUSE_PLAIN_U = range(7)
 
 ABI_SYMBOLS = (
     "qlga_init", "qlga_state_bytes", "qlga_set_option", "qlga_set_state_psi", "qlga_set_state_q",

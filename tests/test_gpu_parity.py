@@ -592,3 +592,36 @@ def test_vorticity_and_vortices_degenerate_phases(qlga, oracle):
             wind = oracle.winding(state)
             want = sorted((int(j), int(x), int(y), int(wind[j, y, x])) for j, y, x in np.argwhere(wind != 0))
             assert count == len(want) and sorted(tuple(int(v) for v in r) for r in rec) == want, (name, precision)
+
+
+def test_plain_ordering_trailing_interaction(qlga, oracle):
+    # Plain ordering, 2D/3D: inside one qlga_step call the U of step t+1 rides on the end of step t's x pass
+    # (QLGA_OPT_FUSE_PLAIN_U, default on).  Same operator product: parity with the oracle for every split of
+    # the steps into calls, with the option off, with a previous-state buffer (eq. 85 needs a true state of
+    # the time series in it), and in fp32 / 3D.
+    c = (1.0, 0.3, -0.1)
+    q0 = inputs.random_spinor_state((45, 38), seed=51, amplitude=0.06)
+    refs = {n: oracle.step(q0, 2, c, 0, n) for n in (1, 2, 3, 5, 6)}
+    for calls in ((1,), (2,), (3,), (5,), (2, 3), (1, 1, 1), (6,)):
+        for fuse in (1, 0):
+            for keep in (False, True):
+                sim = qlga.Qlga(2, (45, 38), c, order="plain", keep_previous=keep)
+                sim.set_option(qlga.OPT_FUSE_PLAIN_U, fuse)
+                sim.set_state_q(q0)
+                for n in calls:
+                    sim.step(n)
+                out = sim.get_state_q()
+                ob = sim.observables()
+                sim.close()
+                total = sum(calls)
+                assert rel_l2(out, refs[total]) < TOL64, (calls, fuse, keep)
+                if keep:
+                    prev = oracle.step(q0, 2, c, 0, total - 1) if total > 1 else q0
+                    want = oracle.observables(refs[total], 2, c, qprev=prev)
+                    assert ob["e_dt_re"] == pytest.approx(want["e_dt_re"], rel=1e-9, abs=1e-13), (calls, fuse)
+                    assert ob["e_dt_im"] == pytest.approx(want["e_dt_im"], rel=1e-9, abs=1e-13), (calls, fuse)
+    q3 = inputs.random_spinor_state((12, 10, 9), seed=52, amplitude=0.06)
+    assert rel_l2(run_gpu(qlga, q3, 3, c, "plain", 4), oracle.step(q3, 3, c, 0, 4)) < TOL64
+    q32 = q0.astype(np.complex64)
+    assert rel_l2(run_gpu(qlga, q32, 2, c, "plain", 5, precision="f32"),
+                  oracle.step(q32.astype(np.complex128), 2, c, 0, 5)) < TOL32
