@@ -264,6 +264,11 @@ def test_config3_full_size_windowed(qlga, oracle):
     q_dev = torch.from_numpy(_q_of(w)).cuda()
     windows = [(0, 0), (L // 4 - 50, 0), (L - 30, 0), (3 * L // 4, 0)]
     _windowed_parity(qlga, oracle, 1, (L, 1), w.couplings, q_dev, 5, windows, 100, "f64", TOL64)
+    # plain ordering and fp32 run two time steps per launch on a lattice of this size
+    _windowed_parity(qlga, oracle, 1, (L, 1), w.couplings, q_dev, 5, windows, 100, "f64", TOL64, order="plain")
+    q32 = q_dev.to(torch.complex64)
+    _windowed_parity(qlga, oracle, 1, (L, 1), w.couplings, q32, 5, windows, 100, "f32", TOL32)
+    _windowed_parity(qlga, oracle, 1, (L, 1), w.couplings, q32, 5, windows, 100, "f32", TOL32, order="plain")
 
 
 # ---------------------------------------------------------------------------
