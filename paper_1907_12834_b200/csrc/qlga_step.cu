@@ -91,6 +91,9 @@ __device__ __forceinline__ void factor(Site<T>& s, const PassArgs<T>& P, int f, 
 #ifndef QLGA_MINB128_F32
 #define QLGA_MINB128_F32 5
 #endif
+#ifndef QLGA_MINB256_NOU
+#define QLGA_MINB256_NOU 2
+#endif
 #ifndef QLGA_MINB_NOU
 #define QLGA_MINB_NOU 4
 #endif
@@ -104,7 +107,7 @@ __device__ __forceinline__ void factor(Site<T>& s, const PassArgs<T>& P, int f, 
 template <typename T, int DIR, int CX, int NT, bool HASU>
 __global__ void __launch_bounds__(NT, (HASU ? (NT >= 192 ? 2 : (NT >= 128 ? (sizeof(T) == 8 ? QLGA_MINB128 : (DIR == 0 ? QLGA_MINB128_F32X : QLGA_MINB128_F32))
                                                                          : (NT >= 96 ? 4 : 6)))
-                                            : (NT >= 192 ? 2 : QLGA_MINB_NOU)))
+                                            : (NT >= 256 ? QLGA_MINB256_NOU : (NT >= 192 ? 2 : QLGA_MINB_NOU))))
 pass_kernel(const __grid_constant__ PassArgs<T> P) {
     using V = typename vec2<T>::type;
     constexpr int TS = NT / CX;              // sites per line handled by the CTA
