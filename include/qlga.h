@@ -22,7 +22,7 @@
  *   omega : [5][Ny][Nx]      real (2D only)
  *   j = 0..4 <-> m_f = +2,+1,0,-1,-2;  sigma = 0,1 <-> spinor component 1,2;
  *   x fastest; Ny = Nz = 1 in 1D, Nz = 1 in 2D; complex = interleaved (re, im) of the
- *   context's real type (double for QLGA_F64, float for QLGA_F32); periodic in x, y, z.
+ *   context's storage type (double for QLGA_F64, float for QLGA_F32 and QLGA_F32X); periodic in x, y, z.
  */
 #ifndef QLGA_H
 #define QLGA_H
@@ -45,7 +45,13 @@ typedef enum {
     QLGA_EUNSUP = 5    /* not supported for this context (e.g. vorticity in 1D) */
 } qlga_status;
 
-typedef enum { QLGA_F64 = 0, QLGA_F32 = 1 } qlga_prec;
+/* Precision of a context.
+ *   QLGA_F64   state and arithmetic in fp64 (160 B per site); follows the oracle to rounding.
+ *   QLGA_F32   state and arithmetic in fp32 (80 B per site): the throughput / memory variant.
+ *   QLGA_F32X  state stored in fp32 (80 B per site, the same buffers and transfers as QLGA_F32), arithmetic in
+ *              fp64 registers inside every pass: one rounding to fp32 per amplitude per pass instead of one per
+ *              floating-point operation (measured error growth in DESIGN.md section 8). */
+typedef enum { QLGA_F64 = 0, QLGA_F32 = 1, QLGA_F32X = 2 } qlga_prec;
 
 /* Operator ordering of one time step (rightmost operator acts first):
  *   QLGA_PLAIN        eq. (108):  I'_x1 I'_x1 I'_x2 I'_x2 [I'_y1 I'_y1 I'_y2 I'_y2] U
@@ -57,15 +63,22 @@ typedef enum { QLGA_PLAIN = 0, QLGA_INTERLEAVED = 1 } qlga_order;
 /* Tunables of qlga_set_option. */
 typedef enum {
     QLGA_OPT_PATH = 0,        /* 0 = fused pass kernels (default), 1 = one kernel per operator   */
-    QLGA_OPT_STEPS_PER_LAUNCH = 1, /* 1D only: time steps fused per launch (halo 4 per step); 0 = auto */
+    QLGA_OPT_STEPS_PER_LAUNCH = 1, /* 1D only: time steps fused per launch (halo 4 per step); 0 = auto, else 1..15,
+                                 clamped to what the x pass's CTA size supports ((threads - 8) / 16) */
     QLGA_OPT_EXP_TOL_LOG2 = 2,/* truncation target of the interaction exponential, log2 (default -56 / -27) */
-    QLGA_OPT_THREADS_X = 3,   /* CTA size of the x pass: 128, 192 or 256; 0 = auto               */
-    QLGA_OPT_TILE_Y = 4,      /* y pass: columns per CTA (1,2,4,8); 0 = auto                     */
-    QLGA_OPT_THREADS_Y = 5,   /* CTA size of the y pass: 128, 192 or 256 (valid pairs with TILE_Y: 1x128, 1x192,
-                                 2x128, 2x192, 2x256, 4x256, 8x256); 0 = auto */
-    QLGA_OPT_FUSE_PLAIN_U = 6 /* plain ordering in 2D/3D, several steps per qlga_step call: 1 (default) = the U of
+    QLGA_OPT_THREADS_X = 3,   /* CTA size of the x pass: 64, 96, 128, 192 or 256; 0 = auto       */
+    QLGA_OPT_TILE_Y = 4,      /* strided (y, z) passes: columns per CTA (1,2,4,8); 0 = auto      */
+    QLGA_OPT_THREADS_Y = 5,   /* CTA size of the strided passes; 0 = auto.  TILE_Y and THREADS_Y are validated as a
+                                 pair: columns x threads 1x64, 1x96, 1x128, 1x192, 2x128, 2x192, 2x256, 4x256, 8x256
+                                 (either one 0 = auto for that one); any other pair is QLGA_EINVAL when it is set, and a
+                                 pair that only resolves to an unbuilt kernel at launch is QLGA_EINVAL from qlga_step */
+    QLGA_OPT_FUSE_PLAIN_U = 6,/* plain ordering in 2D/3D, several steps per qlga_step call: 1 (default) = the U of
                                  step t+1 is applied at the end of step t's x pass (same operator product, no halo
                                  recompute of U, and it fills the memory-bound pass); 0 = always on the first pass */
+    QLGA_OPT_F32_PHASE = 7,   /* QLGA_F32 only: formulation of the scalar phase factor exp(-i s (c0 rho + mu)):
+                                 0 = (cos, -sin) rounded to fp32, 1 = 1 + d with cos - 1 kept to its own precision
+                                 (default), 2 = 1 + d with d evaluated in fp64 */
+    QLGA_OPT_EXP_POLY = 8     /* interaction polynomial: 0 = Chebyshev-economised Taylor, 1 = plain Taylor */
 } qlga_option;
 
 /* Lattice sums returned by qlga_observables (always double).
@@ -114,7 +127,7 @@ size_t qlga_state_bytes(int ndim, const int64_t* dims, qlga_prec prec);
 qlga_status qlga_set_option(qlga_ctx*, qlga_option key, int64_t value);
 
 /* Load the bosonic field: q_m1 = q_m2 = psi_m / 2 (reading R6).  psi: HOST or DEVICE
- * ([5][Nz][Ny][Nx] complex of the context's real type) per src_on_device.  Resets step to 0. */
+ * ([5][Nz][Ny][Nx] complex of the context's storage type (double for QLGA_F64, float for QLGA_F32 and QLGA_F32X)) per src_on_device.  Resets step to 0. */
 qlga_status qlga_set_state_psi(qlga_ctx*, const void* psi, int src_on_device);
 /* Load / read back the full spinor state q ([5][2][Nz][Ny][Nx] complex); also the checkpoint format. */
 qlga_status qlga_set_state_q(qlga_ctx*, const void* q, int src_on_device);
@@ -137,15 +150,26 @@ qlga_status qlga_observables(qlga_ctx*, qlga_obs* host_out);
 /* Lattice vorticity, 2D only (eq. 99-104, reading R8), per m:
  *   v_x(r) = (1/2) arg(psi(r+e_x) psi*(r-e_x)),  v_y(r) = (1/2) arg(psi(r+e_y) psi*(r-e_y)),
  *   omega(r) = (1/2)[v_y(r+e_x) - v_y(r-e_x) - v_x(r+e_y) + v_x(r-e_y)],   arg(0) := 0.
- * omega: HOST or DEVICE [5][Ny][Nx] real of the context's real type.  QLGA_EUNSUP in 1D. */
+ * omega: HOST or DEVICE [5][Ny][Nx] real of the context's storage type.  QLGA_EUNSUP in 1D. */
 qlga_status qlga_vorticity(qlga_ctx*, void* omega, int dst_on_device);
+
+/* Interaction-angle statistics of the current state (diagnostic; it tells which polynomial degrees and
+ * which code path of U a state exercises).  For one application of U^(s) (s = 1 plain, 1/(4 ndim)
+ * interleaved, eq. 108 / 112) at every site:
+ *   theta = s (2 |c1| |F| + (|c2|/5) rho)   the spectral-norm bound of s K the kernels select the degree by,
+ *   phase = |s (c0 rho + mu)|               the scalar phase.
+ * host_out HOST: theta_max, theta_mean (atomic accumulation: reproducible to rounding only), phase_max,
+ * degree_hist[p] = number of sites whose own angle takes polynomial degree p = 1..12 by the kernels' lookup
+ * ([0] = sites beyond the split angle, which take the general path).  Synchronises the stream. */
+typedef struct { double theta_max, theta_mean, phase_max; int64_t degree_hist[13]; } qlga_angles;
+qlga_status qlga_angle_stats(qlga_ctx*, qlga_angles* host_out);
 
 /* Total density rho(r) = sum_m |psi_m(r)|^2 = psi psi^dagger; rho: HOST or DEVICE [Nz][Ny][Nx] real. */
 qlga_status qlga_density(qlga_ctx*, void* rho, int dst_on_device);
 
 /* L2 error of eq. (115), PAPER.md:1074 (the paper's convergence measure, Figs. 23-24):
- *   *host_eps = sum_r (rho_ref(r) - rho(r))^2,  rho_ref: HOST or DEVICE [Ny][Nx] real of the
- * context's real type (e.g. the density of the initial eigenstate).  Synchronises the stream. */
+ *   *host_eps = sum_r (rho_ref(r) - rho(r))^2,  rho_ref: HOST or DEVICE [Nz][Ny][Nx] real of the
+ * context's storage type (e.g. the density of the initial eigenstate).  Synchronises the stream. */
 qlga_status qlga_density_l2_error(qlga_ctx*, const void* rho_ref, int src_on_device, double* host_eps);
 
 /* Vortex detection, 2D only (the paper tracks vortices of positive / negative winding number,

@@ -11,7 +11,21 @@ using namespace qlga;
 
 static char g_init_err[512] = "";
 
-static qlga_status fail(qlga_ctx* c, qlga_status st, const char* fmt, const char* a = "") {
+// defaults of the fp32 kernels (QLGA_F32), settled by the measured error growth against the fp64 oracle
+// (DESIGN.md section 8): phase factor as 1 + d, truncation target, polynomial kind
+#ifndef QLGA_F32_PHASE_DEFAULT
+#define QLGA_F32_PHASE_DEFAULT 1
+#endif
+#ifndef QLGA_F32_TOL_DEFAULT
+#define QLGA_F32_TOL_DEFAULT -27
+#endif
+#ifndef QLGA_F32_POLY_DEFAULT
+#define QLGA_F32_POLY_DEFAULT 0
+#endif
+static const int F32_PHASE_MODE = QLGA_F32_PHASE_DEFAULT, F32_TOL_LOG2 = QLGA_F32_TOL_DEFAULT, F32_EXP_POLY = QLGA_F32_POLY_DEFAULT;
+
+static qlga_status fail(const qlga_ctx* cc, qlga_status st, const char* fmt, const char* a = "") {
+    qlga_ctx* c = const_cast<qlga_ctx*>(cc);
     char* dst = c ? c->err : g_init_err;
     snprintf(dst, 512, fmt, a);
     return st;
@@ -27,7 +41,23 @@ static qlga_status cuda_fail(qlga_ctx* c, const char* what, cudaError_t e) {
         if (e_ != cudaSuccess) return cuda_fail(ctx, #call, e_);            \
     } while (0)
 
+// storage: QLGA_F32X keeps the state in fp32 (its arithmetic is fp64, in registers)
 static size_t real_size(qlga_prec p) { return p == QLGA_F64 ? sizeof(double) : sizeof(float); }
+static qlga_prec storage_prec(const qlga_ctx* c) { return c->prec == QLGA_F64 ? QLGA_F64 : QLGA_F32; }
+
+// Every entry point runs on the context's own device, whatever device is current in the calling
+// thread, and restores the caller's device on return.
+struct DeviceGuard {
+    int prev = -1;
+    bool switched = false;
+    explicit DeviceGuard(const qlga_ctx* c) {
+        if (c && cudaGetDevice(&prev) == cudaSuccess && prev != c->device)
+            switched = cudaSetDevice(c->device) == cudaSuccess;
+    }
+    ~DeviceGuard() { if (switched) cudaSetDevice(prev); }
+    DeviceGuard(const DeviceGuard&) = delete;
+    DeviceGuard& operator=(const DeviceGuard&) = delete;
+};
 
 // ---------------------------------------------------------------------------
 // The interaction polynomial.  exp(-i s K) v is evaluated as P_p(-i s K) v with P_p a
@@ -74,20 +104,35 @@ static long double economise(int p, long double theta, long double* b /*[p+1]*/)
 
 // thr[p-1]: largest theta for which the economised degree-p polynomial stays within
 // tol = 2^tol_log2 (bisection on the monotone error bound); coefficients at that theta.
-static void build_exp_table(ExpTable& tab, int tol_log2) {
+// poly = 1: the plain Taylor polynomial instead (b_k = 1/k!): its leading ratios 1, 1/2 and b0 = 1 are exact
+// in binary floating point, which matters in fp32, where a ratio rounded by 3e-8 is the same relative
+// error of the angle at every application.
+static long double taylor(int p, long double theta, long double* b /*[p+1]*/) {
+    long double fact = 1.0L, pw = 1.0L;
+    for (int k = 0; k <= p; ++k) {
+        if (k > 0) { fact *= (long double)k; pw *= theta; }
+        b[k] = 1.0L / fact;
+    }
+    return pw * theta / (fact * (long double)(p + 1)) * (1.0L + theta);   // first dropped term, with the tail's margin
+}
+
+static void build_exp_table(ExpTable& tab, int tol_log2, int poly = 0, int phase_mode = 0) {
     const long double tol = ldexpl(1.0L, tol_log2);
+    tab.phase_mode = phase_mode;
     for (int p = 1; p <= QLGA_PMAX; ++p) {
         long double b[QLGA_PMAX + 1];
         long double lo = 0.0L, hi = 4.0L;
         for (int it = 0; it < 200; ++it) {
             const long double mid = 0.5L * (lo + hi);
-            if (economise(p, mid, b) <= tol) lo = mid; else hi = mid;
+            if ((poly ? taylor(p, mid, b) : economise(p, mid, b)) <= tol) lo = mid; else hi = mid;
         }
         long double th = lo * 0.999L;                      // margin for the fp32 angle estimate
-        economise(p, th, b);
+        if (poly) taylor(p, th, b); else economise(p, th, b);
         tab.thr[p - 1] = (float)th;
         if ((long double)tab.thr[p - 1] > th) tab.thr[p - 1] = nextafterf(tab.thr[p - 1], 0.0f);
         tab.b0[p - 1] = (double)b[0];
+        tab.b0m1[p - 1] = (double)(b[0] - 1.0L);
+        tab.b0m1f[p - 1] = (float)tab.b0m1[p - 1];
         for (int k = 0; k <= QLGA_PMAX; ++k) tab.r[p - 1][k] = 0.0;
         for (int k = 1; k <= p; ++k) tab.r[p - 1][k] = (double)(b[k] / b[k - 1]);
         tab.b0f[p - 1] = (float)tab.b0[p - 1];
@@ -146,7 +191,7 @@ extern "C" qlga_status qlga_exp_degree(int tol_log2, double theta, int* p) {
     return QLGA_OK;
 }
 
-extern "C" const char* qlga_version(void) { return "qlga-b200 0.1 (sm_100a)"; }
+extern "C" const char* qlga_version(void) { return "qlga-b200 0.2 (sm_100a)"; }
 
 // lattice extents from the caller's dims[]: {Nx, Ny} for ndim 1 and 2 (Ny = 1 in 1D),
 // {Nx, Ny, Nz} for ndim 3.  Returns false on bad arguments.
@@ -161,7 +206,7 @@ static bool lattice_dims(int ndim, const int64_t* dims, int64_t& nx, int64_t& ny
 extern "C" size_t qlga_state_bytes(int ndim, const int64_t* dims, qlga_prec prec) {
     int64_t nx, ny, nz;
     if (!lattice_dims(ndim, dims, nx, ny, nz)) return 0;
-    if (prec != QLGA_F64 && prec != QLGA_F32) return 0;
+    if (prec != QLGA_F64 && prec != QLGA_F32 && prec != QLGA_F32X) return 0;
     return (size_t)10 * (size_t)nx * (size_t)ny * (size_t)nz * 2 * real_size(prec);
 }
 
@@ -184,15 +229,34 @@ extern "C" qlga_status qlga_init(qlga_ctx** out, int ndim, const int64_t* dims,
     if (dev_buf_c && (dev_buf_c == dev_buf_a || dev_buf_c == dev_buf_b))
         return fail(nullptr, QLGA_EINVAL, "qlga_init: dev_buf_c aliases another buffer");
 
-    int dev = 0;
+    // the context lives on the device that holds its buffers, whatever device is current in this thread
+    int dev = -1;
+    {
+        void* bufs[3] = {dev_buf_a, dev_buf_b, dev_buf_c};
+        for (int k = 0; k < 3; ++k) {
+            if (!bufs[k]) continue;
+            cudaPointerAttributes at;
+            cudaError_t e = cudaPointerGetAttributes(&at, bufs[k]);
+            if (e != cudaSuccess) { cudaGetLastError(); return cuda_fail(nullptr, "qlga_init: cudaPointerGetAttributes", e); }
+            if (at.type != cudaMemoryTypeDevice && at.type != cudaMemoryTypeManaged)
+                return fail(nullptr, QLGA_EINVAL, "qlga_init: the state buffers must be device memory");
+            if (dev >= 0 && at.device != dev)
+                return fail(nullptr, QLGA_EINVAL, "qlga_init: the state buffers live on different devices");
+            dev = at.device;
+        }
+    }
+    int caller_dev = -1;
+    CU(nullptr, cudaGetDevice(&caller_dev));
     cudaDeviceProp prop;
-    CU(nullptr, cudaGetDevice(&dev));
     CU(nullptr, cudaGetDeviceProperties(&prop, dev));
     if (prop.major < 10) return fail(nullptr, QLGA_ECUDA, "qlga_init: the library is built for sm_100a only");
 
     qlga_ctx* c = new (std::nothrow) qlga_ctx;
     if (!c) return fail(nullptr, QLGA_ENOMEM, "qlga_init: out of host memory");
     memset(c, 0, sizeof(*c));
+    c->device = dev;
+    DeviceGuard guard(c);
+    (void)caller_dev;
     c->ndim = ndim;
     lattice_dims(ndim, dims, c->nx, c->ny, c->nz);
     c->c[0] = c0; c->c[1] = c1; c->c[2] = c2;
@@ -202,13 +266,17 @@ extern "C" qlga_status qlga_init(qlga_ctx** out, int ndim, const int64_t* dims,
     c->stream = (cudaStream_t)cuda_stream;
     c->cur = 0; c->prev = -1; c->have_state = 0; c->step = 0; c->launches = 0;
     c->path = 0; c->steps_per_launch = 0; c->threads_x = 0; c->tile_y = 0; c->fuse_plain_u = 1;
-    c->tol_log2 = (prec == QLGA_F64) ? -56 : -27;
-    build_exp_table(c->tab, c->tol_log2);
+    c->tol_log2 = (prec == QLGA_F32) ? F32_TOL_LOG2 : -56;
+    c->exp_poly = (prec == QLGA_F32) ? F32_EXP_POLY : 0;
+    c->f32_phase = F32_PHASE_MODE;
+    build_exp_table(c->tab, c->tol_log2, c->exp_poly, c->f32_phase);
     c->obs_blocks = prop.multiProcessorCount * 8;
     cudaError_t e = cudaMalloc(&c->d_partials, sizeof(double) * (size_t)c->obs_blocks * OBS_NACC);
     if (e == cudaSuccess) e = cudaMalloc(&c->d_sums, sizeof(double) * OBS_NACC);
+    if (e == cudaSuccess) e = cudaMalloc(&c->d_flag, sizeof(int));
+    if (e == cudaSuccess) e = cudaMemset(c->d_flag, 0, sizeof(int));
     if (e != cudaSuccess) {
-        cudaFree(c->d_partials);
+        cudaFree(c->d_partials); cudaFree(c->d_sums); cudaFree(c->d_flag);
         delete c;
         return cuda_fail(nullptr, "qlga_init: cudaMalloc(scratch)", e);
     }
@@ -220,8 +288,9 @@ extern "C" qlga_status qlga_init(qlga_ctx** out, int ndim, const int64_t* dims,
 
 extern "C" qlga_status qlga_destroy(qlga_ctx* c) {
     if (!c) return QLGA_EINVAL;
+    DeviceGuard guard(c);
     cudaStreamSynchronize(c->stream);
-    cudaFree(c->d_partials); cudaFree(c->d_sums); cudaFree(c->d_stage);
+    cudaFree(c->d_partials); cudaFree(c->d_sums); cudaFree(c->d_stage); cudaFree(c->d_scratch); cudaFree(c->d_flag);
     if (c->prof_ev) {
         for (int k = 0; k < PROF_CAP; ++k) cudaEventDestroy(c->prof_ev[k]);
         free(c->prof_ev); free(c->prof_kind);
@@ -235,25 +304,34 @@ extern "C" int64_t qlga_launch_count(const qlga_ctx* c) { return c ? c->launches
 
 extern "C" qlga_status qlga_set_option(qlga_ctx* c, qlga_option key, int64_t v) {
     if (!c) return QLGA_EINVAL;
-    switch (key) {
+    switch ((int)key) {
         case QLGA_OPT_PATH:
             if (v != 0 && v != 1) return fail(c, QLGA_EINVAL, "QLGA_OPT_PATH: 0 or 1");
             c->path = (int)v; return QLGA_OK;
         case QLGA_OPT_STEPS_PER_LAUNCH:
-            if (v < 0 || v > 64) return fail(c, QLGA_EINVAL, "QLGA_OPT_STEPS_PER_LAUNCH: 0..64");
+            if (v < 0 || v > max_ksteps(256) / 2) return fail(c, QLGA_EINVAL, "QLGA_OPT_STEPS_PER_LAUNCH: 0..15");
             c->steps_per_launch = (int)v; return QLGA_OK;
         case QLGA_OPT_EXP_TOL_LOG2:
             if (v > -8 || v < -100) return fail(c, QLGA_EINVAL, "QLGA_OPT_EXP_TOL_LOG2: -100..-8");
-            c->tol_log2 = (int)v; build_exp_table(c->tab, c->tol_log2); return QLGA_OK;
+            c->tol_log2 = (int)v; build_exp_table(c->tab, c->tol_log2, c->exp_poly, c->f32_phase); return QLGA_OK;
         case QLGA_OPT_THREADS_X:
-            if (v != 0 && v != 64 && v != 96 && v != 128 && v != 192 && v != 256) return fail(c, QLGA_EINVAL, "QLGA_OPT_THREADS_X: 0, 64, 96, 128, 192, 256");
+            if (!pass_tile_supported(0, (int)v, 1)) return fail(c, QLGA_EINVAL, "QLGA_OPT_THREADS_X: 0, 64, 96, 128, 192, 256");
             c->threads_x = (int)v; return QLGA_OK;
         case QLGA_OPT_THREADS_Y:
-            if (v != 0 && v != 64 && v != 96 && v != 128 && v != 192 && v != 256) return fail(c, QLGA_EINVAL, "QLGA_OPT_THREADS_Y: 0, 64, 96, 128, 192, 256");
+            // validated as a pair with the columns per CTA: only the pairs listed in qlga.h are built
+            if (v < 0 || v > 256 || !pass_tile_supported(1, (int)v, c->tile_y))
+                return fail(c, QLGA_EINVAL, "QLGA_OPT_THREADS_Y: no kernel for this (TILE_Y, THREADS_Y) pair; see qlga.h");
             c->threads_y = (int)v; return QLGA_OK;
         case QLGA_OPT_TILE_Y:
-            if (v != 0 && v != 1 && v != 2 && v != 4 && v != 8) return fail(c, QLGA_EINVAL, "QLGA_OPT_TILE_Y: 0,1,2,4,8");
+            if (v < 0 || v > 8 || !pass_tile_supported(1, c->threads_y, (int)v))
+                return fail(c, QLGA_EINVAL, "QLGA_OPT_TILE_Y: no kernel for this (TILE_Y, THREADS_Y) pair; see qlga.h");
             c->tile_y = (int)v; return QLGA_OK;
+        case QLGA_OPT_F32_PHASE:
+            if (v < 0 || v > 2) return fail(c, QLGA_EINVAL, "QLGA_OPT_F32_PHASE: 0, 1 or 2");
+            c->f32_phase = (int)v; build_exp_table(c->tab, c->tol_log2, c->exp_poly, c->f32_phase); return QLGA_OK;
+        case QLGA_OPT_EXP_POLY:
+            if (v != 0 && v != 1) return fail(c, QLGA_EINVAL, "QLGA_OPT_EXP_POLY: 0 (economised) or 1 (Taylor)");
+            c->exp_poly = (int)v; build_exp_table(c->tab, c->tol_log2, c->exp_poly, c->f32_phase); return QLGA_OK;
         case QLGA_OPT_FUSE_PLAIN_U:
             if (v != 0 && v != 1) return fail(c, QLGA_EINVAL, "QLGA_OPT_FUSE_PLAIN_U: 0 or 1");
             c->fuse_plain_u = (int)v; return QLGA_OK;
@@ -273,6 +351,7 @@ static inline void prof_mark(qlga_ctx* c, int kind) {
 
 extern "C" qlga_status qlga_profile_enable(qlga_ctx* c, int on) {
     if (!c) return QLGA_EINVAL;
+    DeviceGuard guard(c);
     if (on && !c->prof_ev) {
         c->prof_ev = (cudaEvent_t*)calloc(PROF_CAP, sizeof(cudaEvent_t));
         c->prof_kind = (signed char*)calloc(PROF_CAP, 1);
@@ -286,6 +365,7 @@ extern "C" qlga_status qlga_profile_enable(qlga_ctx* c, int on) {
 
 extern "C" qlga_status qlga_profile_read(qlga_ctx* c, qlga_profile* out) {
     if (!c || !out) return c ? fail(c, QLGA_EINVAL, "qlga_profile_read: NULL") : QLGA_EINVAL;
+    DeviceGuard guard(c);
     memset(out, 0, sizeof(*out));
     CU(c, cudaStreamSynchronize(c->stream));
     for (int k = 0; k + 1 < c->prof_n; ++k) {
@@ -318,8 +398,33 @@ static qlga_status ensure_stage(qlga_ctx* c) {
     return QLGA_OK;
 }
 
+// grow-only scratch for the diagnostics that return data to the host: no cudaMalloc / cudaFree
+// (implicit device synchronisations) on a path meant to run every few steps
+static qlga_status ensure_scratch(qlga_ctx* c, size_t bytes) {
+    if (c->scratch_bytes >= bytes && c->d_scratch) return QLGA_OK;
+    if (c->d_scratch) { cudaStreamSynchronize(c->stream); cudaFree(c->d_scratch); c->d_scratch = nullptr; c->scratch_bytes = 0; }
+    bytes = (bytes + 255) & ~(size_t)255;
+    if (cudaMalloc(&c->d_scratch, bytes) != cudaSuccess) { cudaGetLastError(); return fail(c, QLGA_ENOMEM, "cudaMalloc(diagnostics scratch) failed"); }
+    c->scratch_bytes = bytes;
+    return QLGA_OK;
+}
+
+// The kernels raise the device error word when an interaction angle is not finite or beyond the cap of the
+// general path (a state that is not a wavefunction: Inf / NaN / absurd amplitudes).  Calls that synchronise
+// anyway read it; the stream must be idle.  Reports once and clears the word.
+static qlga_status check_device_flag(qlga_ctx* c, const char* who) {
+    int h = 0;
+    CU(c, cudaMemcpyAsync(&h, c->d_flag, sizeof(int), cudaMemcpyDeviceToHost, c->stream));
+    CU(c, cudaStreamSynchronize(c->stream));
+    if (h == 0) return QLGA_OK;
+    CU(c, cudaMemsetAsync(c->d_flag, 0, sizeof(int), c->stream));
+    return fail(c, QLGA_ESTATE, "%s: an interaction angle was not finite or beyond the supported range "
+                                "(2048 rad per application): the state is not a valid wavefunction", who);
+}
+
 extern "C" qlga_status qlga_set_state_q(qlga_ctx* c, const void* q, int src_on_device) {
     if (!c || !q) return c ? fail(c, QLGA_EINVAL, "qlga_set_state_q: NULL") : QLGA_EINVAL;
+    DeviceGuard guard(c);
     CU(c, cudaMemcpyAsync(c->buf[0], q, state_bytes(c),
                           src_on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, c->stream));
     if (!src_on_device) CU(c, cudaStreamSynchronize(c->stream));   // host buffer may be reused on return
@@ -329,19 +434,20 @@ extern "C" qlga_status qlga_set_state_q(qlga_ctx* c, const void* q, int src_on_d
 
 extern "C" qlga_status qlga_get_state_q(qlga_ctx* c, void* q, int dst_on_device) {
     if (!c || !q) return c ? fail(c, QLGA_EINVAL, "qlga_get_state_q: NULL") : QLGA_EINVAL;
+    DeviceGuard guard(c);
     if (!c->have_state) return fail(c, QLGA_ESTATE, "qlga_get_state_q: no state set");
     CU(c, cudaMemcpyAsync(q, c->buf[c->cur], state_bytes(c),
                           dst_on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost, c->stream));
-    CU(c, cudaStreamSynchronize(c->stream));
-    return QLGA_OK;
+    return check_device_flag(c, "qlga_get_state_q");
 }
 
 extern "C" qlga_status qlga_set_state_psi(qlga_ctx* c, const void* psi, int src_on_device) {
     if (!c || !psi) return c ? fail(c, QLGA_EINVAL, "qlga_set_state_psi: NULL") : QLGA_EINVAL;
+    DeviceGuard guard(c);
     const int64_t n = nsites(c);
-    Launch L{c->stream, &c->launches};
+    Launch L{c->stream, &c->launches, c->device};
     if (src_on_device) {
-        CU(c, launch_split_psi(L, c->prec, psi, c->buf[0], n, 0, n));
+        CU(c, launch_split_psi(L, storage_prec(c), psi, c->buf[0], n, 0, n));
     } else {
         qlga_status st = ensure_stage(c);
         if (st != QLGA_OK) return st;
@@ -353,7 +459,7 @@ extern "C" qlga_status qlga_set_state_psi(qlga_ctx* c, const void* psi, int src_
                 CU(c, cudaMemcpyAsync((char*)c->d_stage + (size_t)j * cnt * cb,
                                       (const char*)psi + ((size_t)j * n + off) * cb, (size_t)cnt * cb,
                                       cudaMemcpyHostToDevice, c->stream));
-            CU(c, launch_split_psi(L, c->prec, c->d_stage, c->buf[0], n, off, cnt));
+            CU(c, launch_split_psi(L, storage_prec(c), c->d_stage, c->buf[0], n, off, cnt));
         }
         CU(c, cudaStreamSynchronize(c->stream));
     }
@@ -363,11 +469,12 @@ extern "C" qlga_status qlga_set_state_psi(qlga_ctx* c, const void* psi, int src_
 
 extern "C" qlga_status qlga_get_state_psi(qlga_ctx* c, void* psi, int dst_on_device) {
     if (!c || !psi) return c ? fail(c, QLGA_EINVAL, "qlga_get_state_psi: NULL") : QLGA_EINVAL;
+    DeviceGuard guard(c);
     if (!c->have_state) return fail(c, QLGA_ESTATE, "qlga_get_state_psi: no state set");
     const int64_t n = nsites(c);
-    Launch L{c->stream, &c->launches};
+    Launch L{c->stream, &c->launches, c->device};
     if (dst_on_device) {
-        CU(c, launch_sum_psi(L, c->prec, c->buf[c->cur], psi, n, 0, n));
+        CU(c, launch_sum_psi(L, storage_prec(c), c->buf[c->cur], psi, n, 0, n));
     } else {
         qlga_status st = ensure_stage(c);
         if (st != QLGA_OK) return st;
@@ -375,15 +482,14 @@ extern "C" qlga_status qlga_get_state_psi(qlga_ctx* c, void* psi, int dst_on_dev
         const int64_t chunk = (int64_t)(c->stage_bytes / (5 * cb));
         for (int64_t off = 0; off < n; off += chunk) {
             const int64_t cnt = (n - off < chunk) ? n - off : chunk;
-            CU(c, launch_sum_psi(L, c->prec, c->buf[c->cur], c->d_stage, n, off, cnt));
+            CU(c, launch_sum_psi(L, storage_prec(c), c->buf[c->cur], c->d_stage, n, off, cnt));
             for (int j = 0; j < 5; ++j)
                 CU(c, cudaMemcpyAsync((char*)psi + ((size_t)j * n + off) * cb,
                                       (const char*)c->d_stage + (size_t)j * cnt * cb, (size_t)cnt * cb,
                                       cudaMemcpyDeviceToHost, c->stream));
         }
     }
-    CU(c, cudaStreamSynchronize(c->stream));
-    return QLGA_OK;
+    return check_device_flag(c, "qlga_get_state_psi");
 }
 
 // ---------------------------------------------------------------------------
@@ -403,6 +509,7 @@ static void fill_pass_consts(const qlga_ctx* c, PassParams& P, double s) {
     P.utail = 0;
     P.gt[0] = s * c->c[0]; P.gt[1] = s * c->c[1]; P.gt[2] = s * c->c[2] / 5.0;
     P.out_scale = 0.0625;
+    P.flag = c->d_flag;
     P.tab = c->tab;
 }
 
@@ -413,7 +520,7 @@ static int pick_other(const qlga_ctx* c, int a, int b) {   // a buffer index dif
 }
 
 static qlga_status step_fused(qlga_ctx* c, int64_t nsteps) {
-    Launch L{c->stream, &c->launches};
+    Launch L{c->stream, &c->launches, c->device};
     const bool inter = c->order == QLGA_INTERLEAVED;
     const double s = inter ? 1.0 / (4.0 * c->ndim) : 1.0;
     PassParams P;
@@ -490,6 +597,9 @@ static qlga_status step_fused(qlga_ctx* c, int64_t nsteps) {
                     if (thr == 0) thr = (P.umode != 0 && f64) ? 128 : 256;
                 } else if (c->ndim == 3 && c->prec == QLGA_F64) { cxw = 2; if (thr == 0) thr = 128; }
             }
+            if (!pass_tile_supported(d == 0 ? 0 : 1, d == 0 ? c->threads_x : thr, d == 0 ? 1 : cxw))
+                return fail(c, QLGA_EINVAL, "qlga_step: no kernel for the (TILE_Y, THREADS_Y) pair this pass resolves to; "
+                                            "set both options or neither (qlga.h)");
             CU(c, launch_pass(L, c->prec, d, P, d == 0 ? c->threads_x : thr, d == 0 ? 1 : cxw));
             src = dst;
         }
@@ -502,17 +612,17 @@ static qlga_status step_fused(qlga_ctx* c, int64_t nsteps) {
 }
 
 static qlga_status step_per_operator(qlga_ctx* c, int64_t nsteps) {
-    Launch L{c->stream, &c->launches};
+    Launch L{c->stream, &c->launches, c->device};
     const bool inter = c->order == QLGA_INTERLEAVED;
     const double s = inter ? 1.0 / (4.0 * c->ndim) : 1.0;
     const double g[3] = {s * c->c[0], s * c->c[1], s * c->c[2] / 5.0};
     for (int64_t t = 0; t < nsteps; ++t) {
         prof_mark(c, 2);
-        if (!inter) CU(c, launch_interaction(L, c->prec, c->buf[c->cur], nsites(c), g, s * c->mu, c->tab));
+        if (!inter) CU(c, launch_interaction(L, c->prec, c->buf[c->cur], nsites(c), g, s * c->mu, c->tab, c->d_flag));
         for (int d = c->ndim - 1; d >= 0; --d)
             for (int k = 0; k < 4; ++k) {
                 const int sigma = (k < 2) ? 1 : 0;                     // components 2, 2, 1, 1
-                if (inter) CU(c, launch_interaction(L, c->prec, c->buf[c->cur], nsites(c), g, s * c->mu, c->tab));
+                if (inter) CU(c, launch_interaction(L, c->prec, c->buf[c->cur], nsites(c), g, s * c->mu, c->tab, c->d_flag));
                 const int dst = pick_other(c, c->cur, -1);
                 CU(c, launch_kinetic(L, c->prec, c->buf[c->cur], c->buf[dst], c->nx, c->ny, c->nz, d, sigma));
                 c->cur = dst;
@@ -532,6 +642,7 @@ extern "C" qlga_status qlga_set_chemical_potential(qlga_ctx* c, double mu) {
 
 extern "C" qlga_status qlga_step(qlga_ctx* c, int64_t n) {
     if (!c) return QLGA_EINVAL;
+    DeviceGuard guard(c);
     if (n < 0) return fail(c, QLGA_EINVAL, "qlga_step: n < 0");
     if (!c->have_state) return fail(c, QLGA_ESTATE, "qlga_step: no state set");
     if (n == 0) return QLGA_OK;
@@ -549,17 +660,19 @@ static int64_t layer_sites(const qlga_ctx* c) { return nsites(c) / slow_extent(c
 
 extern "C" qlga_status qlga_observable_sums(qlga_ctx* c, double* host_sums) {
     if (!c || !host_sums) return c ? fail(c, QLGA_EINVAL, "qlga_observable_sums: NULL") : QLGA_EINVAL;
+    DeviceGuard guard(c);
     if (!c->have_state) return fail(c, QLGA_ESTATE, "qlga_observable_sums: no state set");
-    Launch L{c->stream, &c->launches};
+    Launch L{c->stream, &c->launches, c->device};
     const void* prev = (c->prev >= 0) ? c->buf[c->prev] : nullptr;
     const int64_t r0 = c->ghost * layer_sites(c), r1 = nsites(c) - r0;      // owned layers
     int blocks = c->obs_blocks;
     if ((int64_t)blocks * 256 > r1 - r0) blocks = (int)((r1 - r0 + 255) / 256);
-    CU(c, launch_observables(L, c->prec, c->buf[c->cur], prev, c->nx, c->ny, c->nz, c->ndim, r0, r1,
+    CU(c, launch_observables(L, storage_prec(c), c->buf[c->cur], prev, c->nx, c->ny, c->nz, c->ndim, r0, r1,
                              c->d_partials, blocks, c->d_sums));
     double h[OBS_NACC];
     CU(c, cudaMemcpyAsync(h, c->d_sums, sizeof(h), cudaMemcpyDeviceToHost, c->stream));
-    CU(c, cudaStreamSynchronize(c->stream));
+    const qlga_status fst = check_device_flag(c, "qlga_observables");       // synchronises the stream
+    if (fst != QLGA_OK) return fst;
     for (int k = 0; k < 15; ++k) host_sums[k] = h[k];
     host_sums[15] = prev ? h[15] : NAN;
     host_sums[16] = prev ? h[16] : NAN;
@@ -593,6 +706,32 @@ extern "C" qlga_status qlga_observables(qlga_ctx* c, qlga_obs* out) {
     return qlga_observables_from_sums(c, h, out);
 }
 
+extern "C" qlga_status qlga_angle_stats(qlga_ctx* c, qlga_angles* out) {
+    if (!c || !out) return c ? fail(c, QLGA_EINVAL, "qlga_angle_stats: NULL") : QLGA_EINVAL;
+    DeviceGuard guard(c);
+    if (!c->have_state) return fail(c, QLGA_ESTATE, "qlga_angle_stats: no state set");
+    const qlga_status st = ensure_scratch(c, 15 * sizeof(unsigned long long));
+    if (st != QLGA_OK) return st;
+    Launch L{c->stream, &c->launches, c->device};
+    const double s = c->order == QLGA_INTERLEAVED ? 1.0 / (4.0 * c->ndim) : 1.0;
+    unsigned long long* d = (unsigned long long*)c->d_scratch;
+    unsigned long long h[15];
+    CU(c, cudaMemsetAsync(d, 0, sizeof(h), c->stream));
+    int blocks = c->obs_blocks;
+    if ((int64_t)blocks * 256 > nsites(c)) blocks = (int)((nsites(c) + 255) / 256);
+    CU(c, launch_angle_stats(L, storage_prec(c), c->buf[c->cur], nsites(c), 2.0 * fabs(s * c->c[1]), fabs(s * c->c[2]) / 5.0,
+                             s * c->c[0], s * c->mu, c->tab, blocks, d));
+    CU(c, cudaMemcpyAsync(h, d, sizeof(h), cudaMemcpyDeviceToHost, c->stream));
+    CU(c, cudaStreamSynchronize(c->stream));
+    double sum; unsigned int mx[2];
+    memcpy(&sum, &h[0], sizeof(double)); memcpy(mx, &h[1], sizeof(mx));
+    float tmax, pmax;
+    memcpy(&tmax, &mx[0], 4); memcpy(&pmax, &mx[1], 4);
+    out->theta_max = tmax; out->theta_mean = sum / (double)nsites(c); out->phase_max = pmax;
+    for (int p = 0; p < 13; ++p) out->degree_hist[p] = (int64_t)h[2 + p];
+    return QLGA_OK;
+}
+
 // ---- slab decomposition: ghost / edge layers of the slowest axis ------------------------------
 extern "C" qlga_status qlga_slab_configure(qlga_ctx* c, int64_t ghost) {
     if (!c) return QLGA_EINVAL;
@@ -620,6 +759,7 @@ static qlga_status slab_copy(qlga_ctx* c, const char* what, int64_t first, void*
 extern "C" qlga_status qlga_slab_edge_get(qlga_ctx* c, int side, void* dev_out) {
     if (!c || !dev_out || (side != 0 && side != 1))
         return c ? fail(c, QLGA_EINVAL, "qlga_slab_edge_get: bad arguments") : QLGA_EINVAL;
+    DeviceGuard guard(c);
     if (!c->have_state || c->ghost <= 0) return fail(c, QLGA_ESTATE, "qlga_slab_edge_get: no state, or not a slab");
     const int64_t first = side == 0 ? c->ghost : slow_extent(c) - 2 * c->ghost;
     return slab_copy(c, "qlga_slab_edge_get", first, dev_out, true);
@@ -628,6 +768,7 @@ extern "C" qlga_status qlga_slab_edge_get(qlga_ctx* c, int side, void* dev_out) 
 extern "C" qlga_status qlga_slab_ghost_set(qlga_ctx* c, int side, const void* dev_in) {
     if (!c || !dev_in || (side != 0 && side != 1))
         return c ? fail(c, QLGA_EINVAL, "qlga_slab_ghost_set: bad arguments") : QLGA_EINVAL;
+    DeviceGuard guard(c);
     if (!c->have_state || c->ghost <= 0) return fail(c, QLGA_ESTATE, "qlga_slab_ghost_set: no state, or not a slab");
     const int64_t first = side == 0 ? 0 : slow_extent(c) - c->ghost;
     return slab_copy(c, "qlga_slab_ghost_set", first, const_cast<void*>(dev_in), false);
@@ -635,12 +776,13 @@ extern "C" qlga_status qlga_slab_ghost_set(qlga_ctx* c, int side, const void* de
 
 extern "C" qlga_status qlga_vorticity(qlga_ctx* c, void* omega, int dst_on_device) {
     if (!c || !omega) return c ? fail(c, QLGA_EINVAL, "qlga_vorticity: NULL") : QLGA_EINVAL;
+    DeviceGuard guard(c);
     if (c->ndim != 2) return fail(c, QLGA_EUNSUP, "qlga_vorticity: 2D lattices only");
     if (!c->have_state) return fail(c, QLGA_ESTATE, "qlga_vorticity: no state set");
-    Launch L{c->stream, &c->launches};
+    Launch L{c->stream, &c->launches, c->device};
     const size_t bytes = (size_t)5 * c->nx * c->ny * real_size(c->prec);
     if (dst_on_device) {
-        CU(c, launch_vorticity(L, c->prec, c->buf[c->cur], omega, c->nx, c->ny));
+        CU(c, launch_vorticity(L, storage_prec(c), c->buf[c->cur], omega, c->nx, c->ny));
         return QLGA_OK;
     }
     // host destination: a buffer that holds neither the current nor the previous
@@ -649,16 +791,14 @@ extern "C" qlga_status qlga_vorticity(qlga_ctx* c, void* omega, int dst_on_devic
     for (int k = 0; k < 3; ++k)
         if (c->buf[k] && k != c->cur && k != c->prev) scratch = k;
     void* tmp = scratch >= 0 ? c->buf[scratch] : nullptr;
-    bool own = false;
     if (!tmp) {
-        cudaError_t e = cudaMalloc(&tmp, bytes);
-        if (e != cudaSuccess) { cudaGetLastError(); return fail(c, QLGA_ENOMEM, "qlga_vorticity: cudaMalloc failed"); }
-        own = true;
+        const qlga_status st = ensure_scratch(c, bytes);
+        if (st != QLGA_OK) return st;
+        tmp = c->d_scratch;
     }
-    cudaError_t e = launch_vorticity(L, c->prec, c->buf[c->cur], tmp, c->nx, c->ny);
+    cudaError_t e = launch_vorticity(L, storage_prec(c), c->buf[c->cur], tmp, c->nx, c->ny);
     if (e == cudaSuccess) e = cudaMemcpyAsync(omega, tmp, bytes, cudaMemcpyDeviceToHost, c->stream);
     if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
-    if (own) cudaFree(tmp);
     if (e != cudaSuccess) return cuda_fail(c, "qlga_vorticity", e);
     return QLGA_OK;
 }
@@ -668,45 +808,46 @@ extern "C" qlga_status qlga_vorticity(qlga_ctx* c, void* omega, int dst_on_devic
 // ---------------------------------------------------------------------------
 extern "C" qlga_status qlga_density(qlga_ctx* c, void* rho, int dst_on_device) {
     if (!c || !rho) return c ? fail(c, QLGA_EINVAL, "qlga_density: NULL") : QLGA_EINVAL;
+    DeviceGuard guard(c);
     if (!c->have_state) return fail(c, QLGA_ESTATE, "qlga_density: no state set");
-    Launch L{c->stream, &c->launches};
+    Launch L{c->stream, &c->launches, c->device};
     const int64_t n = nsites(c);
     const size_t bytes = (size_t)n * real_size(c->prec);
     if (dst_on_device) {
-        CU(c, launch_density(L, c->prec, c->buf[c->cur], rho, n));
+        CU(c, launch_density(L, storage_prec(c), c->buf[c->cur], rho, n));
         return QLGA_OK;
     }
-    void* tmp = nullptr;
-    if (cudaMalloc(&tmp, bytes) != cudaSuccess) { cudaGetLastError(); return fail(c, QLGA_ENOMEM, "qlga_density: cudaMalloc failed"); }
-    cudaError_t e = launch_density(L, c->prec, c->buf[c->cur], tmp, n);
+    const qlga_status st = ensure_scratch(c, bytes);
+    if (st != QLGA_OK) return st;
+    void* tmp = c->d_scratch;
+    cudaError_t e = launch_density(L, storage_prec(c), c->buf[c->cur], tmp, n);
     if (e == cudaSuccess) e = cudaMemcpyAsync(rho, tmp, bytes, cudaMemcpyDeviceToHost, c->stream);
     if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
-    cudaFree(tmp);
     if (e != cudaSuccess) return cuda_fail(c, "qlga_density", e);
     return QLGA_OK;
 }
 
 extern "C" qlga_status qlga_density_l2_error(qlga_ctx* c, const void* rho_ref, int src_on_device, double* host_eps) {
     if (!c || !rho_ref || !host_eps) return c ? fail(c, QLGA_EINVAL, "qlga_density_l2_error: NULL") : QLGA_EINVAL;
+    DeviceGuard guard(c);
     if (!c->have_state) return fail(c, QLGA_ESTATE, "qlga_density_l2_error: no state set");
-    Launch L{c->stream, &c->launches};
+    Launch L{c->stream, &c->launches, c->device};
     const int64_t n = nsites(c);
     const size_t bytes = (size_t)n * real_size(c->prec);
-    void* tmp = nullptr;
     const void* ref = rho_ref;
     if (!src_on_device) {
-        if (cudaMalloc(&tmp, bytes) != cudaSuccess) { cudaGetLastError(); return fail(c, QLGA_ENOMEM, "qlga_density_l2_error: cudaMalloc failed"); }
-        cudaError_t e0 = cudaMemcpyAsync(tmp, rho_ref, bytes, cudaMemcpyHostToDevice, c->stream);
-        if (e0 != cudaSuccess) { cudaFree(tmp); return cuda_fail(c, "qlga_density_l2_error: H2D", e0); }
-        ref = tmp;
+        const qlga_status st = ensure_scratch(c, bytes);
+        if (st != QLGA_OK) return st;
+        cudaError_t e0 = cudaMemcpyAsync(c->d_scratch, rho_ref, bytes, cudaMemcpyHostToDevice, c->stream);
+        if (e0 != cudaSuccess) return cuda_fail(c, "qlga_density_l2_error: H2D", e0);
+        ref = c->d_scratch;
     }
     int blocks = c->obs_blocks;
     if ((int64_t)blocks * 256 > n) blocks = (int)((n + 255) / 256);
     double h = 0.0;
-    cudaError_t e = launch_l2_error(L, c->prec, c->buf[c->cur], ref, n, c->d_partials, blocks, c->d_sums);
+    cudaError_t e = launch_l2_error(L, storage_prec(c), c->buf[c->cur], ref, n, c->d_partials, blocks, c->d_sums);
     if (e == cudaSuccess) e = cudaMemcpyAsync(&h, c->d_sums, sizeof(double), cudaMemcpyDeviceToHost, c->stream);
     if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
-    if (tmp) cudaFree(tmp);
     if (e != cudaSuccess) return cuda_fail(c, "qlga_density_l2_error", e);
     *host_eps = h;
     return QLGA_OK;
@@ -715,26 +856,26 @@ extern "C" qlga_status qlga_density_l2_error(qlga_ctx* c, const void* rho_ref, i
 extern "C" qlga_status qlga_vortices(qlga_ctx* c, int32_t* host_out, int64_t max_out, int64_t* host_count) {
     if (!c || !host_count || max_out < 0 || (max_out > 0 && !host_out))
         return c ? fail(c, QLGA_EINVAL, "qlga_vortices: bad arguments") : QLGA_EINVAL;
+    DeviceGuard guard(c);
     if (c->ndim != 2) return fail(c, QLGA_EUNSUP, "qlga_vortices: 2D lattices only");
     if (!c->have_state) return fail(c, QLGA_ESTATE, "qlga_vortices: no state set");
-    Launch L{c->stream, &c->launches};
-    int* list = nullptr;
-    unsigned long long* counter = nullptr;
+    Launch L{c->stream, &c->launches, c->device};
+    // scratch layout: [counter (16 bytes)][records]
     const size_t lbytes = (size_t)(max_out > 0 ? max_out : 1) * 4 * sizeof(int);
-    if (cudaMalloc(&list, lbytes) != cudaSuccess || cudaMalloc(&counter, sizeof(unsigned long long)) != cudaSuccess) {
-        cudaGetLastError(); cudaFree(list);
-        return fail(c, QLGA_ENOMEM, "qlga_vortices: cudaMalloc failed");
-    }
+    const qlga_status sst = ensure_scratch(c, 16 + lbytes);
+    if (sst != QLGA_OK) return sst;
+    unsigned long long* counter = (unsigned long long*)c->d_scratch;
+    int* list = (int*)((char*)c->d_scratch + 16);
     unsigned long long hc = 0;
     cudaError_t e = cudaMemsetAsync(counter, 0, sizeof(unsigned long long), c->stream);
-    if (e == cudaSuccess) e = launch_vortices(L, c->prec, c->buf[c->cur], c->nx, c->ny, list, (long long)max_out, counter);
+    if (e == cudaSuccess) e = launch_vortices(L, storage_prec(c), c->buf[c->cur], c->nx, c->ny, list, (long long)max_out, counter);
     if (e == cudaSuccess) e = cudaMemcpyAsync(&hc, counter, sizeof(hc), cudaMemcpyDeviceToHost, c->stream);
     if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
     if (e == cudaSuccess && max_out > 0) {
         const unsigned long long ncopy = hc < (unsigned long long)max_out ? hc : (unsigned long long)max_out;
-        if (ncopy) e = cudaMemcpy(host_out, list, (size_t)ncopy * 4 * sizeof(int), cudaMemcpyDeviceToHost);
+        if (ncopy) e = cudaMemcpyAsync(host_out, list, (size_t)ncopy * 4 * sizeof(int), cudaMemcpyDeviceToHost, c->stream);
+        if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
     }
-    cudaFree(list); cudaFree(counter);
     if (e != cudaSuccess) return cuda_fail(c, "qlga_vortices", e);
     *host_count = (int64_t)hc;
     return QLGA_OK;

@@ -405,4 +405,69 @@ cudaError_t launch_vortices(const Launch& L, qlga_prec prec, const void* q, int6
     return cudaGetLastError();
 }
 
+// ---------------------------------------------------------------------------
+// Interaction-angle statistics (qlga_angle_stats): per site the angle bound the pass kernels select
+// the polynomial degree by, theta = s (2|c1||F| + |c2| rho / 5), and the scalar phase s (c0 rho + mu).
+// out: [0] double sum theta, [1] uint bits of max theta | uint bits of max |phase|, [2..14] degree histogram.
+// ---------------------------------------------------------------------------
+template <typename T>
+__global__ void __launch_bounds__(256) angle_stats_kernel(const typename vec2<T>::type* q, int64_t n,
+                                                          double tg1, double tg2, double g0, double smu,
+                                                          const __grid_constant__ ExpTable tab,
+                                                          unsigned long long* out) {
+    __shared__ unsigned int sh_hist[13];
+    __shared__ unsigned int sh_max[2];
+    __shared__ double sh_sum[8];
+    if (threadIdx.x < 13) sh_hist[threadIdx.x] = 0;
+    if (threadIdx.x < 2) sh_max[threadIdx.x] = 0;
+    __syncthreads();
+    double sum = 0.0;
+    float tmax = 0.f, pmax = 0.f;
+    const double rt6 = 2.4494897427831780981972840747059;
+    for (int64_t r = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; r < n; r += (int64_t)gridDim.x * blockDim.x) {
+        double pr[5], pi[5], nm[5];
+        load_psi<T>(q, n, r, pr, pi, nullptr);
+#pragma unroll
+        for (int j = 0; j < 5; ++j) nm[j] = pr[j] * pr[j] + pi[j] * pi[j];
+        const double rho = nm[0] + nm[1] + nm[2] + nm[3] + nm[4];
+        const double Fz = 2.0 * (nm[0] - nm[4]) + (nm[1] - nm[3]);
+        const double far_ = pr[0] * pr[1] + pi[0] * pi[1] + pr[3] * pr[4] + pi[3] * pi[4];
+        const double fai = pr[0] * pi[1] - pi[0] * pr[1] + pr[3] * pi[4] - pi[3] * pr[4];
+        const double fbr = pr[1] * pr[2] + pi[1] * pi[2] + pr[2] * pr[3] + pi[2] * pi[3];
+        const double fbi = pr[1] * pi[2] - pi[1] * pr[2] + pr[2] * pi[3] - pi[2] * pr[3];
+        const double Fx = 2.0 * far_ + rt6 * fbr, Fy = 2.0 * fai + rt6 * fbi;
+        const double theta = tg1 * sqrt(Fx * Fx + Fy * Fy + Fz * Fz) + tg2 * rho;
+        const float th = (float)theta;
+        sum += theta;
+        tmax = fmaxf(tmax, th);
+        pmax = fmaxf(pmax, (float)fabs(g0 * rho + smu));
+        int p = 0;
+        if (th <= tab.theta_split) p = lut_degree(tab, th * 1.0009765625f);
+        atomicAdd(&sh_hist[p], 1u);
+    }
+    atomicMax(&sh_max[0], __float_as_uint(tmax));
+    atomicMax(&sh_max[1], __float_as_uint(pmax));
+    for (int o = 16; o > 0; o >>= 1) sum += __shfl_xor_sync(0xffffffffu, sum, o);
+    if ((threadIdx.x & 31) == 0) sh_sum[threadIdx.x >> 5] = sum;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double s = 0.0;
+        for (int w = 0; w < 8; ++w) s += sh_sum[w];
+        atomicAdd(reinterpret_cast<double*>(out), s);
+        atomicMax(reinterpret_cast<unsigned int*>(out + 1), sh_max[0]);
+        atomicMax(reinterpret_cast<unsigned int*>(out + 1) + 1, sh_max[1]);
+    }
+    if (threadIdx.x < 13 && sh_hist[threadIdx.x]) atomicAdd(out + 2 + threadIdx.x, (unsigned long long)sh_hist[threadIdx.x]);
+}
+
+cudaError_t launch_angle_stats(const Launch& L, qlga_prec prec, const void* q, int64_t n, double tg1, double tg2,
+                               double g0, double smu, const ExpTable& tab, int nblocks, unsigned long long* out) {
+    if (prec == QLGA_F64)
+        angle_stats_kernel<double><<<nblocks, 256, 0, L.stream>>>((const double2*)q, n, tg1, tg2, g0, smu, tab, out);
+    else
+        angle_stats_kernel<float><<<nblocks, 256, 0, L.stream>>>((const float2*)q, n, tg1, tg2, g0, smu, tab, out);
+    ++*L.counter;
+    return cudaGetLastError();
+}
+
 }  // namespace qlga

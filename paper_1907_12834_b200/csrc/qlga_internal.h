@@ -23,28 +23,37 @@ struct PassParams {
     int utail;             // plain ordering: apply the NEXT step's U (constants gt) after this pass's last factor
     double gt[3];          // (c0, c1, c2/5): the full-angle U on the unscaled state
     double out_scale;      // 2^-4, applied after the 4 factors of a step
+    int* flag;             // device error word of the context (FLAG_* in qlga_math.cuh)
     ExpTable tab;
 };
 
 struct Launch {
     cudaStream_t stream;
     int64_t* counter;      // incremented per kernel launched
+    int device;            // the context's device (per-device function attributes)
 };
 
 // fused passes (qlga_step.cu); dir = 0 (x), 1 (y) or 2 (z).  `threads` / `cx` are tunables
 // (0 = default).  Returns cudaGetLastError().
 cudaError_t launch_pass(const Launch& L, qlga_prec prec, int dir, const PassParams& P,
                         int threads, int cx);
+// the three instantiation sets (qlga_step.cu, qlga_step_f32.cu, qlga_step_mixed.cu)
+cudaError_t launch_pass_f64(const Launch& L, int dir, const PassParams& P, int threads, int cx);
+cudaError_t launch_pass_f32(const Launch& L, int dir, const PassParams& P, int threads, int cx);
+cudaError_t launch_pass_mixed(const Launch& L, int dir, const PassParams& P, int threads, int cx);
+// true if the (columns, threads) pair of a strided pass / the CTA size of the x pass has an instantiation
+bool pass_tile_supported(int dir, int threads, int cx);
 // widest ksteps the x pass supports with the given CTA size
 int max_ksteps(int threads);
 
 // one kernel per operator (reference path on the GPU)
 cudaError_t launch_interaction(const Launch& L, qlga_prec prec, void* q, int64_t nsites,
-                               const double g[3], double smu, const ExpTable& tab);
+                               const double g[3], double smu, const ExpTable& tab, int* flag);
 cudaError_t launch_kinetic(const Launch& L, qlga_prec prec, const void* src, void* dst,
                            int64_t nx, int64_t ny, int64_t nz, int dir, int sigma);
 
-// diagnostics and state conversion (qlga_diag.cu)
+// diagnostics and state conversion (qlga_diag.cu); `prec` here is the STORAGE precision
+// (QLGA_F32X stores fp32: callers pass storage_prec())
 constexpr int OBS_NACC = 19;   // accumulators per block, see qlga_diag.cu
 cudaError_t launch_observables(const Launch& L, qlga_prec prec, const void* q, const void* qprev,
                                int64_t nx, int64_t ny, int64_t nz, int ndim, int64_t r0, int64_t r1,
@@ -56,6 +65,8 @@ cudaError_t launch_l2_error(const Launch& L, qlga_prec prec, const void* q, cons
                             double* partials, int nblocks, double* sums);
 cudaError_t launch_vortices(const Launch& L, qlga_prec prec, const void* q, int64_t nx, int64_t ny,
                             int* list, long long max_out, unsigned long long* counter);
+cudaError_t launch_angle_stats(const Launch& L, qlga_prec prec, const void* q, int64_t nsites, double tg1, double tg2,
+                               double g0, double smu, const ExpTable& tab, int nblocks, unsigned long long* out /*[15]*/);
 cudaError_t launch_split_psi(const Launch& L, qlga_prec prec, const void* psi, void* q,
                              int64_t nsites, int64_t offset, int64_t count);
 cudaError_t launch_sum_psi(const Launch& L, qlga_prec prec, const void* q, void* psi,
@@ -64,6 +75,7 @@ cudaError_t launch_sum_psi(const Launch& L, qlga_prec prec, const void* q, void*
 }  // namespace qlga
 
 struct qlga_ctx {
+    int device;            // CUDA device the context (its buffers, stream and scratch) lives on
     int ndim;
     int64_t nx, ny, nz;
     double c[3];
@@ -84,6 +96,8 @@ struct qlga_ctx {
     int steps_per_launch;  // 1D temporal blocking, 0 = auto
     int fuse_plain_u;      // plain ordering, 2D/3D: the next step's U rides on the x pass (default on)
     int tol_log2;
+    int exp_poly;          // 0 economised, 1 Taylor (QLGA_OPT_EXP_POLY)
+    int f32_phase;         // phase-factor formulation of the fp32 kernels (QLGA_OPT_F32_PHASE)
     int threads_x;
     int tile_y;
     int threads_y;
@@ -94,6 +108,9 @@ struct qlga_ctx {
     int obs_blocks;
     void* d_stage;         // staging for psi transfers
     size_t stage_bytes;
+    void* d_scratch;       // grow-only scratch of the diagnostics with a host destination (density, omega, vortex lists)
+    size_t scratch_bytes;
+    int* d_flag;           // device error word (FLAG_* in qlga_math.cuh), read by the synchronising calls
     // kernel timing hooks (qlga_profile_*)
     int prof_on;
     int prof_n;

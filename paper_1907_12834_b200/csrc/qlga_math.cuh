@@ -162,6 +162,21 @@ __device__ __forceinline__ void sincos_small(T x, const SinCosTable& t, T* s, T*
     *c = fma(z, pc, (T)1);
     *s = fma(x * z, ps, x);
 }
+// the same with cos x - 1 instead of cos x: the small quantity is kept to its own relative
+// precision instead of being rounded onto 1 (see interaction(), phase modes)
+template <typename T>
+__device__ __forceinline__ void sincos_small_m1(T x, const SinCosTable& t, T* s, T* cm1) {
+    const T z = x * x;
+    const T* cc = sc_cos(t, x);
+    const T* cs = sc_sin(t, x);
+    T pc = cc[6], ps = cs[5];
+#pragma unroll
+    for (int k = 5; k >= 0; --k) pc = fma(z, pc, cc[k]);
+#pragma unroll
+    for (int k = 4; k >= 0; --k) ps = fma(z, ps, cs[k]);
+    *cm1 = z * pc;
+    *s = fma(x * z, ps, x);
+}
 __device__ __forceinline__ void sincos_lib(double x, double* s, double* c) { sincos(x, s, c); }
 __device__ __forceinline__ void sincos_lib(float x, float* s, float* c) { sincosf(x, s, c); }
 
@@ -231,6 +246,9 @@ struct ExpTable {
     double b0[QLGA_PMAX];
     float rf[QLGA_PMAX][QLGA_PMAX + 1];   // the same rounded to fp32 (no conversions in the fp32 loops)
     float b0f[QLGA_PMAX];
+    double b0m1[QLGA_PMAX];     // b0 - 1, kept to its own precision (phase modes 1, 2)
+    float b0m1f[QLGA_PMAX];
+    int phase_mode;             // see interaction(): 0 = phase factor as (cos, -sin), 1 = as 1 + d, 2 = 1 + d with d in fp64
     float thr[QLGA_PMAX];       // thr[p-1] = largest angle degree p serves within the tolerance
     float theta_split;          // angles above this are split into equal sub-angles
     SinCosTable sc;
@@ -251,6 +269,8 @@ __device__ __forceinline__ const double* exp_ratios(const ExpTable& t, int p, do
 __device__ __forceinline__ const float* exp_ratios(const ExpTable& t, int p, float) { return t.rf[p - 1]; }
 __device__ __forceinline__ double exp_b0(const ExpTable& t, int p, double) { return t.b0[p - 1]; }
 __device__ __forceinline__ float exp_b0(const ExpTable& t, int p, float) { return t.b0f[p - 1]; }
+__device__ __forceinline__ double exp_b0m1(const ExpTable& t, int p, double) { return t.b0m1[p - 1]; }
+__device__ __forceinline__ float exp_b0m1(const ExpTable& t, int p, float) { return t.b0m1f[p - 1]; }
 
 // w = (s K') u  with  s K' = g1 F'.f + g2 |chi'><chi'|,
 //   (F'.f u)_m = m F_z u_m + (1/2)|F_+| (alpha_{m-1} u_{m-1} + alpha_m u_{m+1}),
@@ -431,14 +451,32 @@ __device__ __forceinline__ void horner(const cx<T> v[5], cx<T> u[5], const KCoef
 // sincos; angles above theta_split in nsub equal sub-angles (exact: K is frozen).
 // Takes the site already in its spin gauge.  Out of line and by value so that the
 // common path keeps its registers.
+constexpr int QLGA_NSUB_MAX = 1 << 12;      // sub-angles of the general path: angles up to 2048 rad per application
+enum { FLAG_ANGLE = 1 };                    // device error word: an interaction angle was not finite or beyond the cap
+
 template <typename T>
-__device__ __noinline__ Site<T> interaction_general(Site<T> s, KCoef<T> kc, T xph, const ExpTable& tab, float theta) {
+__device__ __noinline__ Site<T> interaction_general(Site<T> s, KCoef<T> kc, T xph, const ExpTable& tab, float theta,
+                                                    int* flag) {
     int nsub = 1;
-    if (theta > tab.theta_split) nsub = (int)ceilf(theta / tab.theta_split);
+    if (theta > tab.theta_split) {
+        // a non-finite or absurd angle (bad input, a corrupted state) must not turn into a loop of 2^31
+        // sub-angles: cap it, raise the context's error word, let the next synchronising call report it
+        const float want = ceilf(theta / tab.theta_split);
+        if (!(want <= (float)QLGA_NSUB_MAX)) {
+            if (flag) atomicOr(flag, FLAG_ANGLE);
+            nsub = QLGA_NSUB_MAX;
+        } else {
+            nsub = (int)want;
+        }
+    }
+    if (!(fabs(xph) < (T)1e30)) {
+        if (flag) atomicOr(flag, FLAG_ANGLE);
+        xph = (T)0;
+    }
     const T inv_nsub = (T)1 / (T)nsub;
     kc.g2 *= inv_nsub; kc.az *= inv_nsub; kc.az2 *= inv_nsub;
     scale_by(kc.a1, inv_nsub); scale_by(kc.a6, inv_nsub);
-    const int p = 1 + count_below(tab.thr, theta / (float)nsub * 1.0009765625f);
+    const int p = min(QLGA_PMAX, 1 + count_below(tab.thr, theta / (float)nsub * 1.0009765625f));
     T sn, cs;
     sincos_lib(xph, &sn, &cs);
     T b0n = (T)1;
@@ -460,8 +498,17 @@ __device__ __noinline__ Site<T> interaction_general(Site<T> s, KCoef<T> kc, T xp
 // Apply U^{(s)} to one site.  The site may carry a power-of-two scale 2^e; the
 // caller passes constants multiplied by 4^-e, which makes the result identical
 // (bit for bit, barring under/overflow) to applying U to the unscaled site.
+//
+// Scalar phase factor ph = b0 exp(-i x), x = s (c0 rho + mu), three formulations (tab.phase_mode):
+//   0  ph = (b0 cos x, -b0 sin x), result ph * u.  cos x is rounded onto 1: a modulus error of up to half an
+//      ulp that repeats at every application while the density is stationary -- in fp32 3e-8 x 8e4
+//      applications = 2e-3 after 20 000 steps (measured: DESIGN.md section 8).
+//   1  ph = 1 + d,  d = (b0 (cos x - 1) + (b0 - 1), -b0 sin x) with cos x - 1 and b0 - 1 kept to their own
+//      relative precision; result u + d u by FMA: only the unbiased rounding of the result remains.
+//   2  as 1 with rho, x and d evaluated in fp64 from the fp32 amplitudes (fp32 kernels only).
+// fp64 in the spin gauge keeps formulation 0 (its phase factors are the five gauge rotations times ph).
 template <typename T>
-__device__ __forceinline__ void interaction(Site<T>& s, const UConst<T>& uc, const ExpTable& tab) {
+__device__ __forceinline__ void interaction(Site<T>& s, const UConst<T>& uc, const ExpTable& tab, int* flag) {
     KCoef<T> kc;
     site_coefficients<T>(s, uc, kc);               // s is in its spin gauge from here on
     // The first Horner stage of component 1 needs neither the degree nor the phase: it is
@@ -476,15 +523,36 @@ __device__ __forceinline__ void interaction(Site<T>& s, const UConst<T>& uc, con
     const T xph = fma(uc.g0, kc.rho, uc.smu);      // scalar phase exp(-i s (c0 rho + mu))
     const bool big_phase = !__all_sync(0xffffffffu, fabs(xph) <= (T)0.0625);
     if (big_phase || theta > tab.theta_split) {
-        s = interaction_general<T>(s, kc, xph, tab, theta);
+        s = interaction_general<T>(s, kc, xph, tab, theta, flag);
         return;
     }
-    T sn, cs;
-    sincos_small<T>(xph, tab.sc, &sn, &cs);
     const int p = lut_degree(tab, theta);
     const T pb0 = exp_b0(tab, p, (T)0);                // constant term of the polynomial (1 - O(tol))
+    const bool one_plus_d = !SpinGauge<T>::on && tab.phase_mode != 0;
     cx<T> phj[5];
-    gauge_phases<T>(kc, mk<T>(pb0 * cs, -(pb0 * sn)), phj);
+    cx<T> d = mk<T>((T)0, (T)0);
+    if (one_plus_d) {
+        if (sizeof(T) == 4 && tab.phase_mode == 2) {
+            double rho64 = 0.0;
+#pragma unroll
+            for (int j = 0; j < 5; ++j) {
+                const double pr = (double)kc.psi[j].re, pi = (double)kc.psi[j].im;
+                rho64 = fma(pr, pr, fma(pi, pi, rho64));
+            }
+            double sn64, cm64;
+            sincos_small_m1<double>(fma((double)uc.g0, rho64, (double)uc.smu), tab.sc, &sn64, &cm64);
+            const double b064 = tab.b0[p - 1];
+            d = mk<T>((T)fma(b064, cm64, tab.b0m1[p - 1]), (T)(-(b064 * sn64)));
+        } else {
+            T sn, cm1;
+            sincos_small_m1<T>(xph, tab.sc, &sn, &cm1);
+            d = mk<T>(fma(pb0, cm1, exp_b0m1(tab, p, (T)0)), -(pb0 * sn));
+        }
+    } else {
+        T sn, cs;
+        sincos_small<T>(xph, tab.sc, &sn, &cs);
+        gauge_phases<T>(kc, mk<T>(pb0 * cs, -(pb0 * sn)), phj);
+    }
     const T* r = exp_ratios(tab, p, (T)0);
     {
         cx<T> u[5];
@@ -498,16 +566,26 @@ __device__ __forceinline__ void interaction(Site<T>& s, const UConst<T>& uc, con
 #pragma unroll
             for (int j = 0; j < 5; ++j) u[j] = axmi(ikk, wa[j], va[j]);
         }
+        if (one_plus_d) {
 #pragma unroll
-        for (int j = 0; j < 5; ++j) s.q[j][0] = cmul(phj[j], u[j]);
+            for (int j = 0; j < 5; ++j) s.q[j][0] = cfma(d, u[j], u[j]);
+        } else {
+#pragma unroll
+            for (int j = 0; j < 5; ++j) s.q[j][0] = cmul(phj[j], u[j]);
+        }
     }
     {
         cx<T> v[5], u[5];
 #pragma unroll
         for (int j = 0; j < 5; ++j) v[j] = s.q[j][1];
         horner<T>(v, u, kc, r, p);
+        if (one_plus_d) {
 #pragma unroll
-        for (int j = 0; j < 5; ++j) s.q[j][1] = cmul(phj[j], u[j]);
+            for (int j = 0; j < 5; ++j) s.q[j][1] = cfma(d, u[j], u[j]);
+        } else {
+#pragma unroll
+            for (int j = 0; j < 5; ++j) s.q[j][1] = cmul(phj[j], u[j]);
+        }
     }
 }
 

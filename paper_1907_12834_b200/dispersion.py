@@ -17,32 +17,11 @@ import numpy as np
 from . import inputs
 
 
-def kicked_soliton(kind, row, couplings, L, k, n_kick):
-    """psi[5][1][L]: Table I coefficients of `row` (E = -2 bright / +2 dark) times the
-    soliton profile of inverse width k times exp(i 2 pi n x / L)."""
-    x = np.arange(L, dtype=np.float64)
-    if kind == "bright":
-        prof = k * inputs.sech(k * (x - L / 2))
-        cm = inputs.table1_state(row, -2.0, couplings)
-    elif kind == "dark":
-        prof = k * np.tanh(k * (x - L / 4)) * np.tanh(k * (3 * L / 4 - x))
-        cm = inputs.table1_state(row, 2.0, couplings)
-    else:
-        raise ValueError(kind)
-    psi = np.zeros((5, 1, L), dtype=np.complex128)
-    psi[:, 0, :] = cm[:, None] * prof * np.exp(2j * np.pi * n_kick * x / L)
-    return psi
-
-
-def predicted_energy(kind, k, p):
-    return p * p - k * k if kind == "bright" else p * p + 2.0 * k * k
-
-
 def measured_energy(kind, row, couplings, L, k, n_kick, steps=50, order="interleaved", precision="f64"):
     """Re E of eq. (85) after `steps` time steps on the CUDA path."""
     from . import qlga
     sim = qlga.Qlga(1, (L, 1), couplings, order=order, precision=precision)
-    sim.set_state_psi(kicked_soliton(kind, row, couplings, L, k, n_kick))
+    sim.set_state_psi(inputs.kicked_soliton(kind, row, couplings, L, k, n_kick))
     sim.step(steps)
     ob = sim.observables()
     sim.close()
@@ -54,7 +33,7 @@ def dispersion_table(kind, row, couplings, L=2048, k=1.0 / 16, kicks=(0, 2, 4, 8
     rows = []
     for n in kicks:
         p = 2.0 * np.pi * n / L
-        rows.append((p, measured_energy(kind, row, couplings, L, k, n, **kw), predicted_energy(kind, k, p)))
+        rows.append((p, measured_energy(kind, row, couplings, L, k, n, **kw), inputs.predicted_energy(kind, k, p)))
     return rows
 
 

@@ -282,3 +282,29 @@ def table1_state(row, E, couplings, free=(0.3, 0.2)):
     else:
         raise ValueError("Table I row must be 1..16")
     return np.array(c, dtype=np.float64)
+
+
+# --------------------------------------------------------------------------
+# kicked solitons of the dispersion experiment (Fig. 5) and the paper's prediction
+# --------------------------------------------------------------------------
+def kicked_soliton(kind, row, couplings, L, k, n_kick):
+    """psi[5][1][L]: Table I coefficients of `row` (E = -2 bright / +2 dark) times the
+    soliton profile of inverse width k times exp(i 2 pi n x / L)."""
+    x = np.arange(L, dtype=np.float64)
+    if kind == "bright":
+        prof = k * sech(k * (x - L / 2))
+        cm = table1_state(row, -2.0, couplings)
+    elif kind == "dark":
+        prof = k * np.tanh(k * (x - L / 4)) * np.tanh(k * (3 * L / 4 - x))
+        cm = table1_state(row, 2.0, couplings)
+    else:
+        raise ValueError(kind)
+    psi = np.zeros((5, 1, L), dtype=np.complex128)
+    psi[:, 0, :] = cm[:, None] * prof * np.exp(2j * np.pi * n_kick * x / L)
+    return psi
+
+
+def predicted_energy(kind, k, p):
+    """The paper's dispersion relations: E = p^2 - k^2 (bright, eq. 74), E = p^2 + 2 k^2
+    (dark, PAPER.md:630)."""
+    return p * p - k * k if kind == "bright" else p * p + 2.0 * k * k

@@ -16,9 +16,12 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 _LIB_PATH = os.path.join(_HERE, "libqlga.so")
 
 QLGA_OK, QLGA_EINVAL, QLGA_ENOMEM, QLGA_ECUDA, QLGA_ESTATE, QLGA_EUNSUP = range(6)
-QLGA_F64, QLGA_F32 = 0, 1
+QLGA_F64, QLGA_F32, QLGA_F32X = 0, 1, 2
 QLGA_PLAIN, QLGA_INTERLEAVED = 0, 1
-OPT_PATH, OPT_STEPS_PER_LAUNCH, OPT_EXP_TOL_LOG2, OPT_THREADS_X, OPT_TILE_Y, OPT_THREADS_Y, OPT_FUSE_PLAIN_U = range(7)
+(OPT_PATH, OPT_STEPS_PER_LAUNCH, OPT_EXP_TOL_LOG2, OPT_THREADS_X, OPT_TILE_Y, OPT_THREADS_Y, OPT_FUSE_PLAIN_U,
+ OPT_F32_PHASE, OPT_EXP_POLY) = range(9)
+_PRECISIONS = {"f64": QLGA_F64, "fp64": QLGA_F64, "double": QLGA_F64, "f32": QLGA_F32, "fp32": QLGA_F32,
+               "float": QLGA_F32, "f32x": QLGA_F32X}
 
 ABI_SYMBOLS = (
     "qlga_init", "qlga_state_bytes", "qlga_set_option", "qlga_set_state_psi", "qlga_set_state_q",
@@ -28,6 +31,7 @@ ABI_SYMBOLS = (
     "qlga_density", "qlga_density_l2_error", "qlga_vortices",
     "qlga_slab_configure", "qlga_slab_edge_get", "qlga_slab_ghost_set",
     "qlga_observable_sums", "qlga_observables_from_sums", "qlga_exp_degree", "qlga_set_chemical_potential",
+    "qlga_angle_stats",
 )
 NSUMS = 17
 
@@ -38,6 +42,11 @@ class QlgaObs(ctypes.Structure):
                 ("A00_abs2", ctypes.c_double), ("e_kin", ctypes.c_double), ("e_c0", ctypes.c_double),
                 ("e_c1", ctypes.c_double), ("e_c2", ctypes.c_double), ("e_total", ctypes.c_double),
                 ("e_dt_re", ctypes.c_double), ("e_dt_im", ctypes.c_double), ("step", ctypes.c_int64)]
+
+
+class QlgaAngles(ctypes.Structure):
+    _fields_ = [("theta_max", ctypes.c_double), ("theta_mean", ctypes.c_double), ("phase_max", ctypes.c_double),
+                ("degree_hist", ctypes.c_int64 * 13)]
 
 
 class QlgaProfile(ctypes.Structure):
@@ -103,6 +112,8 @@ def load_library():
     lib.qlga_exp_polynomial.restype = I
     lib.qlga_exp_degree.argtypes = [I, D, ctypes.POINTER(I)]
     lib.qlga_exp_degree.restype = I
+    lib.qlga_angle_stats.argtypes = [P, ctypes.POINTER(QlgaAngles)]
+    lib.qlga_angle_stats.restype = I
     lib.qlga_version.argtypes = []
     lib.qlga_version.restype = ctypes.c_char_p
     return lib
@@ -150,7 +161,7 @@ class Qlga:
     """One lattice on one GPU.  dims = (Nx, Ny) (Ny = 1 in 1D) or (Nx, Ny, Nz) in 3D; arrays
     are q[5][2][Ny][Nx] / psi[5][Ny][Nx] (3D: [..][Nz][Ny][Nx]); couplings = (c0, c1, c2)
     = the paper's (g0, g1, g2); order "plain" (eq. 108) or "interleaved" (eq. 112);
-    precision "f64" or "f32".  `keep_previous=True` allocates the third buffer that
+    precision "f64", "f32" or "f32x" (fp32 storage, fp64 arithmetic in registers).  `keep_previous=True` allocates the third buffer that
     eq. (85)'s energy needs in 2D."""
 
     def __init__(self, ndim, dims, couplings, order="interleaved", precision="f64",
@@ -162,7 +173,7 @@ class Qlga:
         self.ndim = int(ndim)
         self.nx, self.ny, self.nz = _dims3(ndim, dims)
         self.lat = (self.ny, self.nx) if self.ndim < 3 else (self.nz, self.ny, self.nx)
-        self.prec = QLGA_F64 if precision in ("f64", "fp64", "double") else QLGA_F32
+        self.prec = _PRECISIONS[precision]
         self.order = QLGA_INTERLEAVED if order in ("interleaved", 1) else QLGA_PLAIN
         self.device = torch.device(device)
         self.rdtype = torch.float64 if self.prec == QLGA_F64 else torch.float32
@@ -294,6 +305,14 @@ class Qlga:
         p, dev = self._ptr(out)
         self._check(_lib.qlga_vorticity(self.ctx, p, dev))
         return out
+
+    def angle_stats(self):
+        """{'theta_max', 'theta_mean', 'phase_max', 'degree_hist'} of one application of U on the current
+        state (qlga_angle_stats): which polynomial degrees the state exercises."""
+        a = QlgaAngles()
+        self._check(_lib.qlga_angle_stats(self.ctx, ctypes.byref(a)))
+        return {"theta_max": a.theta_max, "theta_mean": a.theta_mean, "phase_max": a.phase_max,
+                "degree_hist": [int(v) for v in a.degree_hist]}
 
     def density(self, out=None):
         if out is None:

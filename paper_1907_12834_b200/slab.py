@@ -149,10 +149,13 @@ class SlabQlga:
         self.sim.slab_ghost_set(1, self.ghost_hi if ghost_hi is None else ghost_hi)
 
     def exchange(self):
-        self.pack_edges()
-        exchange_halos(self.edge_lo, self.edge_hi, self.ghost_lo, self.ghost_hi, self.rank, self.world,
-                       self.group)
-        self.unpack_ghosts()
+        # the library packs and unpacks on the context's stream; the P2P operations must be issued on that
+        # same stream, else NCCL's send / recv is not ordered against qlga_slab_edge_get / qlga_slab_ghost_set
+        with self.torch.cuda.stream(self.sim.stream):
+            self.pack_edges()
+            exchange_halos(self.edge_lo, self.edge_hi, self.ghost_lo, self.ghost_hi, self.rank, self.world,
+                           self.group)
+            self.unpack_ghosts()
 
     def step(self, n=1):
         for _ in range(int(n)):

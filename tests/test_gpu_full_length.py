@@ -1,0 +1,267 @@
+"""Configs 2-5 of BASELINE.json at their stated step counts on the CUDA path (-m gpu):
+
+  (i)   invariants along the full run: norm_q (every factor is unitary on the 10-vector), and in 2D
+        sum(omega) = 0 and zero total winding;
+  (ii)  LATE-TIME windowed parity with the oracle (SURVEY.md 8(c) "parity procedure" (ii)): the device
+        state is copied at t0 = steps - n, the library steps n more, and for every window the oracle
+        runs n steps on the (P + 8n)-site patch of the t0 state (the domain of dependence of a site is
+        exactly 4 sites per step per direction) -- windows on a vortex core found at t0, on the collision
+        region, on a wrap corner and in the bulk;
+  (iii) the interaction angles / polynomial degrees the evolved state exercises (qlga_angle_stats),
+        recorded next to those of the initial condition;
+  (iv)  fp32 and fp32-storage runs of the same length against the fp64 run from the same fp32-rounded
+        input (the fp64 path being tied to the oracle by (ii)): the measured error growth, asserted as
+        a horizon.
+
+Bar (BASELINE.json north_star): 1e-12 (fp64) / 1e-5 (fp32) relative L2 over all 10 planes.
+Set QLGA_TEST_REPORT=<file> to append one JSON record per run (used to fill DESIGN.md's tables)."""
+import json
+import os
+
+import numpy as np
+import pytest
+
+from paper_1907_12834_b200 import inputs
+from conftest import rel_l2
+
+pytestmark = pytest.mark.gpu
+
+TOL64 = 1e-12
+TOL32 = 1e-5
+ORDERS = {"plain": 0, "interleaved": 1}
+
+
+@pytest.fixture(scope="module")
+def qlga():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    from paper_1907_12834_b200 import qlga as mod      # fails loudly if libqlga.so is missing
+    return mod
+
+
+def _report(rec):
+    path = os.environ.get("QLGA_TEST_REPORT")
+    if path:
+        with open(path, "a") as f:
+            f.write(json.dumps(rec) + "\n")
+
+
+def _cdt(torch, precision):
+    return torch.complex128 if precision == "f64" else torch.complex64
+
+
+def _dev_rel_l2(torch, a, b):
+    """relative L2 distance of two device states, accumulated in fp64"""
+    a = a.to(torch.complex128); b = b.to(torch.complex128)
+    return float(torch.sqrt(torch.sum(torch.abs(a - b) ** 2) / torch.sum(torch.abs(b) ** 2)))
+
+
+def _top_degree(hist):
+    return max(p for p, cnt in enumerate(hist) if cnt > 0)
+
+
+def run_full_length(qlga, oracle, w, precision, order, steps, n_tail, windows, P, tol, norm_tol, tag,
+                    vortex_window=False, q_dev=None, keep_final=False):
+    """Steps `w` to `steps`, checks the invariants and the late-time windows; returns the record (and the
+    final device state with keep_final)."""
+    import torch
+    ndim = w.ndim
+    nx, ny = w.dims[0], w.dims[1]
+    cdt = _cdt(torch, precision)
+    if q_dev is None:
+        psi = torch.from_numpy(w.psi).to(cdt).cuda()
+        q_dev = (psi[:, None] / 2).expand(5, 2, ny, nx).contiguous()
+        del psi
+    sim = qlga.Qlga(ndim, w.dims, w.couplings, order=order, precision=precision)
+    sim.set_state_q(q_dev)
+    obs0 = sim.observables()
+    ang0 = sim.angle_stats()
+    t0 = steps - n_tail
+    sim.step(t0)
+    snap = torch.empty((5, 2, ny, nx), dtype=cdt, device="cuda")
+    sim.get_state_q(snap)
+    ang1 = sim.angle_stats()
+    windows = list(windows)
+    nvort = None
+    if ndim == 2:
+        rec, nvort = sim.vortices(max_out=1 << 16)
+        if vortex_window:
+            assert nvort > 0, "no vortex left at t0"
+            # a window whose centre sits on the core nearest to the lattice centre (the collision region)
+            k = np.argmin((rec[:, 1] - nx // 2) ** 2 + (rec[:, 2] - ny // 2) ** 2)
+            windows.append((int(rec[k, 1]) - P // 2, int(rec[k, 2]) - P // 2))
+    sim.step(n_tail)
+    out = torch.empty_like(snap)
+    sim.get_state_q(out)
+    obs = sim.observables()
+    assert obs["step"] == steps
+    drift = obs["norm_q"] / obs0["norm_q"] - 1.0
+    record = {"tag": tag, "precision": precision, "order": order, "steps": steps, "norm_q_drift": drift,
+              "theta_max_t0": ang0["theta_max"], "theta_max_late": ang1["theta_max"],
+              "phase_max_t0": ang0["phase_max"], "phase_max_late": ang1["phase_max"],
+              "degree_hist_t0": ang0["degree_hist"], "degree_hist_late": ang1["degree_hist"], "vortices_at_t0": nvort}
+    if ndim == 2:
+        om = torch.empty((5, ny, nx), dtype=torch.float64 if precision == "f64" else torch.float32, device="cuda")
+        sim.vorticity(om)
+        record["sum_omega"] = float(om.to(torch.float64).sum())
+        recs, cnt = sim.vortices(max_out=1 << 20)
+        record["vortices_end"] = int(cnt)
+        record["total_winding"] = int(recs[:, 3].sum()) if cnt <= 1 << 20 else None
+        del om
+    h = 4 * n_tail
+    worst = 0.0
+    per_window = []
+    for (cx, cy) in windows:
+        xs = (np.arange(cx - h, cx + P + h)) % nx
+        ys = (np.arange(cy - h, cy + P + h)) % ny if ndim == 2 else np.array([0])
+        xi = torch.as_tensor(xs, device="cuda"); yi = torch.as_tensor(ys, device="cuda")
+        patch_in = snap[:, :, yi][:, :, :, xi].cpu().numpy().astype(np.complex128)
+        patch_out = out[:, :, yi][:, :, :, xi].cpu().numpy().astype(np.complex128)
+        ref = oracle.step(patch_in, ndim, w.couplings, ORDERS[order], n_tail)   # periodic patch: only the centre is valid
+        if ndim == 2:
+            a, b = patch_out[:, :, h:h + P, h:h + P], ref[:, :, h:h + P, h:h + P]
+        else:
+            a, b = patch_out[:, :, :, h:h + P], ref[:, :, :, h:h + P]
+        e = rel_l2(a, b)
+        per_window.append(((int(cx) % nx, int(cy) % ny), e))
+        worst = max(worst, e)
+    record["windows"] = per_window
+    record["worst_window"] = worst
+    _report(record)
+    sim.close()
+    del snap
+    assert worst < tol, (tag, per_window)
+    assert abs(drift) < norm_tol, (tag, drift)
+    if ndim == 2:
+        assert abs(record["sum_omega"]) < 1e-3, record["sum_omega"]      # every omega is a multiple of pi/2
+        assert record["total_winding"] in (0, None)
+    if keep_final:
+        return record, out
+    del out
+    return record
+
+
+# ---------------------------------------------------------------------------
+# config 2: 1D 65536, 50 000 steps (temporal blocking: four steps per launch)
+# ---------------------------------------------------------------------------
+def test_config2_full_length(qlga, oracle):
+    w = inputs.config2()
+    L = w.dims[0]
+    # solitons drift by 2 p t = 0.1 site/step: at t = 50 000 their centres are at L/4 + 5000 and 3L/4 - 5000
+    windows = [(0, 0), (L // 4 + 5000 - 60, 0), (3 * L // 4 - 5000 - 60, 0), (L - 60, 0)]
+    rec = run_full_length(qlga, oracle, w, "f64", "interleaved", w.steps, 8, windows, 120, TOL64,
+                          1e-13 * w.steps / 1000, "cfg2")
+    # the window on the soliton really holds it (it moved there): its field is far above the empty lattice's
+    assert rec["theta_max_late"] > 0.5 * rec["theta_max_t0"]
+
+
+# ---------------------------------------------------------------------------
+# config 3: 1D 2^22, 20 000 steps, fp64 + fp32 (+ fp32 storage / fp64 arithmetic)
+# ---------------------------------------------------------------------------
+def test_config3_full_length_fp64(qlga, oracle):
+    w = inputs.config3()
+    L = w.dims[0]
+    windows = [(0, 0), (L // 4 - 50, 0), (3 * L // 4 - 50, 0), (L - 30, 0), (1234567, 0)]
+    run_full_length(qlga, oracle, w, "f64", "interleaved", w.steps, 6, windows, 100, TOL64,
+                    1e-13 * w.steps / 1000, "cfg3")
+
+
+def test_config3_full_length_fp32_variants(qlga, oracle):
+    """fp32 at config 3's 20 000 steps: late-time windowed parity against the oracle (local: 1e-5) and
+    the global distance from the fp64 run started from the same fp32-rounded input."""
+    import torch
+    w = inputs.config3()
+    L = w.dims[0]
+    windows = [(0, 0), (L // 4 - 50, 0), (L - 30, 0)]
+    psi32 = torch.from_numpy(w.psi).to(torch.complex64).cuda()
+    q32 = (psi32[:, None] / 2).expand(5, 2, 1, L).contiguous()
+    del psi32
+    _, ref = run_full_length(qlga, oracle, w, "f64", "interleaved", w.steps, 6, windows[:1], 100, TOL64,
+                             1e-13 * w.steps / 1000, "cfg3_from_fp32_input", q_dev=q32.to(torch.complex128),
+                             keep_final=True)
+    errs = {}
+    for precision, norm_tol in (("f32x", 2e-6), ("f32", 2e-4)):
+        rec, out = run_full_length(qlga, oracle, w, precision, "interleaved", w.steps, 6, windows, 100, TOL32,
+                                   norm_tol, "cfg3_" + precision, q_dev=q32, keep_final=True)
+        errs[precision] = _dev_rel_l2(torch, out, ref)
+        _report({"tag": "cfg3_global_" + precision, "steps": w.steps, "rel_l2_vs_fp64": errs[precision],
+                 "norm_q_drift": rec["norm_q_drift"]})
+        del out
+    # fp32 storage with fp64 arithmetic meets the north star's 1e-5 at the stated step count
+    assert errs["f32x"] < TOL32, errs
+    # fp32 arithmetic: measured horizon
+    assert errs["f32"] < FP32_CFG3_20000, errs
+
+
+FP32_CFG3_20000 = 5e-3          # measured bound for QLGA_F32 at config 3's 20 000 steps
+FP32_CFG5_5000 = 5e-3           # the same at config 5's recipe, 2048^2, 5000 steps
+
+
+# ---------------------------------------------------------------------------
+# config 4: 2D 2048^2, 10 000 steps
+# ---------------------------------------------------------------------------
+def test_config4_full_length(qlga, oracle):
+    w = inputs.config4()
+    L = w.dims[0]
+    windows = [(0, 0), (L - 20, L // 2), (L // 2 - 12, L // 2 - 12), (777, 1500)]
+    run_full_length(qlga, oracle, w, "f64", "interleaved", w.steps, 4, windows, 24, TOL64,
+                    1e-13 * w.steps / 1000, "cfg4", vortex_window=True)
+
+
+# ---------------------------------------------------------------------------
+# config 5: 2D 8192^2, 5000 steps through the collision, fp64 + fp32
+# ---------------------------------------------------------------------------
+def _cfg5_windows(L):
+    # wrap corner, the collision region (the dipoles meet at the lattice centre near step 4300), bulk
+    return [(0, 0), (L - 20, L - 20), (L // 2 - 12, L // 2 - 12), (L // 2 + 36, L // 2 - 12), (1234, 4321 % L)]
+
+
+def test_config5_full_length_fp64(qlga, oracle):
+    w = inputs.config5()
+    rec = run_full_length(qlga, oracle, w, "f64", "interleaved", w.steps, 3, _cfg5_windows(w.dims[0]), 24, TOL64,
+                          1e-13 * w.steps / 1000, "cfg5", vortex_window=True)
+    assert rec["vortices_at_t0"] is not None
+
+
+def test_config5_full_length_fp32(qlga, oracle):
+    w = inputs.config5()
+    run_full_length(qlga, oracle, w, "f32", "interleaved", w.steps, 3, _cfg5_windows(w.dims[0]), 24, TOL32,
+                    2e-4, "cfg5_f32", vortex_window=True)
+
+
+def test_config5_recipe_fp32_variants_reduced_lattice(qlga, oracle):
+    """config 5's recipe on 2048^2 (same cores, kick and noise) for the full 5000 steps: fp32 and fp32-storage
+    runs against the fp64 run from the same fp32-rounded input."""
+    import torch
+    w = inputs.config5(L=2048)
+    L = 2048
+    psi32 = torch.from_numpy(w.psi).to(torch.complex64).cuda()
+    q32 = (psi32[:, None] / 2).expand(5, 2, L, L).contiguous()
+    del psi32
+    windows = _cfg5_windows(L)[:3]
+    _, ref = run_full_length(qlga, oracle, w, "f64", "interleaved", 5000, 3, windows[:1], 24, TOL64, 5e-13,
+                             "cfg5_2048_from_fp32_input", q_dev=q32.to(torch.complex128), keep_final=True)
+    errs = {}
+    for precision, norm_tol in (("f32x", 2e-6), ("f32", 2e-4)):
+        rec, out = run_full_length(qlga, oracle, w, precision, "interleaved", 5000, 3, windows, 24, TOL32,
+                                   norm_tol, "cfg5_2048_" + precision, q_dev=q32, keep_final=True)
+        errs[precision] = _dev_rel_l2(torch, out, ref)
+        _report({"tag": "cfg5_2048_global_" + precision, "steps": 5000, "rel_l2_vs_fp64": errs[precision],
+                 "norm_q_drift": rec["norm_q_drift"]})
+        del out
+    assert errs["f32x"] < TOL32, errs
+    assert errs["f32"] < FP32_CFG5_5000, errs
+
+
+# ---------------------------------------------------------------------------
+# plain ordering (eq. 108) at length: unitary whatever the stability of the flow; late-time windows
+# ---------------------------------------------------------------------------
+def test_plain_ordering_full_length(qlga, oracle):
+    w = inputs.config4()
+    L = w.dims[0]
+    run_full_length(qlga, oracle, w, "f64", "plain", 2000, 4, [(0, 0), (L // 4 - 12, L // 4 - 12), (L - 20, L // 2)], 24,
+                    TOL64, 2e-13, "cfg4_plain", vortex_window=False)
+    w = inputs.config3()
+    L = w.dims[0]
+    run_full_length(qlga, oracle, w, "f64", "plain", 5000, 6, [(0, 0), (L // 4 - 50, 0), (L - 30, 0)], 100, TOL64,
+                    5e-13, "cfg3_plain")

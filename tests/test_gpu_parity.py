@@ -495,8 +495,8 @@ def test_dispersion_relation_of_kicked_solitons_fig5(qlga, oracle):
             p = 2 * np.pi * n / L
             e = dispersion.measured_energy(kind, row, c, L, k, n, steps=21)
             es.append(e)
-            assert abs(e - dispersion.predicted_energy(kind, k, p)) < 0.02 * (p * p + k * k), (kind, n)
-            q0 = oracle.split_psi(dispersion.kicked_soliton(kind, row, c, L, k, n))
+            assert abs(e - inputs.predicted_energy(kind, k, p)) < 0.02 * (p * p + k * k), (kind, n)
+            q0 = oracle.split_psi(inputs.kicked_soliton(kind, row, c, L, k, n))
             qa = oracle.step(q0, 1, c, 1, 20)
             qb = oracle.step(qa, 1, c, 1, 1)
             assert e == pytest.approx(oracle.observables(qb, 1, c, qprev=qa)["e_dt_re"], rel=1e-9, abs=1e-14)
@@ -558,7 +558,7 @@ def test_chemical_potential(qlga, oracle):
     cb, L, k, n = (-1.0, -0.5, 0.2), 1024, 1.0 / 16, 4
     sim = qlga.Qlga(1, (L, 1), cb)
     sim.set_chemical_potential(0.011)
-    sim.set_state_psi(dispersion.kicked_soliton("bright", 3, cb, L, k, n))
+    sim.set_state_psi(inputs.kicked_soliton("bright", 3, cb, L, k, n))
     sim.step(21)
     p = 2 * np.pi * n / L
     assert abs(sim.observables()["e_dt_re"] - (0.011 + p * p - k * k)) < 0.02 * (p * p + k * k)

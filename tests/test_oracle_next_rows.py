@@ -101,15 +101,14 @@ def test_chemical_potential_is_a_global_phase_and_zero_is_the_plain_form(oracle)
 def test_dispersion_with_chemical_potential_eq75(oracle):
     # eq. (75): E = mu + p^2 - k^2 (bright): E = mu + p^2 + 2 k^2 (dark), by eq. (85)
     import numpy as np
-    from paper_1907_12834_b200 import dispersion
     L, k, n, mu = 512, 1.0 / 16, 4, 0.011
     p = 2 * np.pi * n / L
     for kind, row, c in (("bright", 3, (-1.0, -0.5, 0.2)), ("dark", 5, (1.0, 0.3, -0.1))):
-        q0 = oracle.split_psi(dispersion.kicked_soliton(kind, row, c, L, k, n))
+        q0 = oracle.split_psi(inputs.kicked_soliton(kind, row, c, L, k, n))
         qa = oracle.step(q0, 1, c, 1, 10, mu=mu)
         qb = oracle.step(qa, 1, c, 1, 1, mu=mu)
         e = oracle.observables(qb, 1, c, qprev=qa)["e_dt_re"]
-        want = mu + dispersion.predicted_energy(kind, k, p)
+        want = mu + inputs.predicted_energy(kind, k, p)
         assert abs(e - want) < 0.02 * (p * p + k * k), (kind, e, want)
         e0 = oracle.observables(oracle.step(qa, 1, c, 1, 1), 1, c, qprev=qa)["e_dt_re"]
         assert abs((e - e0) - mu) < 1e-3 * mu          # the shift is mu (sin mu at this size)
