@@ -50,7 +50,7 @@ def parse_args():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="cfg5", choices=sorted(WORKLOADS))
-    ap.add_argument("--precision", default="f64", choices=["f64", "f32"])
+    ap.add_argument("--precision", default="f64", choices=["f64", "f32", "f32x"])
     ap.add_argument("--order", default="interleaved", choices=["interleaved", "plain"])
     ap.add_argument("--inner", type=int, default=0, help="time steps per bench step (0 = auto)")
     ap.add_argument("--lattice", type=int, default=0, help="override the lattice edge (testing)")
@@ -151,7 +151,7 @@ class ClockSampler:
 # ---------------------------------------------------------------------------
 def bytes_per_site_update(precision):
     """One read + one write of the 20 reals of a site: SURVEY.md section 8(d)."""
-    return 320.0 if precision == "f64" else 160.0
+    return 320.0 if precision == "f64" else 160.0          # f32 and f32x store fp32
 
 
 def fp_instr_per_site_update(ndim, order, degree, precision="f64"):
@@ -167,28 +167,30 @@ def fp_instr_per_site_update(ndim, order, degree, precision="f64"):
     return n_u * per_u + n_fac * 40.0 + 20.0 * ndim
 
 
-def expected_degree(w, ndim, order, precision):
-    """Degree the kernel's order selection picks on the workload's initial state (same
-    rule as interaction(): theta = s (2|c1||F| + |c2| rho / 5) against the library's
-    thresholds, qlga_exp_polynomial)."""
-    psi = w.psi.reshape(5, -1)
-    idx = np.linspace(0, psi.shape[1] - 1, 4096).astype(np.int64)
-    p5 = psi[:, idx]
-    n = np.abs(p5) ** 2
-    rho = n.sum(0)
-    fz = 2 * (n[0] - n[4]) + n[1] - n[3]
-    fp = (2 * (np.conj(p5[0]) * p5[1] + np.conj(p5[3]) * p5[4])
-          + np.sqrt(6.0) * (np.conj(p5[1]) * p5[2] + np.conj(p5[2]) * p5[3]))
-    fabs = np.sqrt(fz ** 2 + np.abs(fp) ** 2)
-    s = 1.0 / (4 * ndim) if order == "interleaved" else 1.0
-    c0, c1, c2 = w.couplings
-    theta = s * (2 * abs(c1) * fabs + abs(c2) / 5 * rho)
-    from paper_1907_12834_b200 import qlga
-    tol_log2 = -56 if precision == "f64" else -27
-    deg = np.ones_like(theta)
-    for p in range(1, 12):
-        deg += theta * 1.001 > qlga.exp_polynomial(tol_log2, p)[0]
-    return float(np.mean(deg))
+def mean_degree(sim):
+    """Mean per-site polynomial degree of U on the CURRENT (evolved) state, from the library's own degree
+    lookup (qlga_angle_stats): the degree the ALU model charges."""
+    st = sim.angle_stats()
+    hist = st["degree_hist"]
+    n = sum(hist)
+    # sites beyond the split angle ([0]) take the general path: charge them the top degree
+    return (sum(p * c for p, c in enumerate(hist) if p > 0) + 12 * hist[0]) / max(n, 1), st
+
+
+_ALU_PEAKS = {}
+
+
+def alu_peak(qlga, precision):
+    """Measured issue rate of the binding FP pipe (qlga_issue_peak, live in this run): thread-instructions per
+    second and per SM cycle.  fp64 arithmetic: DFMA.  fp32: the larger of the FFMA and packed FFMA2 lane rates."""
+    kinds = ("dfma",) if precision in ("f64", "f32x") else ("ffma", "ffma2")
+    best = None
+    for k in kinds:
+        if k not in _ALU_PEAKS:
+            _ALU_PEAKS[k] = qlga.issue_peak(k)
+        if best is None or _ALU_PEAKS[k]["instr_per_s"] > best[1]["instr_per_s"]:
+            best = (k, _ALU_PEAKS[k])
+    return best
 
 
 # ---------------------------------------------------------------------------
@@ -281,6 +283,49 @@ def max_over_ranks(ms, world, device=None):
 def aggregate_gsups(sites_per_rank, time_steps, world, ms):
     """Whole-job site-updates per second (GSUP/s): every rank advances its own lattice."""
     return sites_per_rank * time_steps * world / (ms * 1e-3) / 1e9
+
+
+def build_roofline(qlga, prof, ndim, sites, time_steps, precision, order, deg_info, clocks, captured):
+    """Both rooflines of the dominant pass kernel; the binding one (larger fraction) on top.
+    HBM: algorithmic bytes per launch / launch time against the measured copy bandwidth.  ALU: FP instructions
+    per launch (model of fp_instr_per_site_update at the mean per-site degree of the evolved state) / launch time
+    against the issue rate measured live by qlga_issue_peak."""
+    hbm_peak, peak_kind, sm_max = load_peaks()
+    bps = bytes_per_site_update(precision)
+    kinds = {k: v for k, v in prof.items() if v[1] > 0}
+    if not kinds:
+        return None
+    dom = max(kinds, key=lambda k: kinds[k][0])
+    dms, dn = kinds[dom]
+    per_launch_ms = dms / dn
+    # a pass launch advances every site by 1/ndim of a time step (times the fused steps in 1D)
+    per_step = 1 if dom == "x_pass" else max(1, ndim - 1)    # the y_pass timer covers the y and z passes
+    units = sites * time_steps * per_step / (ndim * dn)       # site-updates per launch
+    deg, stats = deg_info
+    arith = "f64" if precision in ("f64", "f32x") else "f32"
+    fpi = fp_instr_per_site_update(ndim, order, deg, arith)
+    kind, pk = alu_peak(qlga, precision)
+    alu_peak_t = pk["instr_per_s"] / 1e12
+    alu_ach = units * fpi / (per_launch_ms * 1e-3) / 1e12
+    hbm_ach = units * bps / (per_launch_ms * 1e-3) / 1e9
+    traffic = captured.get(dom, (None, None))[0]
+    roof_hbm = {"bound": "hbm", "achieved": hbm_ach, "peak": hbm_peak, "unit": "GB/s",
+                "frac": hbm_ach / hbm_peak, "traffic": traffic, "peak_kind": peak_kind,
+                "kernel": dom, "ms_per_launch": per_launch_ms,
+                "model": f"{bps:.0f} B per site-update x {units:.3g} site-updates per launch"}
+    roof_alu = {"bound": "alu", "achieved": alu_ach, "peak": alu_peak_t, "unit": "Tinstr/s",
+                "frac": alu_ach / alu_peak_t, "traffic": traffic, "kernel": dom, "peak_kind": "measured",
+                "ms_per_launch": per_launch_ms,
+                "model": f"{fpi:.0f} FP instr per site-update (mean degree {deg:.2f} on the evolved state, "
+                         f"theta_max {stats['theta_max']:.3g}) x {units:.3g} site-updates per launch; peak = {kind.upper()} issue "
+                         f"microbenchmark in this run: {pk['instr_per_clk_per_sm']:.1f} instr/clk/SM, {alu_peak_t:.2f} Tinstr/s "
+                         f"(spec: 148 SMs x {64 if arith == 'f64' else 128} lanes x clock)"}
+    roof = roof_alu if roof_alu["frac"] > roof_hbm["frac"] else roof_hbm
+    if roof is roof_alu:
+        roof["hbm_model"] = roof_hbm
+    else:
+        roof["alu_model"] = roof_alu
+    return roof
 
 
 # ---------------------------------------------------------------------------
@@ -405,6 +450,7 @@ def main():
     ms = ev0.elapsed_time(ev1)
     prof = sim.profile_read()
     sim.profile_enable(False)
+    deg_info = mean_degree(sim)
     ms = max_over_ranks(ms, world, dev)
     value = aggregate_gsups(sites, inner * args.steps, world, ms)
 
@@ -461,43 +507,10 @@ def main():
         return
 
     # ---- roofline of the dominant kernel (the pass kernels) -----------------------------
-    hbm_peak, peak_kind, sm_max = load_peaks()
+    hbm_peak = load_peaks()[0]
     bps = bytes_per_site_update(args.precision)
-    kinds = {k: v for k, v in prof.items() if v[1] > 0}
-    dom = max(kinds, key=lambda k: kinds[k][0]) if kinds else None
-    pass_ms = sum(v[0] for v in kinds.values())
-    roof = None
-    roof_hbm = None
-    if dom:
-        dms, dn = kinds[dom]
-        per_launch_ms = dms / dn
-        # a pass launch advances every site by 1/ndim of a time step (times the fused steps in 1D)
-        per_step = 1 if dom == "x_pass" else max(1, ndim - 1)  # the y_pass timer covers the y and z passes
-        units = sites * inner * args.steps * per_step / (ndim * dn)      # site-updates per launch
-        deg = expected_degree(w, ndim, args.order, args.precision)
-        fpi = fp_instr_per_site_update(ndim, args.order, deg, args.precision)
-        lanes = 64 if args.precision == "f64" else 128       # FP64 / FP32 FMA lanes per SM per clock
-        clk = (clocks.get("sm_mhz") or sm_max) * 1e6
-        alu_peak = 148 * lanes * clk / 1e12                  # T instr/s at the clock seen under load
-        alu_ach = units * fpi / (per_launch_ms * 1e-3) / 1e12
-        hbm_ach = units * bps / (per_launch_ms * 1e-3) / 1e9
-        captured = load_traffic(args.workload, args.precision, args.order) if not args.lattice else {}
-        traffic = captured.get(dom, (None, None))[0]
-        roof_hbm = {"bound": "hbm", "achieved": hbm_ach, "peak": hbm_peak, "unit": "GB/s",
-                    "frac": hbm_ach / hbm_peak, "traffic": traffic, "peak_kind": peak_kind,
-                    "kernel": dom, "ms_per_launch": per_launch_ms,
-                    "model": f"{bps:.0f} B per site-update x {units:.3g} site-updates per launch"}
-        roof_alu = {"bound": "alu", "achieved": alu_ach, "peak": alu_peak, "unit": "Tinstr/s",
-                    "frac": alu_ach / alu_peak, "traffic": traffic, "kernel": dom,
-                    "ms_per_launch": per_launch_ms,
-                    "model": f"{fpi:.0f} FP instr per site-update (mean degree {deg:.2f}) x {units:.3g} site-updates per launch; "
-                             f"peak = 148 SMs x {lanes} lanes x {clk / 1e6:.0f} MHz (median clock under load)"}
-        # the binding roofline is the one with the larger fraction
-        roof = roof_alu if roof_alu["frac"] > roof_hbm["frac"] else roof_hbm
-        if roof is roof_alu:
-            roof["hbm_model"] = roof_hbm
-        else:
-            roof["alu_model"] = roof_alu
+    roof = build_roofline(qlga, prof, ndim, sites, inner * args.steps, args.precision, args.order, deg_info, clocks,
+                          load_traffic(args.workload, args.precision, args.order) if not args.lattice else {})
 
     cpu = None
     if world == 1 and not args.no_cpu_baseline:

@@ -237,6 +237,15 @@ qlga_status qlga_exp_polynomial(int tol_log2, int p, double* theta_max, double* 
  * edge of its bucket -- never below "smallest p with theta <= theta_max(p)", at most one above (host only). */
 qlga_status qlga_exp_degree(int tol_log2, double theta, int* p);
 
+/* Issue rate of the plain floating-point pipes, measured (the denominator of bench.py's "alu" roofline;
+ * SURVEY.md 8(d)): a kernel of independent chains of one instruction kind, kind = 0 DFMA (fp64), 1 FFMA (fp32),
+ * 2 FFMA2 (packed two-wide fp32), at 1024 resident threads per SM on the current device and the given stream
+ * (cuda_stream = the caller's cudaStream_t or NULL).  *instr_per_s: thread-instructions per second (one per
+ * lane; an FFMA2 counts as two) by CUDA events, best of three launches; *instr_per_clk_per_sm: the same per SM
+ * cycle by clock64() (independent of the clock the GPU held); *ms (may be NULL): duration of the best launch.
+ * Needs no context.  Synchronises the stream.  QLGA_EINVAL (kind, NULL), QLGA_ECUDA. */
+qlga_status qlga_issue_peak(int kind, void* cuda_stream, double* instr_per_s, double* instr_per_clk_per_sm, double* ms);
+
 /* Number of kernels this context has launched so far (for bench.py's gpu_launches). */
 int64_t qlga_launch_count(const qlga_ctx*);
 

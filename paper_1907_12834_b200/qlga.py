@@ -31,7 +31,7 @@ ABI_SYMBOLS = (
     "qlga_density", "qlga_density_l2_error", "qlga_vortices",
     "qlga_slab_configure", "qlga_slab_edge_get", "qlga_slab_ghost_set",
     "qlga_observable_sums", "qlga_observables_from_sums", "qlga_exp_degree", "qlga_set_chemical_potential",
-    "qlga_angle_stats",
+    "qlga_angle_stats", "qlga_issue_peak",
 )
 NSUMS = 17
 
@@ -114,6 +114,8 @@ def load_library():
     lib.qlga_exp_degree.restype = I
     lib.qlga_angle_stats.argtypes = [P, ctypes.POINTER(QlgaAngles)]
     lib.qlga_angle_stats.restype = I
+    lib.qlga_issue_peak.argtypes = [I, P, ctypes.POINTER(D), ctypes.POINTER(D), ctypes.POINTER(D)]
+    lib.qlga_issue_peak.restype = I
     lib.qlga_version.argtypes = []
     lib.qlga_version.restype = ctypes.c_char_p
     return lib
@@ -143,6 +145,18 @@ def exp_degree(tol_log2, theta):
     if st != QLGA_OK:
         raise QlgaError(st, "qlga_exp_degree: bad arguments")
     return p.value
+
+
+def issue_peak(kind, stream=None):
+    """Measured issue rate of the DFMA / FFMA / FFMA2 pipes on the current device (qlga_issue_peak):
+    {'instr_per_s', 'instr_per_clk_per_sm', 'ms'}; kind = "dfma" | "ffma" | "ffma2"."""
+    k = {"dfma": 0, "ffma": 1, "ffma2": 2}[kind]
+    a, b, c = ctypes.c_double(), ctypes.c_double(), ctypes.c_double()
+    st = _lib.qlga_issue_peak(k, ctypes.c_void_p(stream.cuda_stream) if stream is not None else None,
+                              ctypes.byref(a), ctypes.byref(b), ctypes.byref(c))
+    if st != QLGA_OK:
+        raise QlgaError(st, "qlga_issue_peak failed")
+    return {"instr_per_s": a.value, "instr_per_clk_per_sm": b.value, "ms": c.value}
 
 
 def _dims3(ndim, dims):
