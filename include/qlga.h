@@ -237,6 +237,30 @@ qlga_status qlga_exp_polynomial(int tol_log2, int p, double* theta_max, double* 
  * edge of its bucket -- never below "smallest p with theta <= theta_max(p)", at most one above (host only). */
 qlga_status qlga_exp_degree(int tol_log2, double theta, int* p);
 
+/* The lattice sums of qlga_observable_sums for callers that cannot allocate device memory (code under CUDA
+ * graph capture, tight serving loops, harnesses that forbid cudaMalloc).  Needs NO context (qlga_init allocates
+ * its scratch with cudaMalloc) and calls no cudaMalloc / cudaFree or allocating routine: the per-block partial
+ * sums live in a static device array inside the library, 19 doubles for each of at most
+ * QLGA_NOALLOC_MAX_BLOCKS = 2048 blocks plus 19 reduced sums = 311 448 bytes, held by every GPU that loads the
+ * library until the process exits.
+ *   dev_q      DEVICE  state [5][2][Nz][Ny][Nx] complex of the storage type of `prec` (layout at the top)
+ *   dev_qprev  DEVICE or NULL  the previous step's state, for the two sums of eq. (85)
+ *   ndim, dims as for qlga_init;  prec: QLGA_F64, or QLGA_F32 / QLGA_F32X (fp32 storage)
+ *   nblocks    grid of the reduction: 0 = the grid qlga_observable_sums uses (8 per SM), else 1..2048;
+ *              a value beyond QLGA_NOALLOC_MAX_BLOCKS is QLGA_EINVAL (the static scratch cannot hold it)
+ *   dev_sums   DEVICE [QLGA_NSUMS] doubles, the caller's: the sums in the order of qlga_observable_sums (whole
+ *              lattice); entries 15, 16 are 0 when dev_qprev is NULL
+ *   cuda_stream  the caller's stream; asynchronous, no synchronisation, no host output
+ * With the same grid the sums equal qlga_observable_sums' bit for bit (same kernels).  All calls share the one
+ * array (nothing in it needs clearing between calls): calls that may overlap on the GPU -- different streams
+ * without an ordering between them -- race; keep them on one stream or order them with events.
+ * Errors: QLGA_EINVAL (arguments, nblocks > 2048), QLGA_EUNSUP (device ordinal > 63), QLGA_ECUDA; the text is
+ * returned by qlga_noalloc_last_error(). */
+#define QLGA_NOALLOC_MAX_BLOCKS 2048
+qlga_status qlga_observable_sums_noalloc(const void* dev_q, const void* dev_qprev, int ndim, const int64_t* dims,
+                                         qlga_prec prec, int nblocks, double* dev_sums, void* cuda_stream);
+const char* qlga_noalloc_last_error(void);
+
 /* Issue rate of the plain floating-point pipes, measured (the denominator of bench.py's "alu" roofline;
  * SURVEY.md 8(d)): a kernel of independent chains of one instruction kind, kind = 0 DFMA (fp64), 1 FFMA (fp32),
  * 2 FFMA2 (packed two-wide fp32), at 1024 resident threads per SM on the current device and the given stream

@@ -471,3 +471,99 @@ cudaError_t launch_angle_stats(const Launch& L, qlga_prec prec, const void* q, i
 }
 
 }  // namespace qlga
+
+// ---------------------------------------------------------------------------
+// qlga_observable_sums_noalloc (include/qlga.h): the observables reduction for callers that cannot call
+// cudaMalloc (CUDA graph capture, serving loops, harnesses that forbid it).  It needs no context and
+// allocates nothing: the per-block partial sums and the 19 reduced sums live in the file-scope device
+// array below, QLGA_NOALLOC_MAX_BLOCKS x 19 + 19 doubles = 311 448 bytes that every GPU loading the
+// library holds until exit.  Same kernels as qlga_observable_sums (observables_kernel,
+// reduce_partials_kernel), same grid: bit-identical sums.
+//
+// In host code the name `g_noalloc_scratch` is a host-side stand-in, not a device address: the address is
+// taken once per device, with that device current, by cudaGetSymbolAddress, and that pointer goes to the
+// kernels.  Every call shares the array: nothing in it has to start at zero (each block overwrites all 19
+// of its partials and the second pass reads exactly the blocks just written), but two calls that overlap
+// on the GPU (different streams, no ordering between them) race on it.
+// ---------------------------------------------------------------------------
+namespace qlga {
+constexpr int NOALLOC_DOUBLES = QLGA_NOALLOC_MAX_BLOCKS * OBS_NACC + OBS_NACC;
+static __device__ __align__(256) double g_noalloc_scratch[NOALLOC_DOUBLES];
+}  // namespace qlga
+
+#include <atomic>
+#include <stdio.h>
+
+static char g_noalloc_err[256] = "";
+extern "C" const char* qlga_noalloc_last_error(void) { return g_noalloc_err; }
+
+static qlga_status noalloc_fail(qlga_status st, const char* text, cudaError_t e = cudaSuccess) {
+    if (e != cudaSuccess) snprintf(g_noalloc_err, sizeof(g_noalloc_err), "%s: %s", text, cudaGetErrorString(e));
+    else snprintf(g_noalloc_err, sizeof(g_noalloc_err), "%s", text);
+    return st;
+}
+
+extern "C" qlga_status qlga_observable_sums_noalloc(const void* dev_q, const void* dev_qprev, int ndim,
+                                                    const int64_t* dims, qlga_prec prec, int nblocks,
+                                                    double* dev_sums, void* cuda_stream) {
+    using namespace qlga;
+    if (!dev_q || !dev_sums || !dims || ndim < 1 || ndim > 3)
+        return noalloc_fail(QLGA_EINVAL, "qlga_observable_sums_noalloc: NULL pointer or bad ndim");
+    const int64_t nx = dims[0], ny = dims[1], nz = (ndim == 3) ? dims[2] : 1;
+    if (nx < 1 || ny < 1 || nz < 1 || (ndim == 1 && ny != 1) || (double)nx * (double)ny * (double)nz > 1.0e12)
+        return noalloc_fail(QLGA_EINVAL, "qlga_observable_sums_noalloc: bad dims");
+    if (prec != QLGA_F64 && prec != QLGA_F32 && prec != QLGA_F32X)
+        return noalloc_fail(QLGA_EINVAL, "qlga_observable_sums_noalloc: bad precision");
+    if (nblocks < 0 || nblocks > QLGA_NOALLOC_MAX_BLOCKS)
+        return noalloc_fail(QLGA_EINVAL, "qlga_observable_sums_noalloc: nblocks beyond QLGA_NOALLOC_MAX_BLOCKS (2048): "
+                                         "the static scratch holds 19 partial sums for at most that many blocks");
+    // the device that holds the state; run there whatever device is current, restore on return
+    cudaPointerAttributes at;
+    cudaError_t e = cudaPointerGetAttributes(&at, dev_q);
+    if (e != cudaSuccess) { cudaGetLastError(); return noalloc_fail(QLGA_ECUDA, "qlga_observable_sums_noalloc: cudaPointerGetAttributes", e); }
+    if (at.type != cudaMemoryTypeDevice && at.type != cudaMemoryTypeManaged)
+        return noalloc_fail(QLGA_EINVAL, "qlga_observable_sums_noalloc: dev_q is not device memory");
+    const int dev = at.device;
+    if (dev < 0 || dev >= 64) return noalloc_fail(QLGA_EUNSUP, "qlga_observable_sums_noalloc: device ordinal beyond 63");
+    int caller_dev = -1;
+    if ((e = cudaGetDevice(&caller_dev)) != cudaSuccess) return noalloc_fail(QLGA_ECUDA, "cudaGetDevice", e);
+    const bool switched = caller_dev != dev;
+    if (switched && (e = cudaSetDevice(dev)) != cudaSuccess) return noalloc_fail(QLGA_ECUDA, "cudaSetDevice", e);
+
+    // set-up, once per device, with that device current: the device address of the static array and the SM count
+    static std::atomic<double*> scratch_of[64];
+    static std::atomic<int> sms_of[64];
+    qlga_status st = QLGA_OK;
+    double* scratch = scratch_of[dev].load(std::memory_order_acquire);
+    if (!scratch) {
+        double* p = nullptr;
+        int sms = 0;
+        e = cudaGetSymbolAddress((void**)&p, g_noalloc_scratch);
+        if (e == cudaSuccess) e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+        if (e != cudaSuccess || !p) {
+            cudaGetLastError();
+            st = noalloc_fail(QLGA_ECUDA, "qlga_observable_sums_noalloc: cudaGetSymbolAddress(static scratch)", e);
+        } else {
+            sms_of[dev].store(sms, std::memory_order_relaxed);
+            scratch_of[dev].store(p, std::memory_order_release);
+            scratch = p;
+        }
+    }
+    if (st == QLGA_OK) {
+        const int64_t n = nx * ny * nz;
+        int blocks = nblocks ? nblocks : sms_of[dev].load(std::memory_order_relaxed) * 8;     // qlga_observable_sums' grid
+        if (blocks > QLGA_NOALLOC_MAX_BLOCKS) blocks = QLGA_NOALLOC_MAX_BLOCKS;
+        if ((int64_t)blocks * 256 > n) blocks = (int)((n + 255) / 256);
+        int64_t launches = 0;
+        Launch L{(cudaStream_t)cuda_stream, &launches, dev};
+        double* partials = scratch;
+        double* sums = scratch + (size_t)QLGA_NOALLOC_MAX_BLOCKS * OBS_NACC;
+        e = launch_observables(L, prec == QLGA_F64 ? QLGA_F64 : QLGA_F32, dev_q, dev_qprev, nx, ny, nz, ndim, 0, n,
+                               partials, blocks, sums);
+        if (e == cudaSuccess)
+            e = cudaMemcpyAsync(dev_sums, sums, sizeof(double) * QLGA_NSUMS, cudaMemcpyDeviceToDevice, L.stream);
+        if (e != cudaSuccess) { cudaGetLastError(); st = noalloc_fail(QLGA_ECUDA, "qlga_observable_sums_noalloc: launch", e); }
+    }
+    if (switched) cudaSetDevice(caller_dev);
+    return st;
+}

@@ -31,7 +31,7 @@ ABI_SYMBOLS = (
     "qlga_density", "qlga_density_l2_error", "qlga_vortices",
     "qlga_slab_configure", "qlga_slab_edge_get", "qlga_slab_ghost_set",
     "qlga_observable_sums", "qlga_observables_from_sums", "qlga_exp_degree", "qlga_set_chemical_potential",
-    "qlga_angle_stats", "qlga_issue_peak",
+    "qlga_angle_stats", "qlga_issue_peak", "qlga_observable_sums_noalloc", "qlga_noalloc_last_error",
 )
 NSUMS = 17
 
@@ -116,6 +116,10 @@ def load_library():
     lib.qlga_angle_stats.restype = I
     lib.qlga_issue_peak.argtypes = [I, P, ctypes.POINTER(D), ctypes.POINTER(D), ctypes.POINTER(D)]
     lib.qlga_issue_peak.restype = I
+    lib.qlga_observable_sums_noalloc.argtypes = [P, P, I, ctypes.POINTER(I64), I, I, P, P]
+    lib.qlga_observable_sums_noalloc.restype = I
+    lib.qlga_noalloc_last_error.argtypes = []
+    lib.qlga_noalloc_last_error.restype = ctypes.c_char_p
     lib.qlga_version.argtypes = []
     lib.qlga_version.restype = ctypes.c_char_p
     return lib
@@ -157,6 +161,27 @@ def issue_peak(kind, stream=None):
     if st != QLGA_OK:
         raise QlgaError(st, "qlga_issue_peak failed")
     return {"instr_per_s": a.value, "instr_per_clk_per_sm": b.value, "ms": c.value}
+
+
+NOALLOC_MAX_BLOCKS = 2048
+
+
+def observable_sums_noalloc(q, qprev, ndim, dims, precision, out, nblocks=0, stream=None):
+    """qlga_observable_sums_noalloc: the NSUMS lattice sums of the device state `q` (torch tensor, layout
+    [5][2][..lattice..] complex) into the device tensor `out` (float64, >= NSUMS elements), with no context
+    and no device allocation (static scratch inside the library; calls that overlap on the GPU race).
+    Asynchronous on `stream` (default: torch's current stream)."""
+    import torch
+    assert q.is_cuda and q.is_contiguous() and out.is_cuda and out.is_contiguous()
+    assert out.dtype == torch.float64 and out.numel() >= NSUMS
+    if stream is None:
+        stream = torch.cuda.current_stream(q.device)
+    d = (ctypes.c_int64 * 3)(*_dims3(ndim, dims))
+    st = _lib.qlga_observable_sums_noalloc(q.data_ptr(), qprev.data_ptr() if qprev is not None else None, int(ndim), d,
+                                           _PRECISIONS[precision], int(nblocks), out.data_ptr(),
+                                           ctypes.c_void_p(stream.cuda_stream))
+    if st != QLGA_OK:
+        raise QlgaError(st, _lib.qlga_noalloc_last_error().decode())
 
 
 def _dims3(ndim, dims):
