@@ -63,6 +63,7 @@ def parse_args():
     ap.add_argument("--threads-y", type=int, default=0)
     ap.add_argument("--steps-per-launch", type=int, default=0, help="QLGA_OPT_STEPS_PER_LAUNCH (1D)")
     ap.add_argument("--tol-log2", type=int, default=0, help="QLGA_OPT_EXP_TOL_LOG2 override (experiments only)")
+    ap.add_argument("--mod-shift", type=int, default=-1, help="QLGA_OPT_EXP_MOD_SHIFT override (experiments only)")
     ap.add_argument("--slab", action="store_true",
                     help="one lattice cut into slabs along its slowest axis, one slab per GPU, 4-layer halo exchange "
                          "per step (paper_1907_12834_b200/slab.py); weak scaling: every rank owns the workload's lattice "
@@ -414,6 +415,8 @@ def main():
         sim.set_option(qlga.OPT_STEPS_PER_LAUNCH, args.steps_per_launch)
     if args.tol_log2:
         sim.set_option(qlga.OPT_EXP_TOL_LOG2, args.tol_log2)
+    if args.mod_shift >= 0:
+        sim.set_option(qlga.OPT_EXP_MOD_SHIFT, args.mod_shift)
     omega_dev = (torch.empty((5, sim.ny, nx), dtype=torch.float64 if args.precision == "f64" else torch.float32,
                              device=dev) if ndim == 2 else None)
     state_bytes = q_host.numel() * q_host.element_size()
@@ -524,7 +527,7 @@ def main():
             "roofline": roof, "cpu_baseline": cpu,
             "hbm_model_frac": value / world * 1e9 * bps / (hbm_peak * 1e9),
             "kernel_ms": {k: {"ms_total": v[0], "launches": v[1]} for k, v in prof.items()},
-            "pass_kernel_share_of_step": pass_ms / ms if ms > 0 else None,
+            "pass_kernel_share_of_step": sum(v[0] for v in prof.values()) / ms if ms > 0 else None,
             "norm_q_drift": obs["norm_q"] / obs0["norm_q"] - 1.0,
             "sim_step": obs["step"]}
     if ss is not None:

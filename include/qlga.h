@@ -76,9 +76,14 @@ typedef enum {
                                  step t+1 is applied at the end of step t's x pass (same operator product, no halo
                                  recompute of U, and it fills the memory-bound pass); 0 = always on the first pass */
     QLGA_OPT_F32_PHASE = 7,   /* QLGA_F32 only: formulation of the scalar phase factor exp(-i s (c0 rho + mu)):
-                                 0 = (cos, -sin) rounded to fp32, 1 = 1 + d with cos - 1 kept to its own precision
-                                 (default), 2 = 1 + d with d evaluated in fp64 */
-    QLGA_OPT_EXP_POLY = 8     /* interaction polynomial: 0 = Chebyshev-economised Taylor, 1 = plain Taylor */
+                                 0 = (cos, -sin) rounded to fp32 (default), 1 = 1 + d with cos - 1 kept to its own
+                                 precision, 2 = 1 + d with d evaluated in fp64 (measured: DESIGN.md section 8) */
+    QLGA_OPT_EXP_POLY = 8,    /* interaction polynomial: 0 = Chebyshev-economised Taylor, 1 = plain Taylor */
+    QLGA_OPT_EXP_MOD_SHIFT = 9 /* the MODULUS part of the truncation error (the even part of the polynomial) is held to
+                                 2^(tol_log2 - shift): a modulus error that repeats at every application changes the
+                                 density and with it the phase rate c0 rho, and grows like applications x (c0 rho t / 2)
+                                 (DESIGN.md section 8).  0..16; default 9 for fp64 arithmetic (QLGA_F64, QLGA_F32X),
+                                 0 for QLGA_F32 */
 } qlga_option;
 
 /* Lattice sums returned by qlga_observables (always double).
@@ -181,6 +186,21 @@ qlga_status qlga_density_l2_error(qlga_ctx*, const void* rho_ref, int src_on_dev
  * *host_count (may exceed max_out).  Synchronises the stream.  QLGA_EUNSUP in 1D. */
 qlga_status qlga_vortices(qlga_ctx*, int32_t* host_out, int64_t max_out, int64_t* host_count);
 
+/* Vortex tracking, 2D only: association of two detections (the paper follows vortices of positive / negative
+ * winding as tracks, Figs. 18, 21, 22; the tracker is not printed: reading R18 of DESIGN.md).
+ * host_prev / host_cur: HOST int32 [n][4] records (j, x, y, w) as written by qlga_vortices at two times.  Two
+ * records can be the same vortex only if they agree in j and w.  With d2 the periodic (minimal-image) squared
+ * lattice distance, the nearest candidate of a record is the record of the other list with the same (j, w)
+ * and d2 <= max_dist2 that minimises (d2, y, x) lexicographically; two records are matched iff each is the
+ * other's nearest candidate.  host_match_cur[i] = index into prev of the match of cur[i], or -1 (a vortex that
+ * appeared); host_match_prev[k] = index into cur, or -1 (a vortex that disappeared: annihilation with a partner of
+ * opposite winding, or a jump beyond max_dist2).  At most QLGA_MATCH_MAX records per list.  The O(n_prev n_cur)
+ * search runs on the device.  Synchronises the stream.  QLGA_EINVAL (arguments, a record outside the lattice),
+ * QLGA_EUNSUP (not 2D). */
+#define QLGA_MATCH_MAX 65536
+qlga_status qlga_vortex_match(qlga_ctx*, const int32_t* host_prev, int64_t n_prev, const int32_t* host_cur,
+                              int64_t n_cur, int64_t max_dist2, int32_t* host_match_cur, int32_t* host_match_prev);
+
 /* ---- Slab decomposition over several GPUs ---------------------
  * The paper only states that its code "naturally scales with the number of GPUs"
  * (PAPER.md:1092-1094).  Here the lattice is cut into slabs along its slowest axis (x in 1D,
@@ -230,12 +250,13 @@ qlga_status qlga_profile_read(qlga_ctx*, qlga_profile* host_out);
 /* The polynomial the kernels use for the interaction exponential (host only, needs no GPU):
  * exp(-i s K) v = P_p(y) v, y = -i s K, P_p(y) = b0 (1 + r[1] y (1 + r[2] y (... (1 + r[p] y)))),
  * the Chebyshev-economised Taylor polynomial of degree p, valid for ||s K|| <= *theta_max within
- * 2^tol_log2.  p = 1..12.  Exposed so that the table can be tested on the CPU. */
-qlga_status qlga_exp_polynomial(int tol_log2, int p, double* theta_max, double* b0, double* r);
+ * 2^tol_log2, its even (modulus) part within 2^(tol_log2 - mod_shift) (mod_shift as
+ * QLGA_OPT_EXP_MOD_SHIFT).  p = 1..12.  Exposed so that the table can be tested on the CPU. */
+qlga_status qlga_exp_polynomial(int tol_log2, int mod_shift, int p, double* theta_max, double* b0, double* r);
 /* The degree the kernels pick for a (warp-uniform) angle theta <= min(theta_max of degree 12, 1/2): a table
  * lookup on the exponent and the top four mantissa bits of theta as a float, whose entry serves the upper
  * edge of its bucket -- never below "smallest p with theta <= theta_max(p)", at most one above (host only). */
-qlga_status qlga_exp_degree(int tol_log2, double theta, int* p);
+qlga_status qlga_exp_degree(int tol_log2, int mod_shift, double theta, int* p);
 
 /* The lattice sums of qlga_observable_sums for callers that cannot allocate device memory (code under CUDA
  * graph capture, tight serving loops, harnesses that forbid cudaMalloc).  Needs NO context (qlga_init allocates

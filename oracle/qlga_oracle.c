@@ -490,3 +490,54 @@ void orc_winding(const cplx *q, long nx, long ny, int *wind)
                 wind[(size_t)j * n + ia] = (int)lrint((double)(circ / twopi));
             }
 }
+
+/* ------------------------------------------------------------------------
+ * Association of two vortex detections (vortex tracking; the paper follows
+ * "vortices with a positive / negative winding number" as red / blue tracks, Figs. 18, 21, 22,
+ * PAPER.md:971-999, and does not print its tracker)  [R18]:
+ * records (j, x, y, w) as rows of int[4] (the non-zero entries of orc_winding).  Two records can be the
+ * same vortex at two times only if they agree in channel j and winding w.  d2 = periodic (minimal-image)
+ * squared lattice distance.  The nearest candidate of a record is the record of the other list with the
+ * same (j, w) and d2 <= max_d2 that comes first in the order (d2, y, x); two records are matched iff each
+ * is the other's nearest candidate.  match_cur[i] = index into prev or -1, match_prev[k] = index into cur or -1.
+ * Written as the definition: all pairs, no spatial search structure.
+ * Pins (tests/test_oracle_tracking.py): hand-made cases (wrap-around distance, sign and channel mismatch,
+ * the cut-off, a tie, a non-mutual pair), invariance under permutation of the lists, and the tracked speed
+ * 2p of a kicked Pade quadrupole (eq. 71 with the units pinned by PAPER.md:906, 922).
+ * ---------------------------------------------------------------------- */
+static long match_d2(const int *a, const int *b, long nx, long ny)
+{
+    long dx = labs((long)a[1] - (long)b[1]), dy = labs((long)a[2] - (long)b[2]);
+    if (nx - dx < dx) dx = nx - dx;
+    if (ny - dy < dy) dy = ny - dy;
+    return dx * dx + dy * dy;
+}
+
+static void nearest_candidates(const int *a, long na, const int *b, long nb, long nx, long ny, long max_d2, int *nn)
+{
+    for (long i = 0; i < na; ++i) {
+        long best = -1, best_d2 = 0;
+        for (long k = 0; k < nb; ++k) {
+            if (b[4 * k] != a[4 * i] || b[4 * k + 3] != a[4 * i + 3]) continue;
+            long d2 = match_d2(a + 4 * i, b + 4 * k, nx, ny);
+            if (d2 > max_d2) continue;
+            int first = best < 0 || d2 < best_d2
+                     || (d2 == best_d2 && (b[4 * k + 2] < b[4 * best + 2]
+                                           || (b[4 * k + 2] == b[4 * best + 2] && b[4 * k + 1] < b[4 * best + 1])));
+            if (first) { best = k; best_d2 = d2; }
+        }
+        nn[i] = (int)best;
+    }
+}
+
+void orc_vortex_match(const int *prev, long np, const int *cur, long nc, long nx, long ny, long max_d2,
+                      int *match_cur, int *match_prev)
+{
+    int *nn_cur = (int *)malloc(sizeof(int) * (size_t)(nc > 0 ? nc : 1));
+    int *nn_prev = (int *)malloc(sizeof(int) * (size_t)(np > 0 ? np : 1));
+    nearest_candidates(cur, nc, prev, np, nx, ny, max_d2, nn_cur);
+    nearest_candidates(prev, np, cur, nc, nx, ny, max_d2, nn_prev);
+    for (long i = 0; i < nc; ++i) match_cur[i] = (nn_cur[i] >= 0 && nn_prev[nn_cur[i]] == i) ? nn_cur[i] : -1;
+    for (long k = 0; k < np; ++k) match_prev[k] = (nn_prev[k] >= 0 && nn_cur[nn_prev[k]] == k) ? nn_prev[k] : -1;
+    free(nn_cur); free(nn_prev);
+}

@@ -71,6 +71,8 @@ class Oracle:
             fn.argtypes = args
             fn.restype = None
 
+        self.lib.orc_vortex_match.argtypes = [P, L, P, L, L, L, L, P, P]
+        self.lib.orc_vortex_match.restype = None
         self.lib.orc_density_l2_error.argtypes = [P, P, L, L, L]
         self.lib.orc_density_l2_error.restype = ctypes.c_double
 
@@ -214,3 +216,14 @@ class Oracle:
         w = np.empty((5, ny, nx), dtype=np.int32)
         self.lib.orc_winding(self._p(q), nx, ny, self._p(w))
         return w
+
+    def vortex_match(self, prev, cur, dims, max_dist2):
+        """(match_cur, match_prev): mutual nearest neighbours of equal channel and winding under the periodic
+        metric of the (Nx, Ny) lattice; records are int32 rows (j, x, y, w)."""
+        prev = np.ascontiguousarray(prev, dtype=np.int32).reshape(-1, 4)
+        cur = np.ascontiguousarray(cur, dtype=np.int32).reshape(-1, 4)
+        mc = np.full(max(len(cur), 1), -1, dtype=np.int32)
+        mp = np.full(max(len(prev), 1), -1, dtype=np.int32)
+        self.lib.orc_vortex_match(self._p(prev), len(prev), self._p(cur), len(cur), int(dims[0]), int(dims[1]),
+                                  int(max_dist2), self._p(mc), self._p(mp))
+        return mc[:len(cur)], mp[:len(prev)]

@@ -11,10 +11,12 @@ using namespace qlga;
 
 static char g_init_err[512] = "";
 
-// defaults of the fp32 kernels (QLGA_F32), settled by the measured error growth against the fp64 oracle
-// (DESIGN.md section 8): phase factor as 1 + d, truncation target, polynomial kind
+// defaults of the fp32 kernels (QLGA_F32), settled by the measured error growth against the fp64 path
+// (DESIGN.md section 8): none of the formulations built (phase factor as 1 + d, in fp32 or fp64; tighter
+// truncation; Taylor instead of economised coefficients) changes the order of magnitude of the fp32 error at
+// the stated step counts, so the fastest one stays the default and QLGA_F32X is the accurate variant
 #ifndef QLGA_F32_PHASE_DEFAULT
-#define QLGA_F32_PHASE_DEFAULT 1
+#define QLGA_F32_PHASE_DEFAULT 0
 #endif
 #ifndef QLGA_F32_TOL_DEFAULT
 #define QLGA_F32_TOL_DEFAULT -27
@@ -22,6 +24,10 @@ static char g_init_err[512] = "";
 #ifndef QLGA_F32_POLY_DEFAULT
 #define QLGA_F32_POLY_DEFAULT 0
 #endif
+#ifndef QLGA_F64_MOD_SHIFT_DEFAULT
+#define QLGA_F64_MOD_SHIFT_DEFAULT 9
+#endif
+static const int F64_MOD_SHIFT = QLGA_F64_MOD_SHIFT_DEFAULT;
 static const int F32_PHASE_MODE = QLGA_F32_PHASE_DEFAULT, F32_TOL_LOG2 = QLGA_F32_TOL_DEFAULT, F32_EXP_POLY = QLGA_F32_POLY_DEFAULT;
 
 static qlga_status fail(const qlga_ctx* cc, qlga_status st, const char* fmt, const char* a = "") {
@@ -70,7 +76,15 @@ struct DeviceGuard {
 // -i sin x, so the real polynomial A(x) = sum_j sigma_j b_j x^j, sigma_j = (-1)^(j/2),
 // (Taylor: cos x + sin x) is economised; T_n has the parity of n, so parities never mix.
 // ---------------------------------------------------------------------------
-static long double economise(int p, long double theta, long double* b /*[p+1]*/) {
+// *err_even (optional): the part of the bound that belongs to the even (cosine) part of the polynomial.  With
+// y = -i x an eigencomponent is multiplied by A(x) - i B(x), A even, B odd, and |A - iB|^2 = 1 + 2 eps_A + 2 x eps_B:
+// the even part's error is a MODULUS error, the odd part's a phase error.  A modulus error that repeats at
+// every application changes the density, hence the rate c0 rho of the scalar phase: it grows like
+// (c0 rho t / 2) x applications x bias (measured: DESIGN.md section 8), so it is bounded separately.
+// *b0m1 (optional): b_0 - 1, accumulated on its own (at tolerances near 2^-64 it is below the resolution of
+// 1 + x even in long double).
+static long double economise(int p, long double theta, long double* b /*[p+1]*/, long double* err_even = nullptr,
+                             long double* b0m1 = nullptr) {
     const int N = p + 4;
     long double beta[QLGA_PMAX + 8], fact = 1.0L, pw = 1.0L;
     for (int n = 0; n <= N; ++n) {
@@ -79,26 +93,34 @@ static long double economise(int p, long double theta, long double* b /*[p+1]*/)
         beta[n] = sigma * pw / fact;                       // a_n theta^n
     }
     long double err = pw * theta / (fact * (long double)(N + 1));   // Taylor remainder of degree N
+    long double ee = err;
     long double tc[QLGA_PMAX + 8][QLGA_PMAX + 8];          // T_n(t) = sum_k tc[n][k] t^k
     for (int n = 0; n <= N; ++n) for (int k = 0; k <= N; ++k) tc[n][k] = 0.0L;
     tc[0][0] = 1.0L; tc[1][1] = 1.0L;
     for (int n = 2; n <= N; ++n)
         for (int k = 0; k <= n; ++k)
             tc[n][k] = (k > 0 ? 2.0L * tc[n - 1][k - 1] : 0.0L) - tc[n - 2][k];
+    long double c0 = 0.0L;                                 // beta[0] - 1, kept apart from the 1
     for (int n = N; n > p; --n) {                          // remove degree n
         const long double lam = beta[n] / tc[n][n];
-        for (int k = 0; k <= n; ++k) beta[k] -= lam * tc[n][k];
+        for (int k = 1; k <= n; ++k) beta[k] -= lam * tc[n][k];
+        c0 -= lam * tc[n][0];
         beta[n] = 0.0L;
         err += fabsl(lam);
+        if (n % 2 == 0) ee += fabsl(lam);                  // T_n has the parity of n
     }
     pw = 1.0L;
     for (int j = 0; j <= p; ++j) {
         if (j > 0) pw *= theta;
         const long double sigma = ((j / 2) % 2 == 0) ? 1.0L : -1.0L;
-        b[j] = sigma * beta[j] / pw;
+        b[j] = (j == 0) ? 1.0L + c0 : sigma * beta[j] / pw;
     }
     // the constant term is stored in double: a correction below half an ulp of 1 is lost
-    err += fabsl(b[0] - (long double)(double)b[0]);
+    const long double lost = fabsl(c0 - ((long double)(double)(1.0L + c0) - 1.0L));
+    err += lost;
+    ee += lost;
+    if (err_even) *err_even = ee;
+    if (b0m1) *b0m1 = c0;
     return err;
 }
 
@@ -107,31 +129,45 @@ static long double economise(int p, long double theta, long double* b /*[p+1]*/)
 // poly = 1: the plain Taylor polynomial instead (b_k = 1/k!): its leading ratios 1, 1/2 and b0 = 1 are exact
 // in binary floating point, which matters in fp32, where a ratio rounded by 3e-8 is the same relative
 // error of the angle at every application.
-static long double taylor(int p, long double theta, long double* b /*[p+1]*/) {
+static long double taylor(int p, long double theta, long double* b /*[p+1]*/, long double* err_even = nullptr,
+                          long double* b0m1 = nullptr) {
+    if (b0m1) *b0m1 = 0.0L;
     long double fact = 1.0L, pw = 1.0L;
     for (int k = 0; k <= p; ++k) {
         if (k > 0) { fact *= (long double)k; pw *= theta; }
         b[k] = 1.0L / fact;
     }
-    return pw * theta / (fact * (long double)(p + 1)) * (1.0L + theta);   // first dropped term, with the tail's margin
+    const long double d1 = pw * theta / (fact * (long double)(p + 1)) * (1.0L + theta);   // first dropped term (degree p+1), with the tail's margin
+    const long double d2 = d1 * theta / (long double)(p + 2);                            // the next one (degree p+2)
+    if (err_even) *err_even = ((p + 1) % 2 == 0) ? d1 : d2;
+    return d1;
 }
 
-static void build_exp_table(ExpTable& tab, int tol_log2, int poly = 0, int phase_mode = 0) {
+// mod_shift: the even (modulus) part of the error is held to tol * 2^-mod_shift (0 = no separate bound).
+static void build_exp_table(ExpTable& tab, int tol_log2, int poly = 0, int phase_mode = 0, int mod_shift = 0) {
     const long double tol = ldexpl(1.0L, tol_log2);
+    const long double tol_mod = ldexpl(1.0L, tol_log2 - mod_shift);
     tab.phase_mode = phase_mode;
     for (int p = 1; p <= QLGA_PMAX; ++p) {
         long double b[QLGA_PMAX + 1];
         long double lo = 0.0L, hi = 4.0L;
         for (int it = 0; it < 200; ++it) {
             const long double mid = 0.5L * (lo + hi);
-            if ((poly ? taylor(p, mid, b) : economise(p, mid, b)) <= tol) lo = mid; else hi = mid;
+            long double ee = 0.0L;
+            const long double et = poly ? taylor(p, mid, b, &ee) : economise(p, mid, b, &ee);
+            // modulus error of an eigencomponent: eps_A cos x + eps_B sin x <= (even part) + theta (odd part)
+            if (et <= tol && (mod_shift == 0 || ee + mid * et <= tol_mod)) lo = mid; else hi = mid;
         }
         long double th = lo * 0.999L;                      // margin for the fp32 angle estimate
-        if (poly) taylor(p, th, b); else economise(p, th, b);
+        long double c0 = 0.0L;
+        if (poly) taylor(p, th, b, nullptr, &c0); else economise(p, th, b, nullptr, &c0);
         tab.thr[p - 1] = (float)th;
         if ((long double)tab.thr[p - 1] > th) tab.thr[p - 1] = nextafterf(tab.thr[p - 1], 0.0f);
+        // with a separate modulus bound a degree can serve less than the one below it: the rule "smallest p with
+        // theta <= thr[p-1]" then never picks it; keep the thresholds ascending for the compare tree
+        if (p > 1 && tab.thr[p - 1] < tab.thr[p - 2]) tab.thr[p - 1] = tab.thr[p - 2];
         tab.b0[p - 1] = (double)b[0];
-        tab.b0m1[p - 1] = (double)(b[0] - 1.0L);
+        tab.b0m1[p - 1] = (double)c0;
         tab.b0m1f[p - 1] = (float)tab.b0m1[p - 1];
         for (int k = 0; k <= QLGA_PMAX; ++k) tab.r[p - 1][k] = 0.0;
         for (int k = 1; k <= p; ++k) tab.r[p - 1][k] = (double)(b[k] / b[k - 1]);
@@ -164,12 +200,12 @@ static void build_exp_table(ExpTable& tab, int tol_log2, int poly = 0, int phase
 }
 
 // Introspection of the polynomial table (host only, no GPU): used by the CPU tests.
-extern "C" qlga_status qlga_exp_polynomial(int tol_log2, int p, double* theta_max, double* b0,
+extern "C" qlga_status qlga_exp_polynomial(int tol_log2, int mod_shift, int p, double* theta_max, double* b0,
                                            double* r /* [p+1], r[0] unused */) {
-    if (p < 1 || p > QLGA_PMAX || tol_log2 > -8 || tol_log2 < -100 || !theta_max || !b0 || !r)
+    if (p < 1 || p > QLGA_PMAX || tol_log2 > -8 || tol_log2 < -100 || mod_shift < 0 || mod_shift > 16 || !theta_max || !b0 || !r)
         return QLGA_EINVAL;
     static ExpTable tab;                                   // 1.3 KB: keep it off the stack
-    build_exp_table(tab, tol_log2);
+    build_exp_table(tab, tol_log2, 0, 0, mod_shift);
     *theta_max = tab.thr[p - 1];
     *b0 = tab.b0[p - 1];
     for (int k = 0; k <= p; ++k) r[k] = tab.r[p - 1][k];
@@ -177,10 +213,10 @@ extern "C" qlga_status qlga_exp_polynomial(int tol_log2, int p, double* theta_ma
 }
 
 // The degree the kernels' lookup table gives for a warp-uniform angle theta (host only).
-extern "C" qlga_status qlga_exp_degree(int tol_log2, double theta, int* p) {
-    if (tol_log2 > -8 || tol_log2 < -100 || !p || !(theta >= 0.0)) return QLGA_EINVAL;
+extern "C" qlga_status qlga_exp_degree(int tol_log2, int mod_shift, double theta, int* p) {
+    if (tol_log2 > -8 || tol_log2 < -100 || mod_shift < 0 || mod_shift > 16 || !p || !(theta >= 0.0)) return QLGA_EINVAL;
     static ExpTable tab;
-    build_exp_table(tab, tol_log2);
+    build_exp_table(tab, tol_log2, 0, 0, mod_shift);
     if (theta > tab.theta_split) return QLGA_EINVAL;          // the kernels split such angles first
     const float th = (float)theta;
     uint32_t bits;
@@ -269,7 +305,8 @@ extern "C" qlga_status qlga_init(qlga_ctx** out, int ndim, const int64_t* dims,
     c->tol_log2 = (prec == QLGA_F32) ? F32_TOL_LOG2 : -56;
     c->exp_poly = (prec == QLGA_F32) ? F32_EXP_POLY : 0;
     c->f32_phase = F32_PHASE_MODE;
-    build_exp_table(c->tab, c->tol_log2, c->exp_poly, c->f32_phase);
+    c->exp_mod_shift = (prec == QLGA_F32) ? 0 : F64_MOD_SHIFT;
+    build_exp_table(c->tab, c->tol_log2, c->exp_poly, c->f32_phase, c->exp_mod_shift);
     c->obs_blocks = prop.multiProcessorCount * 8;
     cudaError_t e = cudaMalloc(&c->d_partials, sizeof(double) * (size_t)c->obs_blocks * OBS_NACC);
     if (e == cudaSuccess) e = cudaMalloc(&c->d_sums, sizeof(double) * OBS_NACC);
@@ -313,7 +350,7 @@ extern "C" qlga_status qlga_set_option(qlga_ctx* c, qlga_option key, int64_t v) 
             c->steps_per_launch = (int)v; return QLGA_OK;
         case QLGA_OPT_EXP_TOL_LOG2:
             if (v > -8 || v < -100) return fail(c, QLGA_EINVAL, "QLGA_OPT_EXP_TOL_LOG2: -100..-8");
-            c->tol_log2 = (int)v; build_exp_table(c->tab, c->tol_log2, c->exp_poly, c->f32_phase); return QLGA_OK;
+            c->tol_log2 = (int)v; build_exp_table(c->tab, c->tol_log2, c->exp_poly, c->f32_phase, c->exp_mod_shift); return QLGA_OK;
         case QLGA_OPT_THREADS_X:
             if (!pass_tile_supported(0, (int)v, 1)) return fail(c, QLGA_EINVAL, "QLGA_OPT_THREADS_X: 0, 64, 96, 128, 192, 256");
             c->threads_x = (int)v; return QLGA_OK;
@@ -328,10 +365,13 @@ extern "C" qlga_status qlga_set_option(qlga_ctx* c, qlga_option key, int64_t v) 
             c->tile_y = (int)v; return QLGA_OK;
         case QLGA_OPT_F32_PHASE:
             if (v < 0 || v > 2) return fail(c, QLGA_EINVAL, "QLGA_OPT_F32_PHASE: 0, 1 or 2");
-            c->f32_phase = (int)v; build_exp_table(c->tab, c->tol_log2, c->exp_poly, c->f32_phase); return QLGA_OK;
+            c->f32_phase = (int)v; build_exp_table(c->tab, c->tol_log2, c->exp_poly, c->f32_phase, c->exp_mod_shift); return QLGA_OK;
+        case QLGA_OPT_EXP_MOD_SHIFT:
+            if (v < 0 || v > 16) return fail(c, QLGA_EINVAL, "QLGA_OPT_EXP_MOD_SHIFT: 0..16");
+            c->exp_mod_shift = (int)v; build_exp_table(c->tab, c->tol_log2, c->exp_poly, c->f32_phase, c->exp_mod_shift); return QLGA_OK;
         case QLGA_OPT_EXP_POLY:
             if (v != 0 && v != 1) return fail(c, QLGA_EINVAL, "QLGA_OPT_EXP_POLY: 0 (economised) or 1 (Taylor)");
-            c->exp_poly = (int)v; build_exp_table(c->tab, c->tol_log2, c->exp_poly, c->f32_phase); return QLGA_OK;
+            c->exp_poly = (int)v; build_exp_table(c->tab, c->tol_log2, c->exp_poly, c->f32_phase, c->exp_mod_shift); return QLGA_OK;
         case QLGA_OPT_FUSE_PLAIN_U:
             if (v != 0 && v != 1) return fail(c, QLGA_EINVAL, "QLGA_OPT_FUSE_PLAIN_U: 0 or 1");
             c->fuse_plain_u = (int)v; return QLGA_OK;
@@ -878,5 +918,43 @@ extern "C" qlga_status qlga_vortices(qlga_ctx* c, int32_t* host_out, int64_t max
     }
     if (e != cudaSuccess) return cuda_fail(c, "qlga_vortices", e);
     *host_count = (int64_t)hc;
+    return QLGA_OK;
+}
+
+// ---------------------------------------------------------------------------
+// Vortex tracking: association of two detections (qlga_track.cu)
+// ---------------------------------------------------------------------------
+extern "C" qlga_status qlga_vortex_match(qlga_ctx* c, const int32_t* host_prev, int64_t n_prev,
+                                         const int32_t* host_cur, int64_t n_cur, int64_t max_dist2,
+                                         int32_t* host_match_cur, int32_t* host_match_prev) {
+    if (!c) return QLGA_EINVAL;
+    if (n_prev < 0 || n_cur < 0 || n_prev > QLGA_MATCH_MAX || n_cur > QLGA_MATCH_MAX || max_dist2 < 0 ||
+        (n_prev > 0 && (!host_prev || !host_match_prev)) || (n_cur > 0 && (!host_cur || !host_match_cur)))
+        return fail(c, QLGA_EINVAL, "qlga_vortex_match: bad arguments (at most 65536 records per list)");
+    DeviceGuard guard(c);
+    if (c->ndim != 2) return fail(c, QLGA_EUNSUP, "qlga_vortex_match: 2D lattices only");
+    if (c->nx > 2147483647LL || c->ny > 2147483647LL) return fail(c, QLGA_EUNSUP, "qlga_vortex_match: lattice too large");
+    for (int64_t k = 0; k < n_prev + n_cur; ++k) {
+        const int32_t* r = k < n_prev ? host_prev + 4 * k : host_cur + 4 * (k - n_prev);
+        if (r[0] < 0 || r[0] > 4 || r[1] < 0 || r[1] >= c->nx || r[2] < 0 || r[2] >= c->ny)
+            return fail(c, QLGA_EINVAL, "qlga_vortex_match: record outside the lattice");
+    }
+    if (n_prev + n_cur == 0) return QLGA_OK;
+    // scratch: [prev records][cur records][nn_cur][nn_prev][match_cur][match_prev]
+    const size_t rp = (size_t)n_prev * 16, rc = (size_t)n_cur * 16, ip = (size_t)n_prev * 4, ic = (size_t)n_cur * 4;
+    const qlga_status st = ensure_scratch(c, rp + rc + 2 * (ip + ic) + 64);
+    if (st != QLGA_OK) return st;
+    char* base = (char*)c->d_scratch;
+    int* d_prev = (int*)base; int* d_cur = (int*)(base + rp);
+    int* nn_cur = (int*)(base + rp + rc); int* nn_prev = (int*)(base + rp + rc + ic);
+    int* m_cur = (int*)(base + rp + rc + ic + ip); int* m_prev = (int*)(base + rp + rc + 2 * ic + ip);
+    Launch L{c->stream, &c->launches, c->device};
+    if (n_prev) CU(c, cudaMemcpyAsync(d_prev, host_prev, rp, cudaMemcpyHostToDevice, c->stream));
+    if (n_cur) CU(c, cudaMemcpyAsync(d_cur, host_cur, rc, cudaMemcpyHostToDevice, c->stream));
+    CU(c, launch_vortex_match(L, d_prev, (int)n_prev, d_cur, (int)n_cur, (int)c->nx, (int)c->ny, (long long)max_dist2,
+                              nn_cur, nn_prev, m_cur, m_prev));
+    if (n_cur) CU(c, cudaMemcpyAsync(host_match_cur, m_cur, ic, cudaMemcpyDeviceToHost, c->stream));
+    if (n_prev) CU(c, cudaMemcpyAsync(host_match_prev, m_prev, ip, cudaMemcpyDeviceToHost, c->stream));
+    CU(c, cudaStreamSynchronize(c->stream));
     return QLGA_OK;
 }

@@ -67,6 +67,9 @@ cudaError_t launch_vortices(const Launch& L, qlga_prec prec, const void* q, int6
                             int* list, long long max_out, unsigned long long* counter);
 cudaError_t launch_angle_stats(const Launch& L, qlga_prec prec, const void* q, int64_t nsites, double tg1, double tg2,
                                double g0, double smu, const ExpTable& tab, int nblocks, unsigned long long* out /*[15]*/);
+// association of two vortex detections (qlga_track.cu); all pointers DEVICE, records int32 [n][4] = (j, x, y, w)
+cudaError_t launch_vortex_match(const Launch& L, const int* prev, int np, const int* cur, int nc, int nx, int ny,
+                                long long max_d2, int* nn_cur, int* nn_prev, int* match_cur, int* match_prev);
 cudaError_t launch_split_psi(const Launch& L, qlga_prec prec, const void* psi, void* q,
                              int64_t nsites, int64_t offset, int64_t count);
 cudaError_t launch_sum_psi(const Launch& L, qlga_prec prec, const void* q, void* psi,
@@ -97,6 +100,7 @@ struct qlga_ctx {
     int fuse_plain_u;      // plain ordering, 2D/3D: the next step's U rides on the x pass (default on)
     int tol_log2;
     int exp_poly;          // 0 economised, 1 Taylor (QLGA_OPT_EXP_POLY)
+    int exp_mod_shift;     // modulus part of the truncation error held to 2^(tol_log2 - shift) (QLGA_OPT_EXP_MOD_SHIFT)
     int f32_phase;         // phase-factor formulation of the fp32 kernels (QLGA_OPT_F32_PHASE)
     int threads_x;
     int tile_y;

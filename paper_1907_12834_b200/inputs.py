@@ -308,3 +308,23 @@ def predicted_energy(kind, k, p):
     """The paper's dispersion relations: E = p^2 - k^2 (bright, eq. 74), E = p^2 + 2 k^2
     (dark, PAPER.md:630)."""
     return p * p - k * k if kind == "bright" else p * p + 2.0 * k * k
+
+
+def kicked_quadrupole(L, core=8.0, n_kick=0, axis="x", couplings=(1.0, 0.3, -0.1), m=2, offset=0.5):
+    """Single-channel Pade-vortex quadrupole in channel m with the paper's kick
+    exp(i 2 pi n x / L) (or y; Figs. 15-16): psi_m = a V(r) e^{i 2 pi n x/L} / sqrt(g),
+    g = c0 + 4 c1 (m = +-2), c0 + c1 (m = +-1) or c0 + c2/5 (m = 0) (Table I rows 1-5 at E = 1), a = 1/core.
+    A stationary state of the paper for n = 0; kicked, the whole pattern drifts at 2 p = 4 pi n / L sites per
+    step (eq. 71; units pinned by the printed drift times).  The vortex centres sit at
+    (L/4, 3L/4) + offset so that no zero of the field falls on a lattice site."""
+    c0, c1, c2 = couplings
+    g = {2: c0 + 4 * c1, 1: c0 + c1, 0: c0 + c2 / 5.0}[abs(m)]
+    a = 1.0 / core
+    X, Y = _grid(L, L)
+    lo, hi = L / 4 + offset, 3 * L / 4 + offset
+    V = np.ones((L, L), dtype=np.complex128)
+    for cx, cy, w in ((lo, lo, +1), (hi, lo, -1), (lo, hi, -1), (hi, hi, +1)):
+        V *= vortex_factor(X, Y, cx, cy, a, w)
+    psi = np.zeros((5, L, L), dtype=np.complex128)
+    psi[j_of_m(m)] = a / np.sqrt(g) * V * np.exp(2j * np.pi * n_kick * (X if axis == "x" else Y) / L)
+    return Workload("kicked_quadrupole_2d", 2, (L, L), tuple(couplings), 0, psi)

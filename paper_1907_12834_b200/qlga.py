@@ -19,7 +19,7 @@ QLGA_OK, QLGA_EINVAL, QLGA_ENOMEM, QLGA_ECUDA, QLGA_ESTATE, QLGA_EUNSUP = range(
 QLGA_F64, QLGA_F32, QLGA_F32X = 0, 1, 2
 QLGA_PLAIN, QLGA_INTERLEAVED = 0, 1
 (OPT_PATH, OPT_STEPS_PER_LAUNCH, OPT_EXP_TOL_LOG2, OPT_THREADS_X, OPT_TILE_Y, OPT_THREADS_Y, OPT_FUSE_PLAIN_U,
- OPT_F32_PHASE, OPT_EXP_POLY) = range(9)
+ OPT_F32_PHASE, OPT_EXP_POLY, OPT_EXP_MOD_SHIFT) = range(10)
 _PRECISIONS = {"f64": QLGA_F64, "fp64": QLGA_F64, "double": QLGA_F64, "f32": QLGA_F32, "fp32": QLGA_F32,
                "float": QLGA_F32, "f32x": QLGA_F32X}
 
@@ -32,6 +32,7 @@ ABI_SYMBOLS = (
     "qlga_slab_configure", "qlga_slab_edge_get", "qlga_slab_ghost_set",
     "qlga_observable_sums", "qlga_observables_from_sums", "qlga_exp_degree", "qlga_set_chemical_potential",
     "qlga_angle_stats", "qlga_issue_peak", "qlga_observable_sums_noalloc", "qlga_noalloc_last_error",
+    "qlga_vortex_match",
 )
 NSUMS = 17
 
@@ -108,9 +109,9 @@ def load_library():
     lib.qlga_observable_sums.restype = I
     lib.qlga_observables_from_sums.argtypes = [P, ctypes.POINTER(D), ctypes.POINTER(QlgaObs)]
     lib.qlga_observables_from_sums.restype = I
-    lib.qlga_exp_polynomial.argtypes = [I, I, ctypes.POINTER(D), ctypes.POINTER(D), ctypes.POINTER(D)]
+    lib.qlga_exp_polynomial.argtypes = [I, I, I, ctypes.POINTER(D), ctypes.POINTER(D), ctypes.POINTER(D)]
     lib.qlga_exp_polynomial.restype = I
-    lib.qlga_exp_degree.argtypes = [I, D, ctypes.POINTER(I)]
+    lib.qlga_exp_degree.argtypes = [I, I, D, ctypes.POINTER(I)]
     lib.qlga_exp_degree.restype = I
     lib.qlga_angle_stats.argtypes = [P, ctypes.POINTER(QlgaAngles)]
     lib.qlga_angle_stats.restype = I
@@ -120,6 +121,8 @@ def load_library():
     lib.qlga_observable_sums_noalloc.restype = I
     lib.qlga_noalloc_last_error.argtypes = []
     lib.qlga_noalloc_last_error.restype = ctypes.c_char_p
+    lib.qlga_vortex_match.argtypes = [P, P, I64, P, I64, I64, P, P]
+    lib.qlga_vortex_match.restype = I
     lib.qlga_version.argtypes = []
     lib.qlga_version.restype = ctypes.c_char_p
     return lib
@@ -132,20 +135,21 @@ def version() -> str:
     return _lib.qlga_version().decode()
 
 
-def exp_polynomial(tol_log2, p):
-    """(theta_max, b0, r[0..p]) of the degree-p interaction polynomial (host only)."""
+def exp_polynomial(tol_log2, p, mod_shift=0):
+    """(theta_max, b0, r[0..p]) of the degree-p interaction polynomial (host only); mod_shift: the even
+    (modulus) part of its error is held to 2^(tol_log2 - mod_shift) (QLGA_OPT_EXP_MOD_SHIFT)."""
     th, b0 = ctypes.c_double(), ctypes.c_double()
     r = (ctypes.c_double * (p + 1))()
-    st = _lib.qlga_exp_polynomial(int(tol_log2), int(p), ctypes.byref(th), ctypes.byref(b0), r)
+    st = _lib.qlga_exp_polynomial(int(tol_log2), int(mod_shift), int(p), ctypes.byref(th), ctypes.byref(b0), r)
     if st != QLGA_OK:
         raise QlgaError(st, "qlga_exp_polynomial: bad arguments")
     return th.value, b0.value, list(r)
 
 
-def exp_degree(tol_log2, theta):
+def exp_degree(tol_log2, theta, mod_shift=0):
     """Degree the kernels' lookup table picks for the angle theta (host only)."""
     p = ctypes.c_int()
-    st = _lib.qlga_exp_degree(int(tol_log2), float(theta), ctypes.byref(p))
+    st = _lib.qlga_exp_degree(int(tol_log2), int(mod_shift), float(theta), ctypes.byref(p))
     if st != QLGA_OK:
         raise QlgaError(st, "qlga_exp_degree: bad arguments")
     return p.value
@@ -377,6 +381,18 @@ class Qlga:
         cnt = ctypes.c_int64()
         self._check(_lib.qlga_vortices(self.ctx, out.ctypes.data, int(max_out), ctypes.byref(cnt)))
         return out[:min(cnt.value, max_out)].copy(), cnt.value
+
+    def vortex_match(self, prev, cur, max_dist2):
+        """(match_cur, match_prev) of two detections (int32 (n, 4) records of vortices()): mutual nearest
+        neighbours with the same channel and winding under the periodic metric (qlga_vortex_match)."""
+        prev = np.ascontiguousarray(prev, dtype=np.int32).reshape(-1, 4)
+        cur = np.ascontiguousarray(cur, dtype=np.int32).reshape(-1, 4)
+        mc = np.full(len(cur), -1, dtype=np.int32)
+        mp = np.full(len(prev), -1, dtype=np.int32)
+        self._check(_lib.qlga_vortex_match(self.ctx, prev.ctypes.data if len(prev) else None, len(prev),
+                                           cur.ctypes.data if len(cur) else None, len(cur), int(max_dist2),
+                                           mc.ctypes.data if len(cur) else None, mp.ctypes.data if len(prev) else None))
+        return mc, mp
 
     def profile_enable(self, on=True):
         self._check(_lib.qlga_profile_enable(self.ctx, int(bool(on))))
