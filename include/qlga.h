@@ -79,6 +79,10 @@ typedef enum {
                                  0 = (cos, -sin) rounded to fp32 (default), 1 = 1 + d with cos - 1 kept to its own
                                  precision, 2 = 1 + d with d evaluated in fp64 (measured: DESIGN.md section 8) */
     QLGA_OPT_EXP_POLY = 8,    /* interaction polynomial: 0 = Chebyshev-economised Taylor, 1 = plain Taylor */
+    QLGA_OPT_MARCH = 10,      /* strided passes that carry no interaction (plain ordering): 1 (default) = column
+                                 marching, one thread per (column, m_f), the four factors as a register pipeline, no
+                                 shared memory (bit-identical results); 0 = the tile kernel.  Setting TILE_Y or
+                                 THREADS_Y also selects the tile kernel */
     QLGA_OPT_EXP_MOD_SHIFT = 9 /* the MODULUS part of the truncation error (the even part of the polynomial) is held to
                                  2^(tol_log2 - shift): a modulus error that repeats at every application changes the
                                  density and with it the phase rate c0 rho, and grows like applications x (c0 rho t / 2)

@@ -17,7 +17,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(CSRC, "build")
 LIB = os.path.join(HERE, "libqlga.so")
-SOURCES = ["qlga_api.cu", "qlga_step.cu", "qlga_step_f32.cu", "qlga_step_mixed.cu", "qlga_diag.cu", "qlga_peak.cu", "qlga_track.cu"]
+SOURCES = ["qlga_api.cu", "qlga_step.cu", "qlga_step_f32.cu", "qlga_step_mixed.cu", "qlga_diag.cu", "qlga_peak.cu", "qlga_track.cu", "qlga_march.cu"]
 HEADERS = ["qlga_math.cuh", "qlga_internal.h", "qlga_pass.cuh", os.path.join("..", "..", "include", "qlga.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC"]

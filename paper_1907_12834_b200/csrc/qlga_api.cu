@@ -301,7 +301,7 @@ extern "C" qlga_status qlga_init(qlga_ctx** out, int ndim, const int64_t* dims,
     c->buf_bytes = buf_bytes;
     c->stream = (cudaStream_t)cuda_stream;
     c->cur = 0; c->prev = -1; c->have_state = 0; c->step = 0; c->launches = 0;
-    c->path = 0; c->steps_per_launch = 0; c->threads_x = 0; c->tile_y = 0; c->fuse_plain_u = 1;
+    c->path = 0; c->steps_per_launch = 0; c->threads_x = 0; c->tile_y = 0; c->fuse_plain_u = 1; c->march = 1;
     c->tol_log2 = (prec == QLGA_F32) ? F32_TOL_LOG2 : -56;
     c->exp_poly = (prec == QLGA_F32) ? F32_EXP_POLY : 0;
     c->f32_phase = F32_PHASE_MODE;
@@ -366,6 +366,9 @@ extern "C" qlga_status qlga_set_option(qlga_ctx* c, qlga_option key, int64_t v) 
         case QLGA_OPT_F32_PHASE:
             if (v < 0 || v > 2) return fail(c, QLGA_EINVAL, "QLGA_OPT_F32_PHASE: 0, 1 or 2");
             c->f32_phase = (int)v; build_exp_table(c->tab, c->tol_log2, c->exp_poly, c->f32_phase, c->exp_mod_shift); return QLGA_OK;
+        case QLGA_OPT_MARCH:
+            if (v != 0 && v != 1) return fail(c, QLGA_EINVAL, "QLGA_OPT_MARCH: 0 or 1");
+            c->march = (int)v; return QLGA_OK;
         case QLGA_OPT_EXP_MOD_SHIFT:
             if (v < 0 || v > 16) return fail(c, QLGA_EINVAL, "QLGA_OPT_EXP_MOD_SHIFT: 0..16");
             c->exp_mod_shift = (int)v; build_exp_table(c->tab, c->tol_log2, c->exp_poly, c->f32_phase, c->exp_mod_shift); return QLGA_OK;
@@ -636,6 +639,12 @@ static qlga_status step_fused(qlga_ctx* c, int64_t nsteps) {
                     cxw = (P.umode != 0) ? (f64 ? 2 : 4) : (f64 ? 4 : 8);
                     if (thr == 0) thr = (P.umode != 0 && f64) ? 128 : 256;
                 } else if (c->ndim == 3 && c->prec == QLGA_F64) { cxw = 2; if (thr == 0) thr = 128; }
+            }
+            if (d > 0 && c->march && c->tile_y == 0 && c->threads_y == 0 && march_supported(d, P)) {
+                // a strided pass without interaction: one thread per (column, m) marching along the line
+                CU(c, launch_march(L, c->prec, d, P));
+                src = dst;
+                continue;
             }
             if (!pass_tile_supported(d == 0 ? 0 : 1, d == 0 ? c->threads_x : thr, d == 0 ? 1 : cxw))
                 return fail(c, QLGA_EINVAL, "qlga_step: no kernel for the (TILE_Y, THREADS_Y) pair this pass resolves to; "

@@ -43,6 +43,9 @@ cudaError_t launch_pass_f32(const Launch& L, int dir, const PassParams& P, int t
 cudaError_t launch_pass_mixed(const Launch& L, int dir, const PassParams& P, int threads, int cx);
 // true if the (columns, threads) pair of a strided pass / the CTA size of the x pass has an instantiation
 bool pass_tile_supported(int dir, int threads, int cx);
+// interaction-free strided pass by column marching (qlga_march.cu): same arithmetic, no shared memory
+bool march_supported(int dir, const PassParams& P);
+cudaError_t launch_march(const Launch& L, qlga_prec prec, int dir, const PassParams& P);
 // widest ksteps the x pass supports with the given CTA size
 int max_ksteps(int threads);
 
@@ -98,6 +101,7 @@ struct qlga_ctx {
     int path;              // 0 fused, 1 per-operator
     int steps_per_launch;  // 1D temporal blocking, 0 = auto
     int fuse_plain_u;      // plain ordering, 2D/3D: the next step's U rides on the x pass (default on)
+    int march;             // interaction-free strided passes by column marching (default on; 0 = tile kernel)
     int tol_log2;
     int exp_poly;          // 0 economised, 1 Taylor (QLGA_OPT_EXP_POLY)
     int exp_mod_shift;     // modulus part of the truncation error held to 2^(tol_log2 - shift) (QLGA_OPT_EXP_MOD_SHIFT)

@@ -180,6 +180,19 @@ __device__ __forceinline__ void sincos_small_m1(T x, const SinCosTable& t, T* s,
 __device__ __forceinline__ void sincos_lib(double x, double* s, double* c) { sincos(x, s, c); }
 __device__ __forceinline__ void sincos_lib(float x, float* s, float* c) { sincosf(x, s, c); }
 
+// element of the state in HBM (storage type S) <-> registers (arithmetic type T)
+template <typename T, typename S>
+__device__ __forceinline__ cx<T> ld_state(const typename vec2<S>::type* p) {
+    const typename vec2<S>::type v = *p;
+    return mk<T>((T)v.x, (T)v.y);
+}
+template <typename T, typename S>
+__device__ __forceinline__ void st_state(typename vec2<S>::type* p, cx<T> z) {
+    typename vec2<S>::type v;
+    v.x = (S)z.re; v.y = (S)z.im;              // round to nearest when S is narrower than T
+    *p = v;
+}
+
 // Site state: q[j][sigma], j = 0..4 <-> m = +2..-2.
 template <typename T> struct Site {
     cx<T> q[5][2];

@@ -44,19 +44,6 @@ struct PassArgs {
     ExpTable tab;
 };
 
-// element of the state in HBM (storage type S) <-> registers (arithmetic type T)
-template <typename T, typename S>
-__device__ __forceinline__ cx<T> ld_state(const typename vec2<S>::type* p) {
-    const typename vec2<S>::type v = *p;
-    return mk<T>((T)v.x, (T)v.y);
-}
-template <typename T, typename S>
-__device__ __forceinline__ void st_state(typename vec2<S>::type* p, cx<T> z) {
-    typename vec2<S>::type v;
-    v.x = (S)z.re; v.y = (S)z.im;              // round to nearest when S is narrower than T
-    *p = v;
-}
-
 __device__ __forceinline__ int64_t pmod(int64_t a, int64_t n) {
     int64_t r = a % n;
     return r < 0 ? r + n : r;

@@ -19,7 +19,7 @@ QLGA_OK, QLGA_EINVAL, QLGA_ENOMEM, QLGA_ECUDA, QLGA_ESTATE, QLGA_EUNSUP = range(
 QLGA_F64, QLGA_F32, QLGA_F32X = 0, 1, 2
 QLGA_PLAIN, QLGA_INTERLEAVED = 0, 1
 (OPT_PATH, OPT_STEPS_PER_LAUNCH, OPT_EXP_TOL_LOG2, OPT_THREADS_X, OPT_TILE_Y, OPT_THREADS_Y, OPT_FUSE_PLAIN_U,
- OPT_F32_PHASE, OPT_EXP_POLY, OPT_EXP_MOD_SHIFT) = range(10)
+ OPT_F32_PHASE, OPT_EXP_POLY, OPT_EXP_MOD_SHIFT, OPT_MARCH) = range(11)
 _PRECISIONS = {"f64": QLGA_F64, "fp64": QLGA_F64, "double": QLGA_F64, "f32": QLGA_F32, "fp32": QLGA_F32,
                "float": QLGA_F32, "f32x": QLGA_F32X}
 

@@ -630,3 +630,28 @@ def test_plain_ordering_trailing_interaction(qlga, oracle):
     q32 = q0.astype(np.complex64)
     assert rel_l2(run_gpu(qlga, q32, 2, c, "plain", 5, precision="f32"),
                   oracle.step(q32.astype(np.complex128), 2, c, 0, 5)) < TOL32
+
+
+def test_marching_pass_is_bit_identical_to_the_tile_kernel(qlga, oracle):
+    # Plain ordering: the interaction-free strided passes run by column marching (QLGA_OPT_MARCH, default on):
+    # the same operations in the same order as the tile kernel, so the states agree bit for bit -- lattices
+    # smaller than the pipeline's run-in, ragged columns, several segments, 3D (y and z passes), every precision.
+    c = (1.0, 0.3, -0.1)
+    cases = [(2, (1, 1)), (2, (3, 2)), (2, (130, 7)), (2, (257, 300)), (2, (64, 2100)), (3, (5, 3, 2)), (3, (33, 40, 9)),
+             (3, (12, 10, 70))]
+    for ndim, dims in cases:
+        q0 = inputs.random_spinor_state(dims, seed=61 + dims[0], amplitude=0.05)
+        for precision in ("f64", "f32", "f32x"):
+            qin = q0 if precision == "f64" else q0.astype(np.complex64)
+            outs = []
+            for march in (1, 0):
+                sim = qlga.Qlga(ndim, dims, c, order="plain", precision=precision)
+                sim.set_option(qlga.OPT_MARCH, march)
+                sim.set_state_q(qin)
+                sim.step(3)
+                outs.append(sim.get_state_q())
+                sim.close()
+            assert np.array_equal(outs[0], outs[1]), (ndim, dims, precision)
+        ref32 = oracle.step(q0.astype(np.complex64).astype(np.complex128), ndim, c, 0, 3)
+        assert rel_l2(outs[0].astype(np.complex128), ref32) < TOL32            # f32x, marching off: the last run
+        assert rel_l2(run_gpu(qlga, q0, ndim, c, "plain", 3), oracle.step(q0, ndim, c, 0, 3)) < TOL64
