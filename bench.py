@@ -63,6 +63,9 @@ def parse_args():
     ap.add_argument("--threads-y", type=int, default=0)
     ap.add_argument("--steps-per-launch", type=int, default=0, help="QLGA_OPT_STEPS_PER_LAUNCH (1D)")
     ap.add_argument("--tol-log2", type=int, default=0, help="QLGA_OPT_EXP_TOL_LOG2 override (experiments only)")
+    ap.add_argument("--no-variants", action="store_true",
+                    help="skip the `variants` record (the other precisions / orderings / config 3, a few bench steps each)")
+    ap.add_argument("--variant-steps", type=int, default=2)
     ap.add_argument("--mod-shift", type=int, default=-1, help="QLGA_OPT_EXP_MOD_SHIFT override (experiments only)")
     ap.add_argument("--slab", action="store_true",
                     help="one lattice cut into slabs along its slowest axis, one slab per GPU, 4-layer halo exchange "
@@ -329,6 +332,65 @@ def build_roofline(qlga, prof, ndim, sites, time_steps, precision, order, deg_in
     return roof
 
 
+# the other precisions / orderings of the headline workload and config 3 (the large 1D lattice), a few bench
+# steps each, so that they are measured by whoever runs bench.py and not only quoted in DESIGN.md
+VARIANTS = (("cfg5", "f32", "interleaved"), ("cfg5", "f32x", "interleaved"), ("cfg5", "f64", "plain"),
+            ("cfg5", "f32", "plain"), ("cfg3", "f64", "interleaved"), ("cfg3", "f32", "interleaved"),
+            ("cfg3", "f64", "plain"), ("cfg3", "f32", "plain"))
+
+
+def run_variant(qlga, torch, dev, local_rank, workload, precision, order, psi_dev, w, steps, lattice):
+    """One variant: `steps` bench steps (same definition of a step as the headline) after 3 warm-up steps,
+    CUDA events on the library's stream, clocks sampled during the timed region, both rooflines."""
+    ndim = WORKLOADS[workload]["ndim"]
+    sites = int(np.prod(w.dims))
+    inner = max(1, min(1000, int(6.0e8 / sites)))
+    sim = qlga.Qlga(ndim, w.dims, w.couplings, order=order, precision=precision, device=dev)
+    cdt = torch.complex128 if precision == "f64" else torch.complex64
+    sim.set_state_psi(psi_dev.to(cdt))
+    omega = (torch.empty((5, sim.ny, sim.nx), dtype=sim.rdtype, device=dev) if ndim == 2 else None)
+
+    def step():
+        sim.step(inner)
+        ob = sim.observables()
+        if omega is not None:
+            sim.vorticity(omega)
+        return ob
+
+    ob0 = sim.observables()
+    for _ in range(3):
+        step()
+    sim.profile_enable(True)
+    sampler = ClockSampler(local_rank)
+    torch.cuda.synchronize()
+    sampler.start()
+    n0 = sim.launch_count()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(steps):
+        ob = step()
+    e1.record()
+    torch.cuda.synchronize()
+    clocks = sampler.stop()
+    ms = e0.elapsed_time(e1)
+    prof = sim.profile_read()
+    deg_info = mean_degree(sim)
+    launches = sim.launch_count() - n0
+    roof = build_roofline(qlga, prof, ndim, sites, inner * steps, precision, order, deg_info, clocks,
+                          load_traffic(workload, precision, order) if not lattice else {})
+    value = sites * inner * steps / (ms * 1e-3) / 1e9
+    out = {"workload": workload, "lattice": list(w.dims), "precision": precision, "order": order, "value": value, "unit": UNIT,
+           "steps": steps, "time_steps_per_bench_step": inner, "ms_per_step": ms / steps, "clocks": clocks,
+           "gpu_launches": launches, "roofline": roof,
+           "hbm_model_frac": value * 1e9 * bytes_per_site_update(precision) / (load_peaks()[0] * 1e9),
+           "kernel_ms": {k: {"ms_total": v[0], "launches": v[1]} for k, v in prof.items() if v[1]},
+           "norm_q_drift": ob["norm_q"] / ob0["norm_q"] - 1.0}
+    sim.close()
+    del sim, omega
+    torch.cuda.empty_cache()
+    return out
+
+
 # ---------------------------------------------------------------------------
 # this repo's arm
 # ---------------------------------------------------------------------------
@@ -515,6 +577,30 @@ def main():
     roof = build_roofline(qlga, prof, ndim, sites, inner * args.steps, args.precision, args.order, deg_info, clocks,
                           load_traffic(args.workload, args.precision, args.order) if not args.lattice else {})
 
+    # ---- variants (rank 0, one GPU): free the headline's buffers first ------------------------------
+    variants = None
+    if world == 1 and not args.no_variants and not args.slab:
+        sim.close()
+        del sim, omega_dev, q_host, out_host
+        torch.cuda.empty_cache()
+        variants = []
+        psi_cache = {}
+        for vw, vp, vo in VARIANTS:
+            if (vw, vp, vo) == (args.workload, args.precision, args.order):
+                continue
+            if vw not in psi_cache:
+                psi_cache.clear()
+                torch.cuda.empty_cache()
+                ww = w if vw == args.workload else WORKLOADS[vw]["gen"](args.lattice if vw == args.workload else 0)
+                psi_cache[vw] = (ww, torch.from_numpy(ww.psi).to(dev))
+            ww, psi_dev = psi_cache[vw]
+            try:
+                variants.append(run_variant(qlga, torch, dev, local_rank, vw, vp, vo, psi_dev, ww, args.variant_steps,
+                                            args.lattice if vw == args.workload else 0))
+            except Exception as exc:                       # a failed variant must not lose the headline line
+                variants.append({"workload": vw, "precision": vp, "order": vo, "error": repr(exc)})
+        psi_cache.clear()
+
     cpu = None
     if world == 1 and not args.no_cpu_baseline:
         rate, sample, _, _ = time_oracle(w, ndim, args.order, args.cpu_seconds)
@@ -524,7 +610,7 @@ def main():
             "warmup": max(3, args.warmup), "ms_per_step": ms / args.steps, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": args.precision, "data": "synthetic",
             "config": config, "clocks": clocks, "e2e": e2e, "e2e_full_state": e2e_q, "gpu_launches": launches,
-            "roofline": roof, "cpu_baseline": cpu,
+            "roofline": roof, "cpu_baseline": cpu, "variants": variants,
             "hbm_model_frac": value / world * 1e9 * bps / (hbm_peak * 1e9),
             "kernel_ms": {k: {"ms_total": v[0], "launches": v[1]} for k, v in prof.items()},
             "pass_kernel_share_of_step": sum(v[0] for v in prof.values()) / ms if ms > 0 else None,

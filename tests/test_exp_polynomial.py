@@ -82,16 +82,16 @@ def test_degree_lookup_table_is_never_below_the_threshold_rule():
         assert above < 0.05 * len(thetas)          # buckets are 4-6 % wide: few angles pay an extra stage
 
 
-@pytest.mark.parametrize("shift", [5, 9])
-def test_modulus_part_of_the_error_is_held_to_its_own_bound(shift):
+@pytest.mark.parametrize("tl,shift", [(-56, 5), (-56, 9), (-58, 7)])          # (-58, 7): the fp64 default
+def test_modulus_part_of_the_error_is_held_to_its_own_bound(tl, shift):
     # QLGA_OPT_EXP_MOD_SHIFT: |P_p(-ix)| - 1 (the error that repeats as a density error at every application)
-    # stays within 2^(-56 - shift) on the interval of every degree, the full error within 2^-56
+    # stays within 2^(tl - shift) on the interval of every degree, the full error within 2^tl
     from paper_1907_12834_b200 import qlga
-    tol, tol_mod = mp.mpf(2) ** -56, mp.mpf(2) ** (-56 - shift)
+    tol, tol_mod = mp.mpf(2) ** tl, mp.mpf(2) ** (tl - shift)
     prev = 0.0
     for p in range(1, 13):
-        theta, b0, r = qlga.exp_polynomial(-56, p, shift)
-        assert theta >= prev and theta <= qlga.exp_polynomial(-56, p, 0)[0]
+        theta, b0, r = qlga.exp_polynomial(tl, p, shift)
+        assert theta >= prev and theta <= qlga.exp_polynomial(tl, p, 0)[0]
         prev = theta
         for i in range(0, 81):
             x = mp.mpf(theta) * (mp.mpf(i) / 40 - 1)
@@ -102,9 +102,9 @@ def test_modulus_part_of_the_error_is_held_to_its_own_bound(shift):
         assert b0 == 1.0
     # small even degrees (nearly) keep the reach of the plain tolerance: their leading error is odd, a phase error
     for p in (2, 4):
-        assert qlga.exp_polynomial(-56, p, shift)[0] >= 0.97 * qlga.exp_polynomial(-56, p, 0)[0]
+        assert qlga.exp_polynomial(tl, p, shift)[0] >= 0.97 * qlga.exp_polynomial(tl, p, 0)[0]
     # the degree lookup follows the shifted thresholds
-    thr = [qlga.exp_polynomial(-56, p, shift)[0] for p in range(1, 13)]
+    thr = [qlga.exp_polynomial(tl, p, shift)[0] for p in range(1, 13)]
     for th in (5.2e-5, 0.0047, 0.015, 0.05):
         rule = 1 + sum(np.float32(th) > np.float32(t) for t in thr)
-        assert rule <= qlga.exp_degree(-56, th, shift) <= rule + 1
+        assert rule <= qlga.exp_degree(tl, th, shift) <= rule + 1
