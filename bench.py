@@ -76,8 +76,8 @@ def parse_args():
 
 def load_traffic(workload, precision, order):
     """{kernel: (dram bytes per launch, FP instr per site per launch)} from the committed ncu
-    capture (profiles/r1_traffic.csv), or {} when this workload was not captured."""
-    path = os.path.join(ROOT, "profiles", "r1_traffic.csv")
+    capture (profiles/r2_traffic.csv), or {} when this workload was not captured."""
+    path = os.path.join(ROOT, "profiles", "r2_traffic.csv")
     out = {}
     if os.path.exists(path):
         import csv
