@@ -655,3 +655,36 @@ def test_marching_pass_is_bit_identical_to_the_tile_kernel(qlga, oracle):
         ref32 = oracle.step(q0.astype(np.complex64).astype(np.complex128), ndim, c, 0, 3)
         assert rel_l2(outs[0].astype(np.complex128), ref32) < TOL32            # f32x, marching off: the last run
         assert rel_l2(run_gpu(qlga, q0, ndim, c, "plain", 3), oracle.step(q0, ndim, c, 0, 3)) < TOL64
+
+
+def test_option_validation_and_the_device_error_word(qlga):
+    # (TILE_Y, THREADS_Y) are validated as a pair (only built kernels), STEPS_PER_LAUNCH against what the kernels support;
+    # a state with a non-finite amplitude does not hang the sub-angle loop: the kernels raise the context's error word
+    # and the next synchronising call reports QLGA_ESTATE (once), after which the context is usable again.
+    c = (1.0, 0.3, -0.1)
+    sim = qlga.Qlga(2, (40, 33), c)
+    sim.set_option(qlga.OPT_TILE_Y, 4)
+    with pytest.raises(qlga.QlgaError) as e:
+        sim.set_option(qlga.OPT_THREADS_Y, 128)                 # 4 columns x 128 threads: no such kernel
+    assert e.value.status == qlga.QLGA_EINVAL
+    sim.set_option(qlga.OPT_THREADS_Y, 256)
+    with pytest.raises(qlga.QlgaError):
+        sim.set_option(qlga.OPT_TILE_Y, 1)                      # 1 x 256: no such kernel either
+    sim.set_option(qlga.OPT_THREADS_Y, 0); sim.set_option(qlga.OPT_TILE_Y, 0)
+    for key, bad in ((qlga.OPT_STEPS_PER_LAUNCH, 16), (qlga.OPT_EXP_MOD_SHIFT, 17), (qlga.OPT_F32_PHASE, 3), (qlga.OPT_MARCH, 2)):
+        with pytest.raises(qlga.QlgaError) as e:
+            sim.set_option(key, bad)
+        assert e.value.status == qlga.QLGA_EINVAL
+    q0 = inputs.random_spinor_state((40, 33), seed=71, amplitude=0.1)
+    for poison in (np.inf, np.nan, 1e200):
+        q = q0.copy()
+        q[2, 0, 5, 7] = poison
+        sim.set_state_q(q)
+        sim.step(1)
+        with pytest.raises(qlga.QlgaError) as e:
+            sim.observables()
+        assert e.value.status == qlga.QLGA_ESTATE and "interaction angle" in str(e.value)
+        sim.set_state_q(q0)                                     # a good state: the word was cleared by the report
+        sim.step(1)
+        assert abs(sim.observables()["norm_q"] / norm2(q0) - 1) < 1e-13
+    sim.close()
