@@ -123,7 +123,9 @@ typedef struct {
  *              passes, so the state of the previous step survives only with a third
  *              buffer; without it e_dt is NaN in 2D and 3D.  Unused in 1D.
  *   buf_bytes  size of each buffer.
- *   cuda_stream  the caller's cudaStream_t (NULL = legacy default stream).
+ *   cuda_stream  the caller's cudaStream_t (NULL = legacy default stream); a stream of the device that holds the buffers.
+ * The context lives on the device its buffers are on (all three on the same one), whatever device is current in the
+ * calling thread: every entry point that takes the context switches to that device and restores the caller's on return.
  * Errors: QLGA_EINVAL (arguments), QLGA_ECUDA (no sm_100 device / CUDA failure), QLGA_ENOMEM. */
 qlga_status qlga_init(qlga_ctx** out, int ndim, const int64_t* dims,
                       double c0, double c1, double c2, qlga_order order, qlga_prec prec,
