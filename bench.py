@@ -616,6 +616,8 @@ def main():
             "pass_kernel_share_of_step": sum(v[0] for v in prof.values()) / ms if ms > 0 else None,
             "norm_q_drift": obs["norm_q"] / obs0["norm_q"] - 1.0,
             "sim_step": obs["step"]}
+    line["issue_peaks"] = {k: {"instr_per_clk_per_sm": v["instr_per_clk_per_sm"], "tinstr_per_s": v["instr_per_s"] / 1e12}
+                           for k, v in _ALU_PEAKS.items()}          # qlga_issue_peak, measured in this run
     if ss is not None:
         halo = 2 * ss.edge_lo.numel() * ss.edge_lo.element_size()
         line["slab"] = {"ghost_layers": 4, "owned_layers": int(w.dims[ndim - 1]),
