@@ -65,8 +65,8 @@ typedef enum {
     QLGA_OPT_PATH = 0,        /* 0 = fused pass kernels (default), 1 = one kernel per operator   */
     QLGA_OPT_STEPS_PER_LAUNCH = 1, /* 1D only: time steps fused per launch (halo 4 per step); 0 = auto, else 1..15,
                                  clamped to what the x pass's CTA size supports ((threads - 8) / 16) */
-    QLGA_OPT_EXP_TOL_LOG2 = 2,/* truncation target of the interaction exponential, log2 (default -58 for fp64
-                                 arithmetic, -27 for QLGA_F32) */
+    QLGA_OPT_EXP_TOL_LOG2 = 2,/* truncation target of the interaction exponential, log2 (default -58 for QLGA_F64,
+                                 -44 for QLGA_F32X, -27 for QLGA_F32) */
     QLGA_OPT_THREADS_X = 3,   /* CTA size of the x pass: 64, 96, 128, 192 or 256; 0 = auto       */
     QLGA_OPT_TILE_Y = 4,      /* strided (y, z) passes: columns per CTA (1,2,4,8); 0 = auto      */
     QLGA_OPT_THREADS_Y = 5,   /* CTA size of the strided passes; 0 = auto.  TILE_Y and THREADS_Y are validated as a
@@ -87,7 +87,7 @@ typedef enum {
     QLGA_OPT_EXP_MOD_SHIFT = 9 /* the MODULUS part of the truncation error (the even part of the polynomial) is held to
                                  2^(tol_log2 - shift): a modulus error that repeats at every application changes the
                                  density and with it the phase rate c0 rho, and grows like applications x (c0 rho t / 2)
-                                 (DESIGN.md section 8).  0..16; default 7 for fp64 arithmetic (QLGA_F64, QLGA_F32X),
+                                 (DESIGN.md section 8).  0..16; default 7 for QLGA_F64 (modulus part 2^-65), 8 for QLGA_F32X (2^-52),
                                  0 for QLGA_F32 */
 } qlga_option;
 
