@@ -232,6 +232,12 @@ __device__ __forceinline__ void kin_update(Site<T>& s, int sigma, const cx<T> Fw
 //   g0 = s c0, g1 = s c1, g2 = s c2 / 5.
 // thr[p-1] = largest angle for which a degree-p polynomial meets the tolerance.
 // ---------------------------------------------------------------------------
+#ifndef QLGA_FUSED_STAGES
+#define QLGA_FUSED_STAGES 1      // inner Horner stages of the gauge path in one sweep (horner_stage_fused)
+#endif
+#ifndef QLGA_FUSED_LAST
+#define QLGA_FUSED_LAST 0        // 1: the last stage (k = 1) too (five or six roundings at full magnitude instead of one)
+#endif
 constexpr int QLGA_PMAX = 12;
 constexpr int QLGA_LUT_BASE = 83 * 16;      // theta = 2^-44: below it degree 1 serves every tolerance in use
 constexpr int QLGA_LUT_N = 44 * 16;         // up to theta = 1 (theta_split <= 1/2 ends the table's use)
@@ -439,6 +445,36 @@ __device__ __forceinline__ void gauge_phases(const KCoef<T>& kc, cx<T> ph, cx<T>
     }
 }
 
+// One inner Horner stage in one sweep (spin gauge, real off-diagonal coefficients):
+//     out_j = v_j - i kap (sK' u)_j
+// accumulated term by term onto v_j with the coefficients pre-multiplied by kap: -i c u = (c u.im, -c u.re) is one FMA pair
+// per term, the rank-one amplitude is rotated once (tk = -i kap g2 <chi'|u>), and the separate update v - i kap w of the
+// plain form disappears: 73 instead of 78 FP64 instructions per stage and vector.  Every term is rounded at the
+// magnitude of v here (five or six roundings per component instead of one), which is harmless in an INNER stage -- its
+// result is multiplied by the angle in the next one -- so the last stage (k = 1) keeps the plain form.
+template <typename T>
+__device__ __forceinline__ void horner_stage_fused(cx<T> u[5], const cx<T> v[5], T kap, const KCoef<T>& kc) {
+    const T az = kap * kc.az, az2 = kap * kc.az2, a1 = kap * kc.a1, a6 = kap * kc.a6, g2 = kap * kc.g2;
+    const cx<T>* psi = kc.psi;
+    cx<T> t = cmul(psi[4], u[0]);
+    t = cfma(psi[2], u[2], t);
+    t = cfma(psi[0], u[4], t);
+    cx<T> t2 = cmul(psi[3], u[1]);
+    t2 = cfma(psi[1], u[3], t2);
+    t = t - t2;
+    const cx<T> tk = mk<T>(g2 * t.im, -(g2 * t.re));                 // -i kap g2 <chi'|u>
+    const cx<T> r0 = axmi(a1, u[1], axmi(az2, u[0], v[0]));
+    const cx<T> r1 = axmi(a6, u[2], axmi(a1, u[0], axmi(az, u[1], v[1])));
+    const cx<T> r2 = axmi(a6, u[3], axmi(a6, u[1], v[2]));
+    const cx<T> r3 = axmi(a1, u[4], axmi(a6, u[2], axmi(-az, u[3], v[3])));
+    const cx<T> r4 = axmi(a1, u[3], axmi(-az2, u[4], v[4]));
+    u[0] = cfma_conj(psi[4], tk, r0);
+    u[1] = cfnma_conj(psi[3], tk, r1);
+    u[2] = cfma_conj(psi[2], tk, r2);
+    u[3] = cfnma_conj(psi[1], tk, r3);
+    u[4] = cfma_conj(psi[0], tk, r4);
+}
+
 // u <- P_p(-i sK') v in Horner form u_{k-1} = v + r_k (-i sK') u_k, k = p..1, u_p = v
 // (stage p acts on v itself: no copy).  psi, hence K, is frozen (reading R4).
 template <typename T>
@@ -451,12 +487,29 @@ __device__ __forceinline__ void horner(const cx<T> v[5], cx<T> u[5], const KCoef
 #pragma unroll
         for (int j = 0; j < 5; ++j) u[j] = axmi(ik, w[j], v[j]);
     }
+    if constexpr (SpinGauge<T>::on && QLGA_FUSED_STAGES) {
+        // stages p-1 .. 2 in one sweep each; the last one in the plain form (see horner_stage_fused).  (Measured at
+        // config 5: 1.525 -> 1.549 GSUP/s; the first stage fused as well, which costs a copy of v: 1.524; the last
+        // one too: 1.554 for 1.3x the rounding error after 20 000 steps: not taken.)
+        if (p >= 2) {
+            constexpr int last_plain = QLGA_FUSED_LAST ? 0 : 1;
 #pragma unroll 1
-    for (int k = p - 1; k >= 1; --k) {
-        apply_sK(u, w, kc.az, kc.az2, kc.a1, kc.a6, kc.g2, kc.psi);
-        const T ik = r[k];
+            for (int k = p - 1; k > last_plain; --k) horner_stage_fused<T>(u, v, r[k], kc);
+            if (!QLGA_FUSED_LAST) {
+                apply_sK(u, w, kc.az, kc.az2, kc.a1, kc.a6, kc.g2, kc.psi);
+                const T ik = r[1];
 #pragma unroll
-        for (int j = 0; j < 5; ++j) u[j] = axmi(ik, w[j], v[j]);
+                for (int j = 0; j < 5; ++j) u[j] = axmi(ik, w[j], v[j]);
+            }
+        }
+    } else {
+#pragma unroll 1
+        for (int k = p - 1; k >= 1; --k) {
+            apply_sK(u, w, kc.az, kc.az2, kc.a1, kc.a6, kc.g2, kc.psi);
+            const T ik = r[k];
+#pragma unroll
+            for (int j = 0; j < 5; ++j) u[j] = axmi(ik, w[j], v[j]);
+        }
     }
 }
 
@@ -572,12 +625,26 @@ __device__ __forceinline__ void interaction(Site<T>& s, const UConst<T>& uc, con
         const T ik = r[p];
 #pragma unroll
         for (int j = 0; j < 5; ++j) u[j] = axmi(ik, wa[j], va[j]);
+        if constexpr (SpinGauge<T>::on && QLGA_FUSED_STAGES) {
+            if (p >= 2) {
+                constexpr int last_plain = QLGA_FUSED_LAST ? 0 : 1;
 #pragma unroll 1
-        for (int k = p - 1; k >= 1; --k) {
-            apply_sK(u, wa, kc.az, kc.az2, kc.a1, kc.a6, kc.g2, kc.psi);
-            const T ikk = r[k];
+                for (int k = p - 1; k > last_plain; --k) horner_stage_fused<T>(u, va, r[k], kc);
+                if (!QLGA_FUSED_LAST) {
+                    apply_sK(u, wa, kc.az, kc.az2, kc.a1, kc.a6, kc.g2, kc.psi);
+                    const T ikk = r[1];
 #pragma unroll
-            for (int j = 0; j < 5; ++j) u[j] = axmi(ikk, wa[j], va[j]);
+                    for (int j = 0; j < 5; ++j) u[j] = axmi(ikk, wa[j], va[j]);
+                }
+            }
+        } else {
+#pragma unroll 1
+            for (int k = p - 1; k >= 1; --k) {
+                apply_sK(u, wa, kc.az, kc.az2, kc.a1, kc.a6, kc.g2, kc.psi);
+                const T ikk = r[k];
+#pragma unroll
+                for (int j = 0; j < 5; ++j) u[j] = axmi(ikk, wa[j], va[j]);
+            }
         }
         if (one_plus_d) {
 #pragma unroll
