@@ -336,7 +336,8 @@ def build_roofline(qlga, prof, ndim, sites, time_steps, precision, order, deg_in
 # steps each, so that they are measured by whoever runs bench.py and not only quoted in DESIGN.md
 VARIANTS = (("cfg5", "f32", "interleaved"), ("cfg5", "f32x", "interleaved"), ("cfg5", "f64", "plain"),
             ("cfg5", "f32", "plain"), ("cfg3", "f64", "interleaved"), ("cfg3", "f32", "interleaved"),
-            ("cfg3", "f64", "plain"), ("cfg3", "f32", "plain"))
+            ("cfg3", "f64", "plain"), ("cfg3", "f32", "plain"),
+            ("cfg4", "f64", "interleaved"), ("cfg2", "f64", "interleaved"), ("cfg1", "f64", "interleaved"))
 
 
 def run_variant(qlga, torch, dev, local_rank, workload, precision, order, psi_dev, w, steps, lattice):

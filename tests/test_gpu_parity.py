@@ -688,3 +688,32 @@ def test_option_validation_and_the_device_error_word(qlga):
         sim.step(1)
         assert abs(sim.observables()["norm_q"] / norm2(q0) - 1) < 1e-13
     sim.close()
+
+
+def test_angle_stats_match_the_definition(qlga):
+    # qlga_angle_stats (diagnostic): theta = s (2|c1||F| + |c2| rho / 5), phase = |s c0 rho| per site of one application of U,
+    # and the histogram of the degrees the kernels' lookup assigns to them
+    c = (0.9, -0.35, 0.6)
+    q0 = inputs.random_spinor_state((64, 48), seed=81, amplitude=0.2)
+    psi = q0[:, 0] + q0[:, 1]
+    n = np.abs(psi) ** 2
+    rho = n.sum(0)
+    fz = 2 * (n[0] - n[4]) + n[1] - n[3]
+    fp = 2 * (np.conj(psi[0]) * psi[1] + np.conj(psi[3]) * psi[4]) + np.sqrt(6.0) * (np.conj(psi[1]) * psi[2] + np.conj(psi[2]) * psi[3])
+    fabs = np.sqrt(fz ** 2 + np.abs(fp) ** 2)
+    for order, s in (("interleaved", 1 / 8), ("plain", 1.0)):
+        sim = qlga.Qlga(2, (64, 48), c, order=order)
+        sim.set_state_q(q0)
+        st = sim.angle_stats()
+        theta = s * (2 * abs(c[1]) * fabs + abs(c[2]) / 5 * rho)
+        assert st["theta_max"] == pytest.approx(theta.max(), rel=1e-6)
+        assert st["theta_mean"] == pytest.approx(theta.mean(), rel=1e-10)
+        assert st["phase_max"] == pytest.approx((s * abs(c[0]) * rho).max(), rel=1e-6)
+        hist = st["degree_hist"]
+        assert sum(hist) == 64 * 48
+        split = min(qlga.exp_polynomial(-58, 12, 7)[0], 0.5)
+        want = np.zeros(13, dtype=np.int64)
+        for th in theta.ravel():
+            want[0 if np.float32(th) > np.float32(split) else qlga.exp_degree(-58, float(np.float32(th) * np.float32(1.0009765625)), 7)] += 1
+        assert np.abs(np.array(hist) - want).sum() <= 4            # sites on a bucket edge may land on either side (fp32 angle)
+        sim.close()
