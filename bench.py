@@ -67,6 +67,17 @@ def parse_args():
                     help="skip the `variants` record (the other precisions / orderings / config 3, a few bench steps each)")
     ap.add_argument("--variant-steps", type=int, default=2)
     ap.add_argument("--mod-shift", type=int, default=-1, help="QLGA_OPT_EXP_MOD_SHIFT override (experiments only)")
+    ap.add_argument("--band", type=int, default=-1, choices=[-1, 0, 1, 2],
+                    help="QLGA_OPT_BAND (plain ordering, 2D): -1 = the library's default (band pipelining through L2 where it "
+                         "pays), 0 = two launches per step, 1 = bands on the library's streams, 2 = replayed as a CUDA graph")
+    ap.add_argument("--band-rows", type=int, default=0, help="QLGA_OPT_BAND_ROWS (0 = auto)")
+    ap.add_argument("--band-slots", type=int, default=0, help="QLGA_OPT_BAND_SLOTS (0 = auto)")
+    ap.add_argument("--band-trace", action="store_true",
+                    help="band mode, library built with QLGA_NVCC_EXTRA=-DQLGA_TRACE: add the timeline of one band step "
+                         "(first CTA start / last CTA end of every y and x kernel, %%globaltimer) to the JSON line")
+    ap.add_argument("--profiler-range", action="store_true",
+                    help="bracket the timed region with cudaProfilerStart / Stop (for `ncu --replay-mode app-range`, "
+                         "which measures the DRAM traffic of the whole region with its kernels running side by side)")
     ap.add_argument("--slab", action="store_true",
                     help="one lattice cut into slabs along its slowest axis, one slab per GPU, 4-layer halo exchange "
                          "per step (paper_1907_12834_b200/slab.py); weak scaling: every rank owns the workload's lattice "
@@ -305,6 +316,8 @@ def build_roofline(qlga, prof, ndim, sites, time_steps, precision, order, deg_in
     # a pass launch advances every site by 1/ndim of a time step (times the fused steps in 1D)
     per_step = 1 if dom == "x_pass" else max(1, ndim - 1)    # the y_pass timer covers the y and z passes
     units = sites * time_steps * per_step / (ndim * dn)       # site-updates per launch
+    if dom == "band_step":                                    # band mode: one graph replay = one whole time step
+        units = float(sites)
     deg, stats = deg_info
     arith = "f64" if precision in ("f64", "f32x") else "f32"
     fpi = fp_instr_per_site_update(ndim, order, deg, arith)
@@ -332,10 +345,55 @@ def build_roofline(qlga, prof, ndim, sites, time_steps, precision, order, deg_in
     return roof
 
 
+def default_inner(sites, order):
+    """Time steps per bench step: about 0.5 s of GPU work for the interleaved ordering; four times as many steps for the
+    plain ordering, whose steps are four times cheaper (and whose first step of every qlga_step call cannot take the band
+    pipeline: its U has not been applied by a previous step)."""
+    inner = max(1, min(1000, int(6.0e8 / sites)))
+    return min(1000, 4 * inner) if order == "plain" else inner
+
+
+def band_timeline(qlga, sim, torch):
+    """Timeline of one band step with the trailing U (QLGA_OPT_BAND; debug build of the library with -DQLGA_TRACE):
+    per band the first CTA start and last CTA end of its y kernel and its x kernel, microseconds from the first."""
+    import ctypes
+    lib = qlga._lib
+    if not hasattr(lib, "qlga_debug_trace"):
+        return {"error": "libqlga.so was not built with -DQLGA_TRACE"}
+    buf = (ctypes.c_ulonglong * (2 * 8192))()
+    torch.cuda.synchronize()
+    lib.qlga_debug_trace(buf, 1)
+    sim.step(3)                     # two-launch step, band step with the trailing U (graph 0), last band step
+    torch.cuda.synchronize()
+    lib.qlga_debug_trace(buf, 0)
+    full = np.array(buf, dtype=np.uint64).reshape(-1, 2).astype(np.int64)
+    # graph n of the context traces into ids [2048 n, 2048 n + 2 bands): take the first region that was written
+    # (the band step with the trailing U is the first of the three steps)
+    a = None
+    for base in range(0, 8192, 2048):
+        reg = full[base:base + 2048]
+        if (reg[:, 1] > 0).sum() >= 16:
+            if a is None or reg[reg[:, 1] > 0, 0].min() < a[a[:, 1] > 0, 0].min():
+                a = reg
+    if a is None:
+        return {"error": "no band step traced"}
+    nb = int((a[:, 1] > 0).sum()) // 2
+    t0 = a[:2 * nb, 0].min()
+    y0, y1, x0, x1 = ((a[0:2 * nb:2, 0] - t0) / 1e3, (a[0:2 * nb:2, 1] - t0) / 1e3,
+                      (a[1:2 * nb:2, 0] - t0) / 1e3, (a[1:2 * nb:2, 1] - t0) / 1e3)
+    mid = slice(nb // 4, 3 * nb // 4)
+    return {"bands": nb, "step_us": float(x1.max()), "period_us": float(np.diff(x0[mid]).mean()),
+            "y_kernel_us": float((y1 - y0)[mid].mean()), "x_kernel_us": float((x1 - x0)[mid].mean()),
+            "x_overlap_with_next_x_us": float((x1[mid][:-1] - x0[mid][1:]).mean()),
+            "sample": [[round(float(v), 1) for v in (y0[k], y1[k], x0[k], x1[k])] for k in range(nb // 2, nb // 2 + 6)],
+            "columns": "y_start, y_end, x_start, x_end (us) of six consecutive bands"}
+
+
 # the other precisions / orderings of the headline workload and config 3 (the large 1D lattice), a few bench
 # steps each, so that they are measured by whoever runs bench.py and not only quoted in DESIGN.md
 VARIANTS = (("cfg5", "f32", "interleaved"), ("cfg5", "f32x", "interleaved"), ("cfg5", "f64", "plain"),
-            ("cfg5", "f32", "plain"), ("cfg3", "f64", "interleaved"), ("cfg3", "f32", "interleaved"),
+            ("cfg5", "f32", "plain"), ("cfg5", "f64", "plain+two-launch"), ("cfg5", "f32", "plain+two-launch"),
+            ("cfg3", "f64", "interleaved"), ("cfg3", "f32", "interleaved"),
             ("cfg3", "f64", "plain"), ("cfg3", "f32", "plain"),
             ("cfg4", "f64", "interleaved"), ("cfg2", "f64", "interleaved"), ("cfg1", "f64", "interleaved"))
 
@@ -345,8 +403,12 @@ def run_variant(qlga, torch, dev, local_rank, workload, precision, order, psi_de
     CUDA events on the library's stream, clocks sampled during the timed region, both rooflines."""
     ndim = WORKLOADS[workload]["ndim"]
     sites = int(np.prod(w.dims))
-    inner = max(1, min(1000, int(6.0e8 / sites)))
+    inner = default_inner(sites, order.split("+")[0])
+    two_launch = order.endswith("+two-launch")     # plain ordering with band mode off (QLGA_OPT_BAND = 0): the comparison
+    tag, order = order, order.split("+")[0]
     sim = qlga.Qlga(ndim, w.dims, w.couplings, order=order, precision=precision, device=dev)
+    if two_launch:
+        sim.set_option(qlga.OPT_BAND, 0)
     cdt = torch.complex128 if precision == "f64" else torch.complex64
     sim.set_state_psi(psi_dev.to(cdt))
     omega = (torch.empty((5, sim.ny, sim.nx), dtype=sim.rdtype, device=dev) if ndim == 2 else None)
@@ -380,7 +442,7 @@ def run_variant(qlga, torch, dev, local_rank, workload, precision, order, psi_de
     roof = build_roofline(qlga, prof, ndim, sites, inner * steps, precision, order, deg_info, clocks,
                           load_traffic(workload, precision, order) if not lattice else {})
     value = sites * inner * steps / (ms * 1e-3) / 1e9
-    out = {"workload": workload, "lattice": list(w.dims), "precision": precision, "order": order, "value": value, "unit": UNIT,
+    out = {"workload": workload, "lattice": list(w.dims), "precision": precision, "order": tag, "value": value, "unit": UNIT,
            "steps": steps, "time_steps_per_bench_step": inner, "ms_per_step": ms / steps, "clocks": clocks,
            "gpu_launches": launches, "roofline": roof,
            "hbm_model_frac": value * 1e9 * bytes_per_site_update(precision) / (load_peaks()[0] * 1e9),
@@ -411,7 +473,7 @@ def main():
     lat = tuple(reversed(w.dims)) if ndim == 3 else (ny, nx)        # array shape of one plane
     cfg_tag = (f"BASELINE.json configs[{int(args.workload[3]) - 1}]" if args.workload[3:].isdigit()
                else "SURVEY.md 8(f) row 3, not a BASELINE.json config")
-    inner = args.inner or max(1, min(1000, int(6.0e8 / sites)))   # ~0.5 s of GPU work per bench step
+    inner = args.inner or default_inner(sites, args.order)
     config = {"workload": f"{w.name} ({cfg_tag}): "
                           f"{ndim}D periodic {'x'.join(str(v) for v in w.dims[:max(2, ndim)])}, {args.precision}, "
                           f"{args.order} ordering (eq. {'112' if args.order == 'interleaved' else '108'})",
@@ -480,6 +542,11 @@ def main():
         sim.set_option(qlga.OPT_EXP_TOL_LOG2, args.tol_log2)
     if args.mod_shift >= 0:
         sim.set_option(qlga.OPT_EXP_MOD_SHIFT, args.mod_shift)
+    if args.band >= 0 or args.band_rows or args.band_slots:
+        sim.set_option(qlga.OPT_BAND, args.band)
+        sim.set_option(qlga.OPT_BAND_ROWS, args.band_rows)
+        sim.set_option(qlga.OPT_BAND_SLOTS, args.band_slots)
+        config["band"] = {"mode": args.band, "rows": args.band_rows, "slots": args.band_slots}
     omega_dev = (torch.empty((5, sim.ny, nx), dtype=torch.float64 if args.precision == "f64" else torch.float32,
                              device=dev) if ndim == 2 else None)
     state_bytes = q_host.numel() * q_host.element_size()
@@ -506,11 +573,15 @@ def main():
     sampler.start()
     launches0 = sim.launch_count()
     ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    if args.profiler_range:
+        torch.cuda.profiler.start()
     ev0.record()
     for _ in range(args.steps):
         obs = hot_path_step()
     ev1.record()
     barrier()
+    if args.profiler_range:
+        torch.cuda.profiler.stop()
     clocks = sampler.stop()
     launches = sim.launch_count() - launches0
     ms = ev0.elapsed_time(ev1)
@@ -519,6 +590,7 @@ def main():
     deg_info = mean_degree(sim)
     ms = max_over_ranks(ms, world, dev)
     value = aggregate_gsups(sites, inner * args.steps, world, ms)
+    band_trace = band_timeline(qlga, sim, torch) if args.band_trace else None
 
     # ---- end to end through the C ABI with host buffers ---------------------------------
     # The user-facing call: upload the five wavefunctions psi_m (the paper's initial condition, split as
@@ -617,6 +689,8 @@ def main():
             "pass_kernel_share_of_step": sum(v[0] for v in prof.values()) / ms if ms > 0 else None,
             "norm_q_drift": obs["norm_q"] / obs0["norm_q"] - 1.0,
             "sim_step": obs["step"]}
+    if band_trace is not None:
+        line["band_trace"] = band_trace
     line["issue_peaks"] = {k: {"instr_per_clk_per_sm": v["instr_per_clk_per_sm"], "tinstr_per_s": v["instr_per_s"] / 1e12}
                            for k, v in _ALU_PEAKS.items()}          # qlga_issue_peak, measured in this run
     if ss is not None:

@@ -84,6 +84,28 @@ typedef enum {
                                  marching, one thread per (column, m_f), the four factors as a register pipeline, no
                                  shared memory (bit-identical results); 0 = the tile kernel.  Setting TILE_Y or
                                  THREADS_Y also selects the tile kernel */
+    QLGA_OPT_BAND = 11,       /* plain ordering in 2D: ONE HBM round trip per time step by band pipelining.  The lattice is
+                                 cut into bands of rows; the interaction-free y pass (marching kernel) of band k writes
+                                 into a small ring buffer owned by the library that stays resident in the 126 MB L2, the
+                                 x pass (with the next step's U) of band k reads it from there and writes the new state;
+                                 the y pass of band k+1 runs beside the x pass of band k (the library's own streams,
+                                 ordered by events).  Same kernels, same arithmetic: results are bit-identical to the
+                                 two-launch step.  0 = off (a y-pass launch and an x-pass launch per step: two round
+                                 trips), 1 = bands issued directly on the library's streams (host-bound; debugging), 2 =
+                                 the band schedule of a step instantiated once as a CUDA graph and replayed with one
+                                 cudaGraphLaunch on the caller's stream, -1 (default) = 2 where it pays: a band's x kernel
+                                 still fills the GPU (rows per band x tiles per row >= 888) and the state is larger than
+                                 256 MB.  Band mode applies to: 2D, QLGA_PLAIN, fused path, marching pass on, at least four
+                                 bands, and every step of a qlga_step call whose U was applied by the step before it, i.e.
+                                 all but the first and, with a third buffer, the last -- step in calls of many steps.
+                                 Side effects of band mode: the library allocates the ring (slots x rows x Nx x 10 planes,
+                                 63 MB at the defaults), creates four streams of its own, and raises the device's
+                                 persisting-L2 set-aside (cudaLimitPersistingL2CacheSize, a per-device limit that stays
+                                 raised) to the ring's size: the ring's lines are marked persisting so that the y pass's
+                                 output is never written back to DRAM.  The first band step of a context allocates and
+                                 captures (not to be called while the caller's stream is itself being captured) */
+    QLGA_OPT_BAND_ROWS = 12,  /* rows per band; 0 = auto (about 20 MB per band) */
+    QLGA_OPT_BAND_SLOTS = 13, /* bands the ring holds: 2..8; 0 = auto (3) */
     QLGA_OPT_EXP_MOD_SHIFT = 9 /* the MODULUS part of the truncation error (the even part of the polynomial) is held to
                                  2^(tol_log2 - shift): a modulus error that repeats at every application changes the
                                  density and with it the phase rate c0 rho, and grows like applications x (c0 rho t / 2)
@@ -248,9 +270,10 @@ qlga_status qlga_observables_from_sums(const qlga_ctx*, const double* host_sums,
  * While enabled, qlga_step records a CUDA event on the caller's stream before every
  * pass kernel and one after the last; qlga_profile_read synchronises the stream,
  * returns the summed durations and launch counts per kernel kind since the last
- * read (0: x pass, 1: y pass, 2: per-operator kernels) and resets them.  At most
+ * read (0: x pass, 1: y pass, 2: per-operator kernels, 3: whole time steps in band mode,
+ * QLGA_OPT_BAND, where the two passes run beside each other) and resets them.  At most
  * 4096 launches are recorded between two reads; later ones are not timed. */
-typedef struct { double ms[3]; int64_t launches[3]; } qlga_profile;
+typedef struct { double ms[4]; int64_t launches[4]; } qlga_profile;
 qlga_status qlga_profile_enable(qlga_ctx*, int on);
 qlga_status qlga_profile_read(qlga_ctx*, qlga_profile* host_out);
 

@@ -77,6 +77,9 @@ struct DeviceGuard {
     DeviceGuard& operator=(const DeviceGuard&) = delete;
 };
 
+static void band_drop_graphs(qlga_ctx* c);
+static void band_release(qlga_ctx* c);
+
 // ---------------------------------------------------------------------------
 // The interaction polynomial.  exp(-i s K) v is evaluated as P_p(-i s K) v with P_p a
 // degree-p polynomial with real coefficients b_j close to 1/j!.  A plain Taylor
@@ -314,6 +317,7 @@ extern "C" qlga_status qlga_init(qlga_ctx** out, int ndim, const int64_t* dims,
     c->stream = (cudaStream_t)cuda_stream;
     c->cur = 0; c->prev = -1; c->have_state = 0; c->step = 0; c->launches = 0;
     c->path = 0; c->steps_per_launch = 0; c->threads_x = 0; c->tile_y = 0; c->fuse_plain_u = 1; c->march = 1;
+    c->band = -1; c->band_rows = 0; c->band_slots = 0;
     c->tol_log2 = (prec == QLGA_F32) ? F32_TOL_LOG2 : (prec == QLGA_F32X ? F32X_TOL_LOG2 : F64_TOL_LOG2);
     c->exp_poly = (prec == QLGA_F32) ? F32_EXP_POLY : 0;
     c->f32_phase = F32_PHASE_MODE;
@@ -340,6 +344,7 @@ extern "C" qlga_status qlga_destroy(qlga_ctx* c) {
     DeviceGuard guard(c);
     cudaStreamSynchronize(c->stream);
     cudaFree(c->d_partials); cudaFree(c->d_sums); cudaFree(c->d_stage); cudaFree(c->d_scratch); cudaFree(c->d_flag);
+    band_release(c);
     if (c->prof_ev) {
         for (int k = 0; k < PROF_CAP; ++k) cudaEventDestroy(c->prof_ev[k]);
         free(c->prof_ev); free(c->prof_kind);
@@ -353,6 +358,10 @@ extern "C" int64_t qlga_launch_count(const qlga_ctx* c) { return c ? c->launches
 
 extern "C" qlga_status qlga_set_option(qlga_ctx* c, qlga_option key, int64_t v) {
     if (!c) return QLGA_EINVAL;
+    {   // the instantiated band graphs hold kernel arguments (tables, tile choices): drop them on any change
+        DeviceGuard guard(c);
+        band_drop_graphs(c);
+    }
     switch ((int)key) {
         case QLGA_OPT_PATH:
             if (v != 0 && v != 1) return fail(c, QLGA_EINVAL, "QLGA_OPT_PATH: 0 or 1");
@@ -390,6 +399,15 @@ extern "C" qlga_status qlga_set_option(qlga_ctx* c, qlga_option key, int64_t v) 
         case QLGA_OPT_FUSE_PLAIN_U:
             if (v != 0 && v != 1) return fail(c, QLGA_EINVAL, "QLGA_OPT_FUSE_PLAIN_U: 0 or 1");
             c->fuse_plain_u = (int)v; return QLGA_OK;
+        case QLGA_OPT_BAND:
+            if (v < -1 || v > 2) return fail(c, QLGA_EINVAL, "QLGA_OPT_BAND: -1 (auto), 0, 1 or 2");
+            c->band = (int)v; return QLGA_OK;
+        case QLGA_OPT_BAND_ROWS:
+            if (v < 0 || v > 4096) return fail(c, QLGA_EINVAL, "QLGA_OPT_BAND_ROWS: 0 (auto) or 1..4096");
+            c->band_rows = (int)v; return QLGA_OK;
+        case QLGA_OPT_BAND_SLOTS:
+            if (v != 0 && (v < 2 || v > 8)) return fail(c, QLGA_EINVAL, "QLGA_OPT_BAND_SLOTS: 0 (auto) or 2..8");
+            c->band_slots = (int)v; return QLGA_OK;
     }
     return fail(c, QLGA_EINVAL, "qlga_set_option: unknown key");
 }
@@ -574,6 +592,235 @@ static int pick_other(const qlga_ctx* c, int a, int b) {   // a buffer index dif
     return -1;
 }
 
+// ---------------------------------------------------------------------------
+// Band mode: one HBM round trip per 2D time step of the plain ordering (QLGA_OPT_BAND).
+//
+// eq. (108) in 2D is  X Y U  (X, Y = the four kinetic factors of a direction).  With the U of step t+1 riding on
+// the end of step t's x pass, a step is [Y: marching kernel, no interaction] then [X + U: tile kernel], and Y acts
+// along columns only: rows [r0, r1) of Y's output depend on rows [r0 - 4, r1 + 4) of its input and on nothing
+// else.  So the lattice is cut into bands of B rows; band k's y pass writes into slot k mod S of a ring of S
+// bands, band k's x pass reads that slot and writes rows of the new state.  The ring (S x B rows x 10 planes:
+// about 60 MB at the defaults) is rewritten every S bands and stays resident in the 126 MB L2: the state is read
+// from HBM once (by the y pass) and written once (by the x pass).  The y pass of band k+1 runs beside the x pass
+// of band k (FP-bound), on the library's own streams ordered by events:
+//     y_k  after x_{k-S} (its slot is free again);   x_k  after y_k;   x_k and x_{k+1} on alternating streams so
+//     that one fills the SMs the other's last wave leaves idle.
+// The schedule of one step is captured once into a CUDA graph per (source, destination, trailing U) and replayed.
+// The kernels and their arithmetic are the two-launch path's: the results are bit-identical.
+// ---------------------------------------------------------------------------
+#ifdef QLGA_TRACE
+static __device__ unsigned long long g_trace[2 * 8192];
+extern "C" int qlga_debug_trace(unsigned long long* host_out, int reset) {
+    if (reset) {
+        static unsigned long long init[2 * 8192];
+        for (int k = 0; k < 8192; ++k) { init[2 * k] = ~0ull; init[2 * k + 1] = 0; }
+        return (int)cudaMemcpyToSymbol(g_trace, init, sizeof(init));
+    }
+    cudaDeviceSynchronize();
+    return (int)cudaMemcpyFromSymbol(host_out, g_trace, sizeof(g_trace));
+}
+#endif
+static int64_t band_rows_eff(const qlga_ctx* c) {
+    if (c->band_rows > 0) return c->band_rows;
+    const int64_t row_bytes = c->nx * 10 * 2 * (int64_t)real_size(c->prec);
+    int64_t b = ((int64_t)20 << 20) / row_bytes;
+    b -= b % 8;
+    if (b < 8) b = 8;
+    if (b > 256) b = 256;
+    return b;
+}
+static int band_slots_eff(const qlga_ctx* c) { return c->band_slots > 0 ? c->band_slots : 3; }
+
+static bool band_applies(const qlga_ctx* c) {
+    if (c->band == 0 || c->ndim != 2 || c->order != QLGA_PLAIN || c->path != 0) return false;
+    if (!c->march || c->tile_y != 0 || c->threads_y != 0 || !c->fuse_plain_u) return false;
+    const int64_t B = band_rows_eff(c);
+    if (c->ny < 4 * B) return false;
+    if (c->band < 0) {
+        // auto: only where a band's x kernel still fills the GPU (two waves of 128-thread CTAs at three per SM on 148
+        // SMs; a narrow lattice would run 512 small kernels below their occupancy) and the state does not fit in L2 anyway
+        const int threads = c->threads_x ? c->threads_x : 128;
+        const int64_t tiles = (c->nx + threads - 9) / (threads - 8);
+        if (B * tiles < 888) return false;
+        if ((size_t)c->nx * c->ny * 10 * 2 * real_size(c->prec) < ((size_t)256 << 20)) return false;
+    }
+    return true;
+}
+
+static void band_drop_graphs(qlga_ctx* c) {
+    for (int k = 0; k < c->band_ngraph; ++k) cudaGraphExecDestroy(c->band_graph[k].exec);
+    c->band_ngraph = 0;
+}
+
+static void band_release(qlga_ctx* c) {
+    band_drop_graphs(c);
+    for (int k = 0; k < 4; ++k) if (c->band_stream[k]) { cudaStreamDestroy(c->band_stream[k]); c->band_stream[k] = nullptr; }
+    if (c->band_ev) {
+        for (int k = 0; k < c->band_nev; ++k) cudaEventDestroy(c->band_ev[k]);
+        free(c->band_ev); c->band_ev = nullptr; c->band_nev = 0;
+    }
+    cudaFree(c->d_band); c->d_band = nullptr; c->band_bytes = 0;
+}
+
+static qlga_status band_setup(qlga_ctx* c, int64_t B, int S, int64_t nb) {
+    if (!c->band_stream[0]) {
+        int lo = 0, hi = 0;
+        CU(c, cudaDeviceGetStreamPriorityRange(&lo, &hi));
+        // the y pass is short and feeds the x pass: highest priority, so that its CTAs take the first free slots
+        CU(c, cudaStreamCreateWithPriority(&c->band_stream[0], cudaStreamNonBlocking, lo));
+        CU(c, cudaStreamCreateWithPriority(&c->band_stream[1], cudaStreamNonBlocking, hi));
+        CU(c, cudaStreamCreateWithPriority(&c->band_stream[2], cudaStreamNonBlocking, lo));
+        CU(c, cudaStreamCreateWithPriority(&c->band_stream[3], cudaStreamNonBlocking, lo));
+    }
+    const size_t need = (size_t)S * 10 * B * c->nx * 2 * real_size(c->prec);
+    if (c->band_bytes < need) {
+        CU(c, cudaStreamSynchronize(c->stream));
+        band_drop_graphs(c);
+        cudaFree(c->d_band); c->d_band = nullptr; c->band_bytes = 0;
+        if (cudaMalloc(&c->d_band, need) != cudaSuccess) { cudaGetLastError(); return fail(c, QLGA_ENOMEM, "cudaMalloc(band ring) failed"); }
+        c->band_bytes = need;
+        // The ring must STAY in L2: without this the dirty lines of the y pass are written back to DRAM within
+        // microseconds (measured: 21.4 GB of DRAM writes per step instead of 10.7) although the x pass reads them
+        // from L2.  The accesses of the library's own streams to the ring are marked persisting (the kernel nodes of
+        // the captured graphs inherit the window); the device's persisting set-aside is raised to the ring's size
+        // (a per-device limit: it stays raised; qlga.h).
+        cudaDeviceProp prop;
+        CU(c, cudaGetDeviceProperties(&prop, c->device));
+        if (prop.persistingL2CacheMaxSize > 0) {
+            size_t cur = 0;
+            CU(c, cudaDeviceGetLimit(&cur, cudaLimitPersistingL2CacheSize));
+            const size_t want = need < (size_t)prop.persistingL2CacheMaxSize ? need : (size_t)prop.persistingL2CacheMaxSize;
+            if (cur < want) CU(c, cudaDeviceSetLimit(cudaLimitPersistingL2CacheSize, want));
+            cudaStreamAttrValue av;
+            memset(&av, 0, sizeof(av));
+            av.accessPolicyWindow.base_ptr = c->d_band;
+            av.accessPolicyWindow.num_bytes = need < (size_t)prop.accessPolicyMaxWindowSize ? need : (size_t)prop.accessPolicyMaxWindowSize;
+            av.accessPolicyWindow.hitRatio = 1.0f;
+            av.accessPolicyWindow.hitProp = cudaAccessPropertyPersisting;
+            av.accessPolicyWindow.missProp = cudaAccessPropertyStreaming;
+            for (int k = 0; k < 4; ++k)
+                CU(c, cudaStreamSetAttribute(c->band_stream[k], cudaStreamAttributeAccessPolicyWindow, &av));
+        }
+    }
+    const int nev = (int)(2 * nb + 1);
+    if (c->band_nev < nev) {
+        cudaEvent_t* ev = (cudaEvent_t*)realloc(c->band_ev, sizeof(cudaEvent_t) * nev);
+        if (!ev) return fail(c, QLGA_ENOMEM, "band events: out of host memory");
+        c->band_ev = ev;
+        for (; c->band_nev < nev; ++c->band_nev)
+            CU(c, cudaEventCreateWithFlags(&c->band_ev[c->band_nev], cudaEventDisableTiming));
+    }
+    return QLGA_OK;
+}
+
+// issue the band schedule of one time step; `origin` is the stream the step is ordered on (the caller's stream,
+// or the capture origin)
+static qlga_status band_issue(qlga_ctx* c, cudaStream_t origin, int src, int dst, bool tail, int64_t B, int S) {
+    const int64_t nb = (c->ny + B - 1) / B;
+    cudaEvent_t* evY = c->band_ev;
+    cudaEvent_t* evX = c->band_ev + nb;
+    cudaEvent_t ev0 = c->band_ev[2 * nb];
+    cudaStream_t sy = c->band_stream[1];
+    cudaStream_t sx[2] = {c->band_stream[2], c->band_stream[3]};
+    const size_t cb = 2 * real_size(c->prec);
+    const int64_t slot_plane = B * c->nx;                            // elements per plane of a ring slot
+
+    CU(c, cudaEventRecord(ev0, origin));
+    CU(c, cudaStreamWaitEvent(sy, ev0, 0));
+    CU(c, cudaStreamWaitEvent(sx[0], ev0, 0));
+    CU(c, cudaStreamWaitEvent(sx[1], ev0, 0));
+
+    PassParams Py, Px;
+    Py.nx = c->nx; Py.ny = c->ny; Py.nz = 1;
+    fill_pass_consts(c, Py, 1.0);
+    Py.ksteps = 1; Py.umode = 0; Py.utail = 0;
+    Px = Py;
+    Px.utail = tail ? 1 : 0;
+    Py.src = c->buf[src];
+    Py.dst_plane = slot_plane;
+    Px.src_plane = slot_plane;
+    Px.dst_plane = c->nx * c->ny;
+
+    auto issue_y = [&](int64_t k) -> qlga_status {
+        if (k >= S) CU(c, cudaStreamWaitEvent(sy, evX[k - S], 0));
+        Launch L{sy, &c->launches, c->device};
+        Py.dst = (char*)c->d_band + (size_t)(k % S) * 10 * slot_plane * cb;
+        Py.row_begin = k * B;
+        Py.row_end = (k + 1) * B < c->ny ? (k + 1) * B : c->ny;
+        Py.dst_row_origin = k * B;
+#ifdef QLGA_TRACE
+        { void* tp = nullptr; cudaGetSymbolAddress(&tp, g_trace); Py.trace = (unsigned long long*)tp; Py.trace_id = (int)(2 * k) + 2048 * (c->band_ngraph & 3); }   // debug build: graph n traces into ids [2048 n, 2048 n + 2 bands)
+#endif
+        CU(c, launch_march(L, c->prec, 1, Py));
+        CU(c, cudaEventRecord(evY[k], sy));
+        return QLGA_OK;
+    };
+    auto issue_x = [&](int64_t k) -> qlga_status {
+        cudaStream_t s = sx[k & 1];
+        CU(c, cudaStreamWaitEvent(s, evY[k], 0));
+        Launch L{s, &c->launches, c->device};
+        const int64_t r0 = k * B, r1 = (k + 1) * B < c->ny ? (k + 1) * B : c->ny;
+        Px.ny = r1 - r0;
+        Px.src = (const char*)c->d_band + (size_t)(k % S) * 10 * slot_plane * cb;
+        Px.dst = (char*)c->buf[dst] + (size_t)r0 * c->nx * cb;
+#ifdef QLGA_TRACE
+        { void* tp = nullptr; cudaGetSymbolAddress(&tp, g_trace); Px.trace = (unsigned long long*)tp; Px.trace_id = (int)(2 * k + 1) + 2048 * (c->band_ngraph & 3); }
+#endif
+        CU(c, launch_pass(L, c->prec, 0, Px, c->threads_x, 1));
+        CU(c, cudaEventRecord(evX[k], s));
+        return QLGA_OK;
+    };
+    qlga_status st;
+    for (int64_t k = 0; k < S && k < nb; ++k)
+        if ((st = issue_y(k)) != QLGA_OK) return st;
+    for (int64_t k = 0; k < nb; ++k) {
+        if ((st = issue_x(k)) != QLGA_OK) return st;
+        if (k + S < nb && (st = issue_y(k + S)) != QLGA_OK) return st;
+    }
+    // join: each x stream is ordered, so its last event covers it; every y precedes an x
+    CU(c, cudaStreamWaitEvent(origin, evX[nb - 1], 0));
+    if (nb >= 2) CU(c, cudaStreamWaitEvent(origin, evX[nb - 2], 0));
+    return QLGA_OK;
+}
+
+static qlga_status step_band(qlga_ctx* c, int src, int dst, bool tail) {
+    const int64_t B = band_rows_eff(c);
+    const int S = band_slots_eff(c);
+    const int64_t nb = (c->ny + B - 1) / B;
+    qlga_status st = band_setup(c, B, S, nb);
+    if (st != QLGA_OK) return st;
+    if (c->band == 1) return band_issue(c, c->stream, src, dst, tail, B, S);      // -1 (auto) and 2: the graph
+
+    qlga_ctx::BandGraph* g = nullptr;
+    for (int k = 0; k < c->band_ngraph; ++k) {
+        qlga_ctx::BandGraph& h = c->band_graph[k];
+        if (h.src == src && h.dst == dst && h.tail == (int)tail && h.rows == B && h.slots == S) { g = &h; break; }
+    }
+    if (!g) {
+        if (c->band_ngraph == 12) band_drop_graphs(c);
+        // (the per-device shared-memory opt-in of the x pass, run_pass, was made by the first step of the call,
+        // which always takes the two-launch path: nothing but launches, event records and waits is captured)
+        const int64_t before = c->launches;
+        cudaGraph_t graph = nullptr;
+        CU(c, cudaStreamBeginCapture(c->band_stream[0], cudaStreamCaptureModeRelaxed));
+        st = band_issue(c, c->band_stream[0], src, dst, tail, B, S);
+        cudaError_t e = cudaStreamEndCapture(c->band_stream[0], &graph);
+        const int64_t nodes = c->launches - before;
+        c->launches = before;
+        if (st != QLGA_OK) { if (graph) cudaGraphDestroy(graph); cudaGetLastError(); return st; }
+        if (e != cudaSuccess) return cuda_fail(c, "cudaStreamEndCapture(band schedule)", e);
+        cudaGraphExec_t exec = nullptr;
+        e = cudaGraphInstantiate(&exec, graph, 0);
+        cudaGraphDestroy(graph);
+        if (e != cudaSuccess) return cuda_fail(c, "cudaGraphInstantiate(band schedule)", e);
+        g = &c->band_graph[c->band_ngraph++];
+        g->src = src; g->dst = dst; g->tail = (int)tail; g->rows = B; g->slots = S; g->exec = exec; g->nodes = nodes;
+    }
+    CU(c, cudaGraphLaunch(g->exec, c->stream));
+    c->launches += g->nodes;
+    return QLGA_OK;
+}
+
 static qlga_status step_fused(qlga_ctx* c, int64_t nsteps) {
     Launch L{c->stream, &c->launches, c->device};
     const bool inter = c->order == QLGA_INTERLEAVED;
@@ -623,6 +870,18 @@ static qlga_status step_fused(qlga_ctx* c, int64_t nsteps) {
         const int third = pick_other(c, start, pick_other(c, start, -1));
         int src = start;
         const bool tail = !inter && c->fuse_plain_u && (t + 1 < nsteps) && !(keeps_prev && t + 2 == nsteps);
+        if (u_done && band_applies(c)) {
+            // one HBM round trip: the y pass and the x pass of the step pipelined band by band through L2
+            const int dst = pick_other(c, start, -1);
+            prof_mark(c, 3);
+            const qlga_status st = step_band(c, start, dst, tail);
+            if (st != QLGA_OK) return st;
+            u_done = tail;
+            c->prev = (third >= 0) ? start : -1;
+            c->cur = dst;
+            ++c->step;
+            continue;
+        }
         for (int d = c->ndim - 1; d >= 0; --d) {
             int dst;
             if (third >= 0) {
@@ -697,6 +956,7 @@ static qlga_status step_per_operator(qlga_ctx* c, int64_t nsteps) {
 extern "C" qlga_status qlga_set_chemical_potential(qlga_ctx* c, double mu) {
     if (!c) return QLGA_EINVAL;
     if (!(mu == mu) || mu - mu != 0.0) return fail(c, QLGA_EINVAL, "qlga_set_chemical_potential: not a finite value");
+    { DeviceGuard guard(c); band_drop_graphs(c); }
     c->mu = mu;
     return QLGA_OK;
 }

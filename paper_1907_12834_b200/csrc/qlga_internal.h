@@ -25,6 +25,15 @@ struct PassParams {
     double out_scale;      // 2^-4, applied after the 4 factors of a step
     int* flag;             // device error word of the context (FLAG_* in qlga_math.cuh)
     ExpTable tab;
+    // Band mode (qlga_band.cu): source and destination are different views of the lattice.  0 = the lattice's own.
+    int64_t src_plane = 0; // elements between consecutive planes of src (default nx*ny*nz)
+    int64_t dst_plane = 0; // the same for dst
+    // marching pass only: output rows [row_begin, row_end) of the line (default the whole line); row r is stored
+    // at row r - dst_row_origin of dst (a band buffer that starts at row dst_row_origin of the lattice)
+    int64_t row_begin = 0, row_end = 0, dst_row_origin = 0;
+#ifdef QLGA_TRACE
+    unsigned long long* trace = nullptr; int trace_id = 0;   // debug build: first start / last end (globaltimer) per launch
+#endif
 };
 
 struct Launch {
@@ -109,7 +118,19 @@ struct qlga_ctx {
     int threads_x;
     int tile_y;
     int threads_y;
+    int band;              // plain ordering in 2D: one HBM round trip per step by band pipelining (QLGA_OPT_BAND)
+    int band_rows;         // rows per band, 0 = auto (QLGA_OPT_BAND_ROWS)
+    int band_slots;        // slots of the band ring, 0 = auto (QLGA_OPT_BAND_SLOTS)
     qlga::ExpTable tab;
+    // band mode (qlga_api.cu, step_band): the ring that carries the y pass's output to the x pass through L2, the
+    // library's own streams (capture origin, y, x0, x1), the events that order the bands, the instantiated graphs
+    void* d_band;
+    size_t band_bytes;
+    cudaStream_t band_stream[4];
+    cudaEvent_t* band_ev;
+    int band_nev;
+    struct BandGraph { int src, dst, tail; int64_t rows, slots; cudaGraphExec_t exec; int64_t nodes; } band_graph[12];
+    int band_ngraph;
     // scratch owned by the library
     double* d_partials;    // [obs_blocks][OBS_NACC]
     double* d_sums;        // [OBS_NACC]

@@ -29,11 +29,20 @@ struct MarchArgs {
     int64_t len;           // sites along the line
     int64_t stride;        // elements between consecutive sites of a line
     int64_t outer_stride;  // elements between consecutive outer indices (blockIdx.z)
-    int64_t nsites;        // elements per plane
+    int64_t nsites;        // elements per plane of src
+    int64_t dst_nsites;    // elements per plane of dst (= nsites unless dst is a band buffer)
+    int64_t row0, row1;    // output rows [row0, row1) of the line (the whole line, or one band of it)
+    int64_t dst_row_origin;// row r of the line is row r - dst_row_origin of dst
     int64_t seg;           // rows per segment
     int nseg;
     double out_scale;
+#ifdef QLGA_TRACE
+    unsigned long long* trace; int trace_id;
+#endif
 };
+#ifdef QLGA_TRACE
+__device__ __forceinline__ unsigned long long gtimer_m() { unsigned long long t; asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t)); return t; }
+#endif
 
 template <typename T> struct MarchStage { cx<T> F, aP; };
 
@@ -66,15 +75,19 @@ __device__ __forceinline__ void cp_async_elem(float2* sm, const float2* g) {
 template <typename T, typename S, int PF>
 __global__ void __launch_bounds__(128, QLGA_MARCH_MINB) march_kernel(const __grid_constant__ MarchArgs<S> A) {
     using VS = typename vec2<S>::type;
+#ifdef QLGA_TRACE
+    if (A.trace && threadIdx.x == 0) atomicMin(&A.trace[2 * A.trace_id], gtimer_m());
+#endif
     const int64_t x = (int64_t)blockIdx.x * 128 + threadIdx.x;
     if (x >= A.ncol) return;
     // level slowest: the CTAs resident at one time work on the same pair of planes (fewer concurrent DRAM streams:
     // measured 6.5-6.7 TB/s against 6.0-6.2 for a copy kernel of this access pattern)
     const int j = blockIdx.y / A.nseg;
     const int64_t sg = blockIdx.y % A.nseg;
-    const int64_t s0 = sg * A.seg;
-    const int64_t s1 = (s0 + A.seg < A.len) ? s0 + A.seg : A.len;     // output rows [s0, s1)
+    const int64_t s0 = A.row0 + sg * A.seg;
+    const int64_t s1 = (s0 + A.seg < A.row1) ? s0 + A.seg : A.row1;   // output rows [s0, s1)
     const int64_t base = (int64_t)(2 * j) * A.nsites + (int64_t)blockIdx.z * A.outer_stride + x;
+    const int64_t base_dst = (int64_t)(2 * j) * A.dst_nsites + (int64_t)blockIdx.z * A.outer_stride + x;
     const T scale = (T)A.out_scale;
 
     // input rows r0 .. r1-1 (periodic), r0 = s0 - 4, r1 = s1 + 4; the load pointer walks down the line and wraps.
@@ -89,7 +102,7 @@ __global__ void __launch_bounds__(128, QLGA_MARCH_MINB) march_kernel(const __gri
     const VS* __restrict__ pl = A.src + base + rl * A.stride;          // component 1; component 2 is one plane further
     const VS* __restrict__ pl_wrap = A.src + base;
     int64_t to_wrap = A.len - rl;                                     // rows until the pointer wraps to row 0
-    VS* __restrict__ ps = A.dst + base + s0 * A.stride;                // store pointer (no wrap: s0 .. s1-1)
+    VS* __restrict__ ps = A.dst + base_dst + (s0 - A.dst_row_origin) * A.stride;                // store pointer (no wrap: s0 .. s1-1)
     int nload = nrows;
 #pragma unroll
     for (int u = 0; u < PF; ++u) {
@@ -127,13 +140,16 @@ __global__ void __launch_bounds__(128, QLGA_MARCH_MINB) march_kernel(const __gri
                 march_stage<T>(st[3], c1, c2);
                 if (done >= 8) {                               // the row that leaves the pipeline: r - 4 >= s0
                     st_state<T, S>(ps, rmul(scale, c1));
-                    st_state<T, S>(ps + A.nsites, rmul(scale, c2));
+                    st_state<T, S>(ps + A.dst_nsites, rmul(scale, c2));
                     ps += A.stride;
                 }
                 ++done;
             }
         }
     }
+#ifdef QLGA_TRACE
+    if (A.trace && threadIdx.x == 0) atomicMax(&A.trace[2 * A.trace_id + 1], gtimer_m());
+#endif
 }
 
 template <typename T, typename S>
@@ -141,18 +157,24 @@ static cudaError_t run_march(const Launch& L, const PassParams& P, int dir) {
     MarchArgs<S> A;
     A.src = (const typename vec2<S>::type*)P.src;
     A.dst = (typename vec2<S>::type*)P.dst;
-    A.nsites = P.nx * P.ny * P.nz;
+    A.nsites = P.src_plane ? P.src_plane : P.nx * P.ny * P.nz;
+    A.dst_nsites = P.dst_plane ? P.dst_plane : P.nx * P.ny * P.nz;
     A.out_scale = P.out_scale;
+#ifdef QLGA_TRACE
+    A.trace = P.trace; A.trace_id = P.trace_id;
+#endif
     int64_t n_outer;
     if (dir == 1) { A.ncol = P.nx; A.len = P.ny; A.stride = P.nx; n_outer = P.nz; A.outer_stride = P.nx * P.ny; }
     else          { A.ncol = P.nx * P.ny; A.len = P.nz; A.stride = P.nx * P.ny; n_outer = 1; A.outer_stride = 0; }
     // segments: about six waves of threads at full residency, at least 32 rows each (run-in and run-out cost 8)
+    A.row0 = P.row_begin; A.row1 = P.row_end > P.row_begin ? P.row_end : A.len; A.dst_row_origin = P.dst_row_origin;
+    const int64_t rows = A.row1 - A.row0;
     const int64_t per_seg = A.ncol * 5 * n_outer;
     int64_t nseg = (int64_t)(1400000 + per_seg - 1) / per_seg;
-    if (nseg > A.len / 32) nseg = A.len / 32;
+    if (nseg > rows / 32) nseg = rows / 32;
     if (nseg < 1) nseg = 1;
-    A.seg = (A.len + nseg - 1) / nseg;
-    nseg = (A.len + A.seg - 1) / A.seg;
+    A.seg = (rows + nseg - 1) / nseg;
+    nseg = (rows + A.seg - 1) / A.seg;
     A.nseg = (int)nseg;
     const int64_t bx = (A.ncol + 127) / 128;
     if (bx > 2147483647LL || nseg * 5 > 65535 || n_outer > 65535) return cudaErrorInvalidValue;

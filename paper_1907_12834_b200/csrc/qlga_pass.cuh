@@ -36,13 +36,21 @@ struct PassArgs {
     // the lines.  x pass: len = nx, the lines are the ny*nz rows (outer_stride = nx).
     // y pass: stride = nx, len = ny, outer = z.   z pass: stride = nx*ny, len = nz, outer = y.
     int64_t nx, len, stride, n_outer, outer_stride, nsites;
+    int64_t nsites_dst;         // plane stride of dst (= nsites unless dst is another view of the lattice: band mode)
     int ksteps, umode, utail;
     UConst<T> uc[4];
     UConst<T> uct;              // trailing U of the plain ordering (see pass_kernel)
     T out_scale;
     int* flag;                  // device error word (qlga_internal.h, FLAG_*)
     ExpTable tab;
+#ifdef QLGA_TRACE
+    unsigned long long* trace; int trace_id;
+#endif
 };
+
+#ifdef QLGA_TRACE
+__device__ __forceinline__ unsigned long long gtimer() { unsigned long long t; asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t)); return t; }
+#endif
 
 __device__ __forceinline__ int64_t pmod(int64_t a, int64_t n) {
     int64_t r = a % n;
@@ -128,6 +136,9 @@ pass_kernel(const __grid_constant__ PassArgs<T, S> P) {
     V (*sB)[5][NT] = sF + 2;
 
     const int t = threadIdx.x;
+#ifdef QLGA_TRACE
+    if (P.trace && t == 0) atomicMin(&P.trace[2 * P.trace_id], gtimer());
+#endif
     const int c = t % CX, i = t / CX;
     const int H = 4 * P.ksteps;
     const int wout = TS - 2 * H;
@@ -193,10 +204,13 @@ pass_kernel(const __grid_constant__ PassArgs<T, S> P) {
     if (i >= H && i < TS - H && spos < extent && col_ok) {
 #pragma unroll
         for (int j = 0; j < 5; ++j) {
-            st_state<T, S>(P.dst + (int64_t)(2 * j + 0) * n + idx, s.q[j][0]);
-            st_state<T, S>(P.dst + (int64_t)(2 * j + 1) * n + idx, s.q[j][1]);
+            st_state<T, S>(P.dst + (int64_t)(2 * j + 0) * P.nsites_dst + idx, s.q[j][0]);
+            st_state<T, S>(P.dst + (int64_t)(2 * j + 1) * P.nsites_dst + idx, s.q[j][1]);
         }
     }
+#ifdef QLGA_TRACE
+    if (P.trace && t == 0) atomicMax(&P.trace[2 * P.trace_id + 1], gtimer());
+#endif
 }
 
 template <typename T, typename S>
@@ -205,11 +219,15 @@ static PassArgs<T, S> make_args(const PassParams& P, int dir) {
     A.src = (const typename vec2<S>::type*)P.src;
     A.dst = (typename vec2<S>::type*)P.dst;
     A.flag = P.flag;
-    A.nx = P.nx; A.nsites = P.nx * P.ny * P.nz; A.ksteps = P.ksteps; A.umode = P.umode; A.utail = P.utail;
+    A.nx = P.nx; A.nsites = P.src_plane ? P.src_plane : P.nx * P.ny * P.nz;
+    A.nsites_dst = P.dst_plane ? P.dst_plane : P.nx * P.ny * P.nz; A.ksteps = P.ksteps; A.umode = P.umode; A.utail = P.utail;
     A.uct = make_uconst<T>(P.gt[0], P.gt[1], P.gt[2], P.smu);
     for (int f = 0; f < 4; ++f) A.uc[f] = make_uconst<T>(P.g[f][0], P.g[f][1], P.g[f][2], P.smu);
     A.out_scale = (T)P.out_scale;
     A.tab = P.tab;
+#ifdef QLGA_TRACE
+    A.trace = P.trace; A.trace_id = P.trace_id;
+#endif
     if (dir == 0)      { A.len = P.nx; A.stride = 1;           A.n_outer = P.ny * P.nz; A.outer_stride = P.nx; }
     else if (dir == 1) { A.len = P.ny; A.stride = P.nx;        A.n_outer = P.nz;        A.outer_stride = P.nx * P.ny; }
     else               { A.len = P.nz; A.stride = P.nx * P.ny; A.n_outer = P.ny;        A.outer_stride = P.nx; }

@@ -19,7 +19,7 @@ QLGA_OK, QLGA_EINVAL, QLGA_ENOMEM, QLGA_ECUDA, QLGA_ESTATE, QLGA_EUNSUP = range(
 QLGA_F64, QLGA_F32, QLGA_F32X = 0, 1, 2
 QLGA_PLAIN, QLGA_INTERLEAVED = 0, 1
 (OPT_PATH, OPT_STEPS_PER_LAUNCH, OPT_EXP_TOL_LOG2, OPT_THREADS_X, OPT_TILE_Y, OPT_THREADS_Y, OPT_FUSE_PLAIN_U,
- OPT_F32_PHASE, OPT_EXP_POLY, OPT_EXP_MOD_SHIFT, OPT_MARCH) = range(11)
+ OPT_F32_PHASE, OPT_EXP_POLY, OPT_EXP_MOD_SHIFT, OPT_MARCH, OPT_BAND, OPT_BAND_ROWS, OPT_BAND_SLOTS) = range(14)
 _PRECISIONS = {"f64": QLGA_F64, "fp64": QLGA_F64, "double": QLGA_F64, "f32": QLGA_F32, "fp32": QLGA_F32,
                "float": QLGA_F32, "f32x": QLGA_F32X}
 
@@ -51,7 +51,7 @@ class QlgaAngles(ctypes.Structure):
 
 
 class QlgaProfile(ctypes.Structure):
-    _fields_ = [("ms", ctypes.c_double * 3), ("launches", ctypes.c_int64 * 3)]
+    _fields_ = [("ms", ctypes.c_double * 4), ("launches", ctypes.c_int64 * 4)]
 
 
 class QlgaError(RuntimeError):
@@ -398,10 +398,10 @@ class Qlga:
         self._check(_lib.qlga_profile_enable(self.ctx, int(bool(on))))
 
     def profile_read(self):
-        """{'x_pass': (ms, launches), 'y_pass': ..., 'per_operator': ...} since the last read."""
+        """{'x_pass': (ms, launches), 'y_pass': ..., 'per_operator': ..., 'band_step': ...} since the last read."""
         pr = QlgaProfile()
         self._check(_lib.qlga_profile_read(self.ctx, ctypes.byref(pr)))
-        names = ("x_pass", "y_pass", "per_operator")
+        names = ("x_pass", "y_pass", "per_operator", "band_step")
         return {n: (pr.ms[k], int(pr.launches[k])) for k, n in enumerate(names)}
 
     def launch_count(self):

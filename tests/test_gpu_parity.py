@@ -657,6 +657,73 @@ def test_marching_pass_is_bit_identical_to_the_tile_kernel(qlga, oracle):
         assert rel_l2(run_gpu(qlga, q0, ndim, c, "plain", 3), oracle.step(q0, ndim, c, 0, 3)) < TOL64
 
 
+def test_band_mode_is_bit_identical_and_matches_the_oracle(qlga, oracle):
+    # QLGA_OPT_BAND: the plain 2D step pipelined band by band (marching y pass -> ring in L2 -> x pass with the next
+    # step's U), issued on the library's own streams (1) or replayed as a CUDA graph (2).  Same kernels, same
+    # arithmetic: bit-identical to the two-launch step -- ragged last band, bands of one row, more slots than bands
+    # would need, lattices with fewer than four bands (falls back), every precision, with and without the
+    # previous-state buffer, every split of the steps into calls, options and the chemical potential changed
+    # between calls (the instantiated graphs hold kernel arguments and must be dropped).  And against the oracle.
+    c = (1.0, 0.3, -0.1)
+    cases = [((300, 203), 16, 3), ((130, 64), 8, 2), ((257, 100), 25, 4), ((64, 40), 1, 8), ((96, 33), 0, 0), ((50, 20), 8, 3)]
+    for dims, rows, slots in cases:
+        q0 = inputs.random_spinor_state(dims, seed=71 + dims[0], amplitude=0.05)
+        for precision in ("f64", "f32", "f32x"):
+            qin = q0 if precision == "f64" else q0.astype(np.complex64)
+            for keep in (False, True):
+                outs, obs, launches = [], [], []
+                for band in (0, 1, 2):
+                    sim = qlga.Qlga(2, dims, c, order="plain", precision=precision, keep_previous=keep)
+                    sim.set_option(qlga.OPT_BAND, band)
+                    sim.set_option(qlga.OPT_BAND_ROWS, rows)
+                    sim.set_option(qlga.OPT_BAND_SLOTS, slots)
+                    sim.set_state_q(qin)
+                    n0 = sim.launch_count()
+                    sim.step(6)
+                    launches.append(sim.launch_count() - n0)
+                    outs.append(sim.get_state_q())
+                    obs.append(sim.observables())
+                    sim.close()
+                assert np.array_equal(outs[0], outs[1]) and np.array_equal(outs[0], outs[2]), (dims, precision, keep)
+                assert launches[1] == launches[2], (dims, launches)       # the graph replays what mode 1 launches
+                if rows and dims[1] >= 4 * rows:
+                    assert launches[1] > launches[0], (dims, launches)    # band mode really ran
+                if keep:
+                    for k in (1, 2):
+                        assert obs[k]["e_dt_re"] == obs[0]["e_dt_re"] and obs[k]["e_dt_im"] == obs[0]["e_dt_im"]
+        assert rel_l2(outs[2].astype(np.complex128),
+                      oracle.step(q0.astype(np.complex64).astype(np.complex128), 2, c, 0, 6)) < TOL32      # f32x
+    # several calls, an option and the chemical potential changed in between; against the oracle
+    dims = (300, 203)
+    q0 = inputs.random_spinor_state(dims, seed=77, amplitude=0.05)
+    sim = qlga.Qlga(2, dims, c, order="plain")
+    sim.set_option(qlga.OPT_BAND, 2)
+    sim.set_option(qlga.OPT_BAND_ROWS, 16)
+    sim.set_state_q(q0)
+    sim.step(4)
+    sim.step(3)
+    assert rel_l2(sim.get_state_q(), oracle.step(q0, 2, c, 0, 7)) < TOL64
+    q7 = sim.get_state_q()
+    sim.set_chemical_potential(0.37)
+    sim.set_option(qlga.OPT_BAND_ROWS, 24)
+    sim.step(4)
+    out = sim.get_state_q()
+    sim.close()
+    assert rel_l2(out, oracle.step(q7, 2, c, 0, 4, mu=0.37)) < TOL64
+    ref = qlga.Qlga(2, dims, c, order="plain")
+    ref.set_chemical_potential(0.37)
+    ref.set_state_q(q7)
+    ref.step(4)
+    assert np.array_equal(out, ref.get_state_q())
+    ref.close()
+    # the options are validated
+    sim = qlga.Qlga(2, dims, c, order="plain")
+    for key, bad in ((qlga.OPT_BAND, 3), (qlga.OPT_BAND, -2), (qlga.OPT_BAND_ROWS, -2), (qlga.OPT_BAND_SLOTS, 1), (qlga.OPT_BAND_SLOTS, 9)):
+        with pytest.raises(qlga.QlgaError):
+            sim.set_option(key, bad)
+    sim.close()
+
+
 def test_option_validation_and_the_device_error_word(qlga):
     # (TILE_Y, THREADS_Y) are validated as a pair (only built kernels), STEPS_PER_LAUNCH against what the kernels support;
     # a state with a non-finite amplitude does not hang the sub-angle loop: the kernels raise the context's error word
