@@ -27,6 +27,64 @@ __device__ __forceinline__ void load_psi(const typename vec2<T>::type* q, int64_
     if (normq) *normq = nq;
 }
 
+// The sums of one site: psi = (pr, pi), |q|^2 = nq, the +x / +y / +z neighbours' psi, the previous state's psi.
+__device__ __forceinline__ void obs_site(double acc[OBS_NACC], int ndim, bool has_prev, double nq,
+                                         const double pr[5], const double pi[5], const double xr[5], const double xi[5],
+                                         const double yr[5], const double yi[5], const double zr[5], const double zi[5],
+                                         const double or_[5], const double oi[5]) {
+    const double rt6 = 2.4494897427831780981972840747059;
+    const double irt5 = 0.44721359549995793928183473374626;
+    acc[A_NQ] += nq;
+    double nm[5];
+#pragma unroll
+    for (int j = 0; j < 5; ++j) { nm[j] = pr[j] * pr[j] + pi[j] * pi[j]; acc[A_N0 + j] += nm[j]; }
+    const double rho = nm[0] + nm[1] + nm[2] + nm[3] + nm[4];
+    const double Fz = 2.0 * (nm[0] - nm[4]) + (nm[1] - nm[3]);
+    // F_+ = 2(conj(psi_2) psi_1 + conj(psi_-1) psi_-2) + sqrt6 (conj(psi_1) psi_0 + conj(psi_0) psi_-1)
+    const double far_ = pr[0] * pr[1] + pi[0] * pi[1] + pr[3] * pr[4] + pi[3] * pi[4];
+    const double fai = pr[0] * pi[1] - pi[0] * pr[1] + pr[3] * pi[4] - pi[3] * pr[4];
+    const double fbr = pr[1] * pr[2] + pi[1] * pi[2] + pr[2] * pr[3] + pi[2] * pi[3];
+    const double fbi = pr[1] * pi[2] - pi[1] * pr[2] + pr[2] * pi[3] - pi[2] * pr[3];
+    const double Fx = 2.0 * far_ + rt6 * fbr, Fy = 2.0 * fai + rt6 * fbi;
+    acc[A_FX] += Fx; acc[A_FY] += Fy; acc[A_FZ] += Fz;
+    // A00 = (2 psi_2 psi_-2 - 2 psi_1 psi_-1 + psi_0^2)/sqrt5
+    const double tr = 2.0 * (pr[0] * pr[4] - pi[0] * pi[4]) - 2.0 * (pr[1] * pr[3] - pi[1] * pi[3])
+            + (pr[2] * pr[2] - pi[2] * pi[2]);
+    const double ti = 2.0 * (pr[0] * pi[4] + pi[0] * pr[4]) - 2.0 * (pr[1] * pi[3] + pi[1] * pr[3])
+            + 2.0 * pr[2] * pi[2];
+    const double ar = tr * irt5, ai = ti * irt5;
+    acc[A_A00R] += ar; acc[A_A00I] += ai; acc[A_A2] += ar * ar + ai * ai;
+    acc[A_RHO2] += rho * rho;
+    acc[A_F2] += Fx * Fx + Fy * Fy + Fz * Fz;
+    // kinetic: forward differences along x (and y, z)
+#pragma unroll
+    for (int j = 0; j < 5; ++j) {
+        const double dr = xr[j] - pr[j], di = xi[j] - pi[j];
+        acc[A_EKIN] += dr * dr + di * di;
+    }
+    if (ndim >= 2) {
+#pragma unroll
+        for (int j = 0; j < 5; ++j) {
+            const double dr = yr[j] - pr[j], di = yi[j] - pi[j];
+            acc[A_EKIN] += dr * dr + di * di;
+        }
+    }
+    if (ndim == 3) {
+#pragma unroll
+        for (int j = 0; j < 5; ++j) {
+            const double dr = zr[j] - pr[j], di = zi[j] - pi[j];
+            acc[A_EKIN] += dr * dr + di * di;
+        }
+    }
+    if (has_prev) {       // <psi(t)|psi(t - tau)>
+#pragma unroll
+        for (int j = 0; j < 5; ++j) {
+            acc[A_OVR] += pr[j] * or_[j] + pi[j] * oi[j];
+            acc[A_OVI] += pr[j] * oi[j] - pi[j] * or_[j];
+        }
+    }
+}
+
 // Work unit = 128 columns (x) x a segment of rows (y) of one z layer.  A thread owns one column of the unit and
 // marches down its rows: every site's ten amplitudes are loaded once (the row below is kept in registers for the
 // y difference of the kinetic energy; the +x neighbour is a load that hits the line its neighbour thread just
@@ -72,60 +130,140 @@ __global__ void __launch_bounds__(128, sizeof(T) == 8 ? 2 : 4) observables_kerne
             if (G.ndim == 3) load_psi<T>(q, n, (zn * G.ny + y) * G.nx + x, zr, zi, nullptr);
             if (qprev) load_psi<T>(qprev, n, row + x, or_, oi, nullptr);
 
-            acc[A_NQ] += nq;
-            double nm[5];
-#pragma unroll
-            for (int j = 0; j < 5; ++j) { nm[j] = pr[j] * pr[j] + pi[j] * pi[j]; acc[A_N0 + j] += nm[j]; }
-            const double rho = nm[0] + nm[1] + nm[2] + nm[3] + nm[4];
-            const double Fz = 2.0 * (nm[0] - nm[4]) + (nm[1] - nm[3]);
-            // F_+ = 2(conj(psi_2) psi_1 + conj(psi_-1) psi_-2) + sqrt6 (conj(psi_1) psi_0 + conj(psi_0) psi_-1)
-            const double far_ = pr[0] * pr[1] + pi[0] * pi[1] + pr[3] * pr[4] + pi[3] * pi[4];
-            const double fai = pr[0] * pi[1] - pi[0] * pr[1] + pr[3] * pi[4] - pi[3] * pr[4];
-            const double fbr = pr[1] * pr[2] + pi[1] * pi[2] + pr[2] * pr[3] + pi[2] * pi[3];
-            const double fbi = pr[1] * pi[2] - pi[1] * pr[2] + pr[2] * pi[3] - pi[2] * pr[3];
-            const double Fx = 2.0 * far_ + rt6 * fbr, Fy = 2.0 * fai + rt6 * fbi;
-            acc[A_FX] += Fx; acc[A_FY] += Fy; acc[A_FZ] += Fz;
-            // A00 = (2 psi_2 psi_-2 - 2 psi_1 psi_-1 + psi_0^2)/sqrt5
-            const double tr = 2.0 * (pr[0] * pr[4] - pi[0] * pi[4]) - 2.0 * (pr[1] * pr[3] - pi[1] * pi[3])
-                            + (pr[2] * pr[2] - pi[2] * pi[2]);
-            const double ti = 2.0 * (pr[0] * pi[4] + pi[0] * pr[4]) - 2.0 * (pr[1] * pi[3] + pi[1] * pr[3])
-                            + 2.0 * pr[2] * pi[2];
-            const double ar = tr * irt5, ai = ti * irt5;
-            acc[A_A00R] += ar; acc[A_A00I] += ai; acc[A_A2] += ar * ar + ai * ai;
-            acc[A_RHO2] += rho * rho;
-            acc[A_F2] += Fx * Fx + Fy * Fy + Fz * Fz;
-            // kinetic: forward differences along x (and y, z)
-#pragma unroll
-            for (int j = 0; j < 5; ++j) {
-                const double dr = xr[j] - pr[j], di = xi[j] - pi[j];
-                acc[A_EKIN] += dr * dr + di * di;
-            }
-            if (G.ndim >= 2) {
-#pragma unroll
-                for (int j = 0; j < 5; ++j) {
-                    const double dr = yr[j] - pr[j], di = yi[j] - pi[j];
-                    acc[A_EKIN] += dr * dr + di * di;
-                }
-            }
-            if (G.ndim == 3) {
-#pragma unroll
-                for (int j = 0; j < 5; ++j) {
-                    const double dr = zr[j] - pr[j], di = zi[j] - pi[j];
-                    acc[A_EKIN] += dr * dr + di * di;
-                }
-            }
-            if (qprev) {       // <psi(t)|psi(t - tau)>
-#pragma unroll
-                for (int j = 0; j < 5; ++j) {
-                    acc[A_OVR] += pr[j] * or_[j] + pi[j] * oi[j];
-                    acc[A_OVI] += pr[j] * oi[j] - pi[j] * or_[j];
-                }
-            }
+            obs_site(acc, G.ndim, qprev != nullptr, nq, pr, pi, xr, xi, yr, yi, zr, zi, or_, oi);
             // the row below becomes the current row
 #pragma unroll
             for (int j = 0; j < 5; ++j) { pr[j] = yr[j]; pi[j] = yi[j]; }
             nq = ynq;
         }
+    }
+
+    __shared__ double sm[4][OBS_NACC];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+#pragma unroll
+    for (int k = 0; k < OBS_NACC; ++k) {
+        double v = acc[k];
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+        if (lane == 0) sm[warp][k] = v;
+    }
+    __syncthreads();
+    if (threadIdx.x < OBS_NACC) {
+        double v = 0.0;
+        for (int w = 0; w < 4; ++w) v += sm[w][threadIdx.x];
+        partials[(int64_t)blockIdx.x * OBS_NACC + threadIdx.x] = v;
+    }
+}
+
+// 2D lattices: the same work units with the loads staged through shared memory (round 2).  Every thread copies the ten
+// amplitudes of its column, one row per cp.async group, R - 2 rows ahead of the row it sums (no registers held by loads
+// in flight: 40 KB per CTA, 80 KB per SM in flight, against ~40 KB of the register version, which reached 58 % of the
+// copy bandwidth at 250 registers); psi of the row below is formed once per site from the ring and handed to the left
+// neighbour through a small double-buffered array (the +x difference of the next row), so a site costs 20 + 5 shared
+// loads and 5 stores instead of 20 more global loads.  One barrier per row.  Same units, same order of the sums per
+// thread as observables_kernel.
+constexpr int OBS_RING = 4;
+template <typename T> struct ObsRing {
+    typename vec2<T>::type ring[OBS_RING][10][129];   // [slot][plane][column; 128 = the +x neighbour of the last column]
+    double2 psi[2][5][129];                            // psi of a row, [row parity][level][column]
+};
+
+template <typename T>
+__device__ __forceinline__ void obs_cp_async(typename vec2<T>::type* sm, const typename vec2<T>::type* g) {
+    if constexpr (sizeof(T) == 8)
+        asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"((unsigned)__cvta_generic_to_shared(sm)), "l"(g) : "memory");
+    else
+        asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"((unsigned)__cvta_generic_to_shared(sm)), "l"(g) : "memory");
+}
+
+template <typename T>
+__global__ void __launch_bounds__(128, sizeof(T) == 8 ? 2 : 3) observables_ring_kernel(const typename vec2<T>::type* __restrict__ q,
+                                                          const typename vec2<T>::type* __restrict__ qprev,
+                                                          const __grid_constant__ ObsGeom G, double* partials) {
+    using V = typename vec2<T>::type;
+    extern __shared__ __align__(16) unsigned char obs_smem[];
+    ObsRing<T>& S = *reinterpret_cast<ObsRing<T>*>(obs_smem);
+    const int64_t n = G.nx * G.ny;
+    const int t = threadIdx.x;
+    double acc[OBS_NACC];
+#pragma unroll
+    for (int k = 0; k < OBS_NACC; ++k) acc[k] = 0.0;
+    double zr[5] = {0, 0, 0, 0, 0}, zi[5] = {0, 0, 0, 0, 0};        // no z direction in 2D
+
+    const int64_t units = G.ncb * G.nsg;
+    for (int64_t u = blockIdx.x; u < units; u += gridDim.x) {
+        const int64_t cb = u % G.ncb, sg = u / G.ncb;
+        const int64_t xb = G.x0 + cb * 128;
+        const int ncols = (int)((G.x1 - xb < 128) ? G.x1 - xb : 128);
+        const bool own = t < ncols;                                     // this thread sums a column
+        const int64_t x = xb + (own ? t : 0);
+        const int64_t xe = (xb + ncols == G.nx) ? 0 : xb + ncols;       // the +x neighbour of the unit's last column
+        const int64_t ys = G.y0 + sg * G.seg;
+        const int64_t ye = (ys + G.seg < G.y1) ? ys + G.seg : G.y1;
+        const int nr = (int)(ye - ys);                                  // rows summed; rows ys .. ye are needed
+        // copy row ys + i (periodic) of this thread's column (thread 0: also of column xe) into slot i mod R
+        auto issue = [&](int i) {
+            if (i <= nr) {
+                int64_t y = ys + i;
+                if (y >= G.ny) y -= G.ny;
+                const V* g = q + y * G.nx;
+                V (*slot)[129] = S.ring[i % OBS_RING];
+                if (own) {
+#pragma unroll
+                    for (int pl = 0; pl < 10; ++pl) obs_cp_async<T>(&slot[pl][t], g + (int64_t)pl * n + x);
+                }
+                if (t == 0) {
+#pragma unroll
+                    for (int pl = 0; pl < 10; ++pl) obs_cp_async<T>(&slot[pl][ncols], g + (int64_t)pl * n + xe);
+                }
+            }
+            asm volatile("cp.async.commit_group;" ::: "memory");
+        };
+        // psi and |q|^2 of column c of the row in `slot`
+        auto form = [&](int slot, int c, double pr[5], double pi[5], double& nq) {
+            nq = 0.0;
+#pragma unroll
+            for (int j = 0; j < 5; ++j) {
+                const V a = S.ring[slot][2 * j][c], b = S.ring[slot][2 * j + 1][c];
+                const double ar = a.x, ai = a.y, br = b.x, bi = b.y;
+                pr[j] = ar + br; pi[j] = ai + bi;
+                nq += ar * ar + ai * ai + br * br + bi * bi;
+            }
+        };
+        auto publish = [&](int par, int c, const double pr[5], const double pi[5]) {
+#pragma unroll
+            for (int j = 0; j < 5; ++j) S.psi[par][j][c] = make_double2(pr[j], pi[j]);
+        };
+
+        __syncthreads();                                   // the previous unit's readers are done with the ring
+#pragma unroll
+        for (int i = 0; i < OBS_RING - 1; ++i) issue(i);
+        asm volatile("cp.async.wait_group %0;" ::"n"(OBS_RING - 2) : "memory");      // row ys has landed
+        __syncthreads();
+        double pr[5], pi[5], nq = 0.0;
+        if (own) { form(0, t, pr, pi, nq); publish(0, t, pr, pi); }
+        if (t == 0) { double er[5], ei[5], en; form(0, ncols, er, ei, en); publish(0, ncols, er, ei); }
+        for (int i = 0; i < nr; ++i) {
+            asm volatile("cp.async.wait_group %0;" ::"n"(OBS_RING - 3) : "memory");  // row ys + i + 1 has landed
+            __syncthreads();                               // ... for every thread; psi of row ys + i is published
+            issue(i + OBS_RING - 1);                       // into the slot of row ys + i - 1
+            double yr[5], yi[5], ynq = 0.0, xr[5], xi[5], or_[5], oi[5];
+            if (own) {
+                form((i + 1) % OBS_RING, t, yr, yi, ynq);
+                publish((i + 1) & 1, t, yr, yi);
+            }
+            if (t == 0) { double er[5], ei[5], en; form((i + 1) % OBS_RING, ncols, er, ei, en); publish((i + 1) & 1, ncols, er, ei); }
+            if (own) {
+#pragma unroll
+                for (int j = 0; j < 5; ++j) { const double2 v = S.psi[i & 1][j][t + 1]; xr[j] = v.x; xi[j] = v.y; }
+                if (qprev) load_psi<T>(qprev, n, (ys + i) * G.nx + x, or_, oi, nullptr);
+                obs_site(acc, 2, qprev != nullptr, nq, pr, pi, xr, xi, yr, yi, zr, zi, or_, oi);
+#pragma unroll
+                for (int j = 0; j < 5; ++j) { pr[j] = yr[j]; pi[j] = yi[j]; }
+                nq = ynq;
+            }
+        }
+        asm volatile("cp.async.wait_group 0;" ::: "memory");
     }
 
     __shared__ double sm[4][OBS_NACC];
@@ -184,7 +322,19 @@ cudaError_t launch_observables(const Launch& L, qlga_prec prec, const void* q, c
     G.nsg = (rows + G.seg - 1) / G.seg;
     const int64_t units = G.ncb * G.nsg * (G.z1 - G.z0);
     if (units < nblocks) nblocks = (int)units;
-    if (prec == QLGA_F64)
+    if (ndim == 2) {
+        // (the shared-memory opt-in is a per-device attribute of the function: set on every launch, idempotent and cheap)
+        cudaError_t e;
+        if (prec == QLGA_F64) {
+            e = cudaFuncSetAttribute(observables_ring_kernel<double>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(ObsRing<double>));
+            if (e != cudaSuccess) return e;
+            observables_ring_kernel<double><<<nblocks, 128, sizeof(ObsRing<double>), L.stream>>>((const double2*)q, (const double2*)qprev, G, partials);
+        } else {
+            e = cudaFuncSetAttribute(observables_ring_kernel<float>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(ObsRing<float>));
+            if (e != cudaSuccess) return e;
+            observables_ring_kernel<float><<<nblocks, 128, sizeof(ObsRing<float>), L.stream>>>((const float2*)q, (const float2*)qprev, G, partials);
+        }
+    } else if (prec == QLGA_F64)
         observables_kernel<double><<<nblocks, 128, 0, L.stream>>>((const double2*)q, (const double2*)qprev, G, partials);
     else
         observables_kernel<float><<<nblocks, 128, 0, L.stream>>>((const float2*)q, (const float2*)qprev, G, partials);
