@@ -475,6 +475,52 @@ __device__ __forceinline__ void horner_stage_fused(cx<T> u[5], const cx<T> v[5],
     u[4] = cfma_conj(psi[0], tk, r4);
 }
 
+// Plain Horner stages k = kfirst .. 1 (u <- v - i r_k sK u) of the path without the spin gauge (fp32).  A one-stage loop
+// cost the fp32 kernels 33 MOVs per 47 packed FP instructions: register-pair copies of the loop-carried (re, im) pairs
+// around the back edge (ptxas).  The degrees that occur in fp32 (kfirst <= 3, i.e. p <= 4) are therefore straight-line
+// code, every stage writing a fresh vector; higher degrees run two stages per trip with ping-pong vectors.
+template <typename T>
+__device__ __forceinline__ void horner_plain_stage(const cx<T> uin[5], cx<T> uout[5], const cx<T> v[5], const KCoef<T>& kc, T ik) {
+    cx<T> w[5];
+    apply_sK(uin, w, kc.az, kc.az2, kc.a1, kc.a6, kc.g2, kc.psi);
+#pragma unroll
+    for (int j = 0; j < 5; ++j) uout[j] = axmi(ik, w[j], v[j]);
+}
+template <typename T>
+__device__ __forceinline__ void horner_plain_stages(cx<T> u[5], const cx<T> v[5], const KCoef<T>& kc,
+                                                    const T* __restrict__ r, int kfirst) {
+    cx<T> a[5], b[5];
+    if (kfirst == 1) {
+        horner_plain_stage<T>(u, a, v, kc, r[1]);
+#pragma unroll
+        for (int j = 0; j < 5; ++j) u[j] = a[j];
+    } else if (kfirst == 2) {
+        horner_plain_stage<T>(u, a, v, kc, r[2]);
+        horner_plain_stage<T>(a, b, v, kc, r[1]);
+#pragma unroll
+        for (int j = 0; j < 5; ++j) u[j] = b[j];
+    } else if (kfirst == 3) {
+        horner_plain_stage<T>(u, a, v, kc, r[3]);
+        horner_plain_stage<T>(a, b, v, kc, r[2]);
+        horner_plain_stage<T>(b, a, v, kc, r[1]);
+#pragma unroll
+        for (int j = 0; j < 5; ++j) u[j] = a[j];
+    } else if (kfirst > 3) {
+        int k = kfirst;
+        if (k & 1) {
+            horner_plain_stage<T>(u, a, v, kc, r[k]);
+#pragma unroll
+            for (int j = 0; j < 5; ++j) u[j] = a[j];
+            --k;
+        }
+#pragma unroll 1
+        for (; k >= 2; k -= 2) {
+            horner_plain_stage<T>(u, a, v, kc, r[k]);
+            horner_plain_stage<T>(a, u, v, kc, r[k - 1]);
+        }
+    }
+}
+
 // u <- P_p(-i sK') v in Horner form u_{k-1} = v + r_k (-i sK') u_k, k = p..1, u_p = v
 // (stage p acts on v itself: no copy).  psi, hence K, is frozen (reading R4).
 template <typename T>
@@ -503,13 +549,7 @@ __device__ __forceinline__ void horner(const cx<T> v[5], cx<T> u[5], const KCoef
             }
         }
     } else {
-#pragma unroll 1
-        for (int k = p - 1; k >= 1; --k) {
-            apply_sK(u, w, kc.az, kc.az2, kc.a1, kc.a6, kc.g2, kc.psi);
-            const T ik = r[k];
-#pragma unroll
-            for (int j = 0; j < 5; ++j) u[j] = axmi(ik, w[j], v[j]);
-        }
+        horner_plain_stages<T>(u, v, kc, r, p - 1);
     }
 }
 
@@ -638,13 +678,7 @@ __device__ __forceinline__ void interaction(Site<T>& s, const UConst<T>& uc, con
                 }
             }
         } else {
-#pragma unroll 1
-            for (int k = p - 1; k >= 1; --k) {
-                apply_sK(u, wa, kc.az, kc.az2, kc.a1, kc.a6, kc.g2, kc.psi);
-                const T ikk = r[k];
-#pragma unroll
-                for (int j = 0; j < 5; ++j) u[j] = axmi(ikk, wa[j], va[j]);
-            }
+            horner_plain_stages<T>(u, va, kc, r, p - 1);
         }
         if (one_plus_d) {
 #pragma unroll
