@@ -345,12 +345,12 @@ def build_roofline(qlga, prof, ndim, sites, time_steps, precision, order, deg_in
     return roof
 
 
-def default_inner(sites, order):
+def default_inner(sites, order, ndim):
     """Time steps per bench step: about 0.5 s of GPU work for the interleaved ordering; four times as many steps for the
-    plain ordering, whose steps are four times cheaper (and whose first step of every qlga_step call cannot take the band
-    pipeline: its U has not been applied by a previous step)."""
+    plain ordering in 2D / 3D, whose steps are four times cheaper (and whose first step of every qlga_step call cannot
+    take the band pipeline: its U has not been applied by a previous step)."""
     inner = max(1, min(1000, int(6.0e8 / sites)))
-    return min(1000, 4 * inner) if order == "plain" else inner
+    return min(1000, 4 * inner) if (order == "plain" and ndim >= 2) else inner
 
 
 def band_timeline(qlga, sim, torch):
@@ -403,7 +403,7 @@ def run_variant(qlga, torch, dev, local_rank, workload, precision, order, psi_de
     CUDA events on the library's stream, clocks sampled during the timed region, both rooflines."""
     ndim = WORKLOADS[workload]["ndim"]
     sites = int(np.prod(w.dims))
-    inner = default_inner(sites, order.split("+")[0])
+    inner = default_inner(sites, order.split("+")[0], ndim)
     two_launch = order.endswith("+two-launch")     # plain ordering with band mode off (QLGA_OPT_BAND = 0): the comparison
     tag, order = order, order.split("+")[0]
     sim = qlga.Qlga(ndim, w.dims, w.couplings, order=order, precision=precision, device=dev)
@@ -473,7 +473,7 @@ def main():
     lat = tuple(reversed(w.dims)) if ndim == 3 else (ny, nx)        # array shape of one plane
     cfg_tag = (f"BASELINE.json configs[{int(args.workload[3]) - 1}]" if args.workload[3:].isdigit()
                else "SURVEY.md 8(f) row 3, not a BASELINE.json config")
-    inner = args.inner or default_inner(sites, args.order)
+    inner = args.inner or default_inner(sites, args.order, ndim)
     config = {"workload": f"{w.name} ({cfg_tag}): "
                           f"{ndim}D periodic {'x'.join(str(v) for v in w.dims[:max(2, ndim)])}, {args.precision}, "
                           f"{args.order} ordering (eq. {'112' if args.order == 'interleaved' else '108'})",
