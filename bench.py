@@ -395,7 +395,8 @@ VARIANTS = (("cfg5", "f32", "interleaved"), ("cfg5", "f32x", "interleaved"), ("c
             ("cfg5", "f32", "plain"), ("cfg5", "f64", "plain+two-launch"), ("cfg5", "f32", "plain+two-launch"),
             ("cfg3", "f64", "interleaved"), ("cfg3", "f32", "interleaved"),
             ("cfg3", "f64", "plain"), ("cfg3", "f32", "plain"),
-            ("cfg4", "f64", "interleaved"), ("cfg2", "f64", "interleaved"), ("cfg1", "f64", "interleaved"))
+            ("cfg4", "f64", "interleaved"), ("cfg2", "f64", "interleaved"), ("cfg1", "f64", "interleaved"),
+            ("cfg3d", "f64", "interleaved"))
 
 
 def run_variant(qlga, torch, dev, local_rank, workload, precision, order, psi_dev, w, steps, lattice):
