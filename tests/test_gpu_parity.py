@@ -303,6 +303,34 @@ def test_observables_match_oracle(qlga, oracle):
         sim.close()
 
 
+def test_diagnostics_on_ragged_lattices(qlga, oracle):
+    # The shared-memory diagnostics of round 2 -- observables_ring_kernel (units of 128 columns x a segment of rows, loads
+    # staged through a cp.async ring, psi handed to the left neighbour) and vorticity_tile_kernel (tiles of 32 x 8
+    # sites with a one-site halo) -- on lattices smaller than a unit / tile, with ragged last units and tiles, one
+    # row, one column, several segments, in fp64 and fp32, with the previous-state overlap of eq. (85).
+    c = (1.0, 0.3, -0.1)
+    for dims in ((1, 1), (5, 3), (31, 7), (33, 9), (130, 9), (1, 40), (257, 40), (300, 203), (128, 64), (129, 2100)):
+        q0 = inputs.random_spinor_state(dims, seed=17 + dims[0], amplitude=0.3)
+        for precision, rtol, vtol in (("f64", 1e-11, 1e-12), ("f32", 2e-6, 1e-6)):
+            qin = q0 if precision == "f64" else q0.astype(np.complex64)
+            q64 = qin.astype(np.complex128)
+            sim = qlga.Qlga(2, dims, c, precision=precision, keep_previous=True)
+            sim.set_state_q(qin)
+            ob = sim.observables()
+            ref = oracle.observables(q64, 2, c)
+            for k, v in ref.items():
+                if not k.startswith("e_dt"):
+                    assert abs(ob[k] - v) <= rtol * max(1.0, abs(v)), (dims, precision, k)
+            assert np.abs(sim.vorticity() - oracle.vorticity(q64)).max() < vtol, (dims, precision)
+            sim.step(1)
+            q1 = sim.get_state_q().astype(np.complex128)
+            ob = sim.observables()
+            ref = oracle.observables(q1, 2, c, qprev=q64)
+            for k, v in ref.items():
+                assert abs(ob[k] - v) <= (1e-9 if precision == "f64" else 2e-5) * max(1.0, abs(v)), (dims, precision, k)
+            sim.close()
+
+
 def test_psi_roundtrip_and_device_transfers(qlga, oracle):
     import torch
     c = (1.0, 0.3, -0.1)
