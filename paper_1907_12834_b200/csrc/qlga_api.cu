@@ -659,6 +659,7 @@ static void band_release(qlga_ctx* c) {
         for (int k = 0; k < c->band_nev; ++k) cudaEventDestroy(c->band_ev[k]);
         free(c->band_ev); c->band_ev = nullptr; c->band_nev = 0;
     }
+    if (c->d_band) cudaCtxResetPersistingL2Cache();        // the ring's lines go back to normal before its memory is reused
     cudaFree(c->d_band); c->d_band = nullptr; c->band_bytes = 0;
 }
 
