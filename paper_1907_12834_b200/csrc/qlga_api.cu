@@ -648,6 +648,7 @@ static bool band_applies(const qlga_ctx* c) {
 }
 
 static void band_drop_graphs(qlga_ctx* c) {
+    if (c->band_ngraph > 0) cudaStreamSynchronize(c->stream);        // a replay may still be running on the caller's stream
     for (int k = 0; k < c->band_ngraph; ++k) cudaGraphExecDestroy(c->band_graph[k].exec);
     c->band_ngraph = 0;
 }
