@@ -477,7 +477,7 @@ __device__ __forceinline__ void horner_stage_fused(cx<T> u[5], const cx<T> v[5],
 
 // Plain Horner stages k = kfirst .. 1 (u <- v - i r_k sK u) of the path without the spin gauge (fp32).  A one-stage loop
 // cost the fp32 kernels 33 MOVs per 47 packed FP instructions: register-pair copies of the loop-carried (re, im) pairs
-// around the back edge (ptxas).  The degrees that occur in fp32 (kfirst <= 3, i.e. p <= 4) are therefore straight-line
+// around the back edge (ptxas).  The degrees that occur in fp32 (kfirst <= 2, i.e. p <= 3) are therefore straight-line
 // code, every stage writing a fresh vector; higher degrees run two stages per trip with ping-pong vectors.
 template <typename T>
 __device__ __forceinline__ void horner_plain_stage(const cx<T> uin[5], cx<T> uout[5], const cx<T> v[5], const KCoef<T>& kc, T ik) {
@@ -499,13 +499,7 @@ __device__ __forceinline__ void horner_plain_stages(cx<T> u[5], const cx<T> v[5]
         horner_plain_stage<T>(a, b, v, kc, r[1]);
 #pragma unroll
         for (int j = 0; j < 5; ++j) u[j] = b[j];
-    } else if (kfirst == 3) {
-        horner_plain_stage<T>(u, a, v, kc, r[3]);
-        horner_plain_stage<T>(a, b, v, kc, r[2]);
-        horner_plain_stage<T>(b, a, v, kc, r[1]);
-#pragma unroll
-        for (int j = 0; j < 5; ++j) u[j] = a[j];
-    } else if (kfirst > 3) {
+    } else if (kfirst > 2) {
         int k = kfirst;
         if (k & 1) {
             horner_plain_stage<T>(u, a, v, kc, r[k]);
