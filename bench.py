@@ -392,7 +392,7 @@ def band_timeline(qlga, sim, torch):
 # the other precisions / orderings of the headline workload and config 3 (the large 1D lattice), a few bench
 # steps each, so that they are measured by whoever runs bench.py and not only quoted in DESIGN.md
 VARIANTS = (("cfg5", "f32", "interleaved"), ("cfg5", "f32x", "interleaved"), ("cfg5", "f64", "plain"),
-            ("cfg5", "f32", "plain"), ("cfg5", "f64", "plain+two-launch"), ("cfg5", "f32", "plain+two-launch"),
+            ("cfg5", "f32", "plain"), ("cfg5", "f32x", "plain"), ("cfg5", "f64", "plain+two-launch"), ("cfg5", "f32", "plain+two-launch"),
             ("cfg3", "f64", "interleaved"), ("cfg3", "f32", "interleaved"),
             ("cfg3", "f64", "plain"), ("cfg3", "f32", "plain"),
             ("cfg4", "f64", "interleaved"), ("cfg2", "f64", "interleaved"), ("cfg1", "f64", "interleaved"),
